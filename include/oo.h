@@ -1,0 +1,176 @@
+/*
+ * oo.h — C ABI of liboo: batched per-query radiance evaluation of an OctaOctree neural radiosity cache on one
+ * NVIDIA B200 (sm_100a).
+ *
+ * What the library computes (paper: /root/reference/PAPER.md, cited P:line; readings A1-A24 in DESIGN.md §2):
+ * "rendering reduces to standard primary visibility plus one OctaOctree query and one decoder evaluation per visible
+ * shading point".  For each query (position x, normal n, outgoing direction wo[, extras]):
+ *   1. locate the cell containing x at every used octree level (sparse octree);
+ *   2. project wo onto the unfolded octahedron (Eq. 4-5), remap to [0,1]^2, and interpolate that
+ *      cell's directional feature map bilinearly with octahedral border wrap (texel reading of Eq. 6; continuity
+ *      across faces);
+ *   3. concatenate the per-level features (Eq. 11) with the per-query attributes (Eq. 12-13);
+ *   4. decode with a small MLP (hidden width 64, ReLU, no biases) to RGB.
+ * This is the nearest-cell / raw-direction variant that the paper itself names as ablations; see
+ * DESIGN.md §1 for the differences from the full method.
+ *
+ * Conventions
+ *   - Every pointer is marked HOST or DEVICE.  DEVICE pointers must belong to the context's CUDA device.
+ *   - Uploads copy (and re-lay-out) into library-owned device memory; the caller may free its buffers once the
+ *     stream has completed.  A second upload replaces the first.
+ *   - Query and output buffers are owned by the caller.  Kernels are enqueued on the caller's stream (a cudaStream_t
+ *     passed as void*; NULL = the legacy default stream) and the call returns without synchronising, except where
+ *     stated.  Hot calls never allocate (call oo_reserve first if you use oo_sort_queries / oo_query_host).
+ *   - Every call returns oo_status; nothing throws.  oo_last_error() describes the last failure on that context.
+ *   - Not checked per query (result undefined, never a crash): non-finite inputs, wo = 0.  x outside [0,1]^3 is
+ *     clamped componentwise (A16).
+ *   - There is no CPU fallback: without a usable CUDA device oo_create fails.
+ */
+#ifndef OO_H_
+#define OO_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define OO_API __attribute__((visibility("default")))
+#else
+#define OO_API
+#endif
+
+#define OO_MAX_LEVELS 8      /* used levels L */
+#define OO_MAX_DEPTH 16      /* octree depth (root = depth 0) */
+#define OO_MAX_HIDDEN 8      /* hidden layers H */
+#define OO_MAX_EXTRA 10      /* per-query extra scalars appended to the MLP input */
+
+typedef struct oo_ctx oo_ctx; /* opaque; one per device */
+
+typedef enum {
+    OO_OK = 0,
+    OO_ERR_INVALID_ARG = 1, /* null pointer, inconsistent sizes, malformed tree ... (see oo_last_error) */
+    OO_ERR_NOT_READY = 2,   /* tree / MLP not uploaded yet, or MLP input width does not match the tree */
+    OO_ERR_UNSUPPORTED = 3, /* valid request outside what the kernels implement (e.g. width != 64) */
+    OO_ERR_CUDA = 4,        /* a CUDA call failed (also reports an earlier asynchronous fault) */
+    OO_ERR_OOM = 5          /* host or device allocation failed */
+} oo_status;
+
+typedef enum { OO_F16 = 0, OO_F32 = 1 } oo_dtype;
+typedef enum { OO_ACT_NONE = 0, OO_ACT_EXP = 1 } oo_out_act;
+
+/* Which kernels oo_encode / oo_query run.  Every choice computes the same function; all are CUDA. */
+typedef enum {
+    OO_PATH_AUTO = 0,        /* fastest available for the uploaded shapes */
+    OO_PATH_GENERIC = 1,     /* any tree: plain child-table descent; encode -> features in HBM -> MLP kernel */
+    OO_PATH_UNFUSED = 2,     /* hop-table descent, specialised gather; features round-trip HBM; MLP kernel */
+    OO_PATH_FUSED_MMA = 3,   /* one kernel: gather -> shared memory -> mma.sync MLP -> RGB */
+    OO_PATH_FUSED_TC = 4     /* one kernel: gather -> shared memory -> tcgen05.mma (TMEM accumulators) -> RGB */
+} oo_path;
+
+/* The octree and its feature atlases ("every non-empty cell stores a learnable octahedral feature map").
+ * Node 0 is the root (depth 0, the cube [0,1]^3); a node of depth d is a cell of side 2^-d with half-open extent.
+ * Octant index o = bx | by<<1 | bz<<2 (b = 1 for the upper half along that axis).  Used levels are listed coarse to
+ * fine; every existing node at a used depth owns one map: atlas[l][map_slot[node]] is an R_l x R_l array of F-vectors,
+ * row j (v_y) major, column i (v_x) minor, texel centres at ((i+1/2)/R, (j+1/2)/R) of the unfolded octahedron (A2, A3). */
+typedef struct {
+    uint32_t n_nodes;
+    uint32_t max_depth;          /* <= OO_MAX_DEPTH */
+    const int32_t* child;        /* HOST [n_nodes][8]; -1 = absent; a child is one level deeper than its parent */
+    const uint8_t* depth;        /* HOST [n_nodes] */
+    const int32_t* map_slot;     /* HOST [n_nodes]; slot in its level's atlas; -1 where depth is not a used level */
+    uint32_t n_levels;           /* L in 1..OO_MAX_LEVELS */
+    const uint32_t* level_depth; /* HOST [L] strictly increasing, 1 <= depth <= max_depth */
+    const uint32_t* level_res;   /* HOST [L] R_l: power of two, 2 <= R_l <= 256 */
+    const uint32_t* level_slots; /* HOST [L] number of maps in level l (= number of nodes at that depth) */
+    uint32_t n_features;         /* F; F * sizeof(dtype) must be 16, 32 or 64 bytes */
+    oo_dtype dtype;              /* storage type of the texels */
+    const void* const* atlas;    /* HOST array [L] of DEVICE pointers, each [level_slots[l]][R_l][R_l][F], 16-byte aligned */
+} oo_tree_desc;
+
+/* Decoder f_phi: n_hidden x (linear width x in, ReLU), then linear out_dim x width, then out_act.
+ * No biases (A10).  fp16 weights, row-major [out][in].  in_dim must equal L*F + 6 + n_extra of the queries:
+ * input order [h_0 .. h_{L-1} | n | wo | extra] (A7). */
+typedef struct {
+    uint32_t in_dim;
+    uint32_t width;              /* must be 64 */
+    uint32_t n_hidden;           /* 1..OO_MAX_HIDDEN */
+    uint32_t out_dim;            /* 1..8 (3 = RGB) */
+    const void* const* weights;  /* HOST array [n_hidden+1] of HOST pointers to fp16 matrices:
+                                    [width][in_dim], (n_hidden-1) x [width][width], [out_dim][width] */
+    oo_out_act out_act;
+} oo_mlp_desc;
+
+/* A batch of queries.  All arrays packed fp32.  For oo_encode / oo_query / oo_sort_queries they are DEVICE pointers,
+ * for oo_query_host HOST pointers.  Read-only for the library. */
+typedef struct {
+    uint64_t n;
+    const float* x;              /* [n][3] position */
+    const float* nrm;            /* [n][3] surface normal (may be NULL for oo_encode) */
+    const float* wo;             /* [n][3] outgoing direction, need not be normalised (A22), must not be 0 */
+    const float* extra;          /* [n][n_extra] or NULL */
+    uint32_t n_extra;            /* 0..OO_MAX_EXTRA (roughness: 1) */
+    const uint32_t* perm;        /* optional DEVICE [n]: processing order (thread t handles query perm[t]); results are
+                                    always written at the query's own index, i.e. in the caller's order.  NULL = identity */
+} oo_queries;
+
+typedef struct {
+    uint64_t launches;           /* kernels launched by this context so far (all kinds) */
+    uint64_t query_launches;     /* kernels launched by oo_query / oo_encode / oo_sort_queries / oo_query_host */
+    uint64_t node_table_bytes;   /* device bytes of the descent tables */
+    uint64_t atlas_bytes;        /* device bytes of the re-laid-out (border-padded) atlases */
+    uint32_t path_last_query;    /* oo_path actually used by the last oo_query */
+    uint32_t path_last_encode;   /* oo_path actually used by the last oo_encode */
+    uint32_t hop_plan_ok;        /* 1 if the uploaded tree admits the hop-table descent (else only OO_PATH_GENERIC) */
+    uint32_t n_sms;
+} oo_info;
+
+/* Create a context on a CUDA device.  Fails with OO_ERR_CUDA if the device is absent or is not compute capability
+ * 10.x (the kernels are built for sm_100a only). */
+OO_API oo_status oo_create(oo_ctx** out, int cuda_device);
+OO_API void oo_destroy(oo_ctx* ctx);
+/* Message for the last non-OK status on ctx (valid until the next call on ctx); "" if none. */
+OO_API const char* oo_last_error(const oo_ctx* ctx);
+
+/* Validate the tree (child indices in range and one level deeper, depth consistent, map_slot unique per level and
+ * < level_slots), build the descent tables, and copy every atlas into library-owned border-padded maps
+ * ((R+2)^2 texels per map, the one-texel border filled by the octahedral wrap).  Synchronises the stream. */
+OO_API oo_status oo_upload_tree(oo_ctx* ctx, const oo_tree_desc* tree, void* cuda_stream);
+/* Copy the decoder weights into the library's padded shared-memory image.  Synchronises the stream. */
+OO_API oo_status oo_upload_mlp(oo_ctx* ctx, const oo_mlp_desc* mlp, void* cuda_stream);
+/* Pre-allocate scratch for up to max_queries (sort keys/buffers, staging for oo_query_host). */
+OO_API oo_status oo_reserve(oo_ctx* ctx, uint64_t max_queries);
+/* Select the kernels used from now on (default OO_PATH_AUTO).  OO_ERR_UNSUPPORTED at query time if the uploaded
+ * shapes have no such kernel. */
+OO_API oo_status oo_set_path(oo_ctx* ctx, oo_path path);
+OO_API oo_status oo_get_info(const oo_ctx* ctx, oo_info* out);
+
+/* Row a1: d_perm_out[k] = index of the k-th query in ascending order of the 30-bit Morton key of
+ * clamp(floor(x*1024), 0, 1023) (bit b of q_x -> key bit 3b, q_y -> 3b+1, q_z -> 3b+2), ties in original order
+ * (stable).  d_perm_out: DEVICE [n].  Needs oo_reserve(n). */
+OO_API oo_status oo_sort_queries(oo_ctx* ctx, const oo_queries* q, uint32_t* d_perm_out, void* cuda_stream);
+
+/* Steps 1-3 only.  d_features: DEVICE [n][L*F] in the tree's dtype (fp32 accumulate, one rounding on store).
+ * Optional debug outputs: d_slot DEVICE [n][L] (atlas slot per level, -1 = no cell at that level, whose features are
+ * then 0, A17); d_texel DEVICE [n][L][2] = base texel (i0, j0) before wrapping, each in [-1, R_l-1], decided in fp32 by
+ * the fixed sequence of DESIGN.md "Index contract".  q->nrm and q->extra are ignored. */
+OO_API oo_status oo_encode(oo_ctx* ctx, const oo_queries* q, void* d_features, int32_t* d_slot, int16_t* d_texel,
+                    void* cuda_stream);
+
+/* The whole path.  d_rgb: DEVICE [n][out_dim] fp32, written at each query's own index. */
+OO_API oo_status oo_query(oo_ctx* ctx, const oo_queries* q, float* d_rgb, void* cuda_stream);
+
+/* The whole path from HOST buffers: copies the queries to the device (cudaMemcpyAsync on the stream), runs oo_query,
+ * copies RGB back to h_rgb (HOST [n][out_dim]) and synchronises the stream.  q->perm must be NULL.  Pinned host
+ * memory makes the copies asynchronous; pageable memory works.  Needs oo_reserve(n). */
+OO_API oo_status oo_query_host(oo_ctx* ctx, const oo_queries* q, float* h_rgb, void* cuda_stream);
+
+/* Debug read-back of the library's re-laid-out atlas: copies the padded map of (level, slot) to HOST
+ * h_out [(R+2)][(R+2)][F] in the tree's dtype.  Synchronous. */
+OO_API oo_status oo_read_padded_map(oo_ctx* ctx, uint32_t level, uint32_t slot, void* h_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* OO_H_ */

@@ -1,0 +1,242 @@
+"""ctypes binding of liboo (include/oo.h): same names, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import List, Optional, Sequence
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "liboo.so")
+
+PATH_AUTO, PATH_GENERIC, PATH_UNFUSED, PATH_FUSED_MMA, PATH_FUSED_TC = 0, 1, 2, 3, 4
+OO_F16, OO_F32 = 0, 1
+OO_ACT_NONE, OO_ACT_EXP = 0, 1
+_STATUS = {0: "OO_OK", 1: "OO_ERR_INVALID_ARG", 2: "OO_ERR_NOT_READY", 3: "OO_ERR_UNSUPPORTED", 4: "OO_ERR_CUDA", 5: "OO_ERR_OOM"}
+
+EXPORTED_SYMBOLS = ["oo_create", "oo_destroy", "oo_last_error", "oo_upload_tree", "oo_upload_mlp", "oo_reserve", "oo_set_path",
+                    "oo_get_info", "oo_sort_queries", "oo_encode", "oo_query", "oo_query_host", "oo_read_padded_map"]
+
+
+class OOError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__("%s: %s" % (_STATUS.get(status, str(status)), msg))
+        self.status = status
+
+
+class _TreeDesc(C.Structure):
+    _fields_ = [("n_nodes", C.c_uint32), ("max_depth", C.c_uint32), ("child", C.c_void_p), ("depth", C.c_void_p),
+                ("map_slot", C.c_void_p), ("n_levels", C.c_uint32), ("level_depth", C.c_void_p), ("level_res", C.c_void_p),
+                ("level_slots", C.c_void_p), ("n_features", C.c_uint32), ("dtype", C.c_int), ("atlas", C.c_void_p)]
+
+
+class _MlpDesc(C.Structure):
+    _fields_ = [("in_dim", C.c_uint32), ("width", C.c_uint32), ("n_hidden", C.c_uint32), ("out_dim", C.c_uint32),
+                ("weights", C.c_void_p), ("out_act", C.c_int)]
+
+
+class _Queries(C.Structure):
+    _fields_ = [("n", C.c_uint64), ("x", C.c_void_p), ("nrm", C.c_void_p), ("wo", C.c_void_p), ("extra", C.c_void_p),
+                ("n_extra", C.c_uint32), ("perm", C.c_void_p)]
+
+
+class _Info(C.Structure):
+    _fields_ = [("launches", C.c_uint64), ("query_launches", C.c_uint64), ("node_table_bytes", C.c_uint64),
+                ("atlas_bytes", C.c_uint64), ("path_last_query", C.c_uint32), ("path_last_encode", C.c_uint32),
+                ("hop_plan_ok", C.c_uint32), ("n_sms", C.c_uint32)]
+
+
+_lib = None
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """Load liboo.so.  Fails loudly if it has not been built (python -m paper_2606_08469_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise OOError(4, "liboo.so is not built (%s); run `python -m paper_2606_08469_b200.build` — there is no CPU fallback" % _LIB_PATH)
+    L = C.CDLL(_LIB_PATH)
+    vp, u64, u32 = C.c_void_p, C.c_uint64, C.c_uint32
+    L.oo_create.argtypes = [C.POINTER(vp), C.c_int]
+    L.oo_destroy.argtypes = [vp]
+    L.oo_destroy.restype = None
+    L.oo_last_error.argtypes = [vp]
+    L.oo_last_error.restype = C.c_char_p
+    L.oo_upload_tree.argtypes = [vp, C.POINTER(_TreeDesc), vp]
+    L.oo_upload_mlp.argtypes = [vp, C.POINTER(_MlpDesc), vp]
+    L.oo_reserve.argtypes = [vp, u64]
+    L.oo_set_path.argtypes = [vp, C.c_int]
+    L.oo_get_info.argtypes = [vp, C.POINTER(_Info)]
+    L.oo_sort_queries.argtypes = [vp, C.POINTER(_Queries), vp, vp]
+    L.oo_encode.argtypes = [vp, C.POINTER(_Queries), vp, vp, vp, vp]
+    L.oo_query.argtypes = [vp, C.POINTER(_Queries), vp, vp]
+    L.oo_query_host.argtypes = [vp, C.POINTER(_Queries), vp, vp]
+    L.oo_read_padded_map.argtypes = [vp, u32, u32, vp]
+    for name in EXPORTED_SYMBOLS:
+        if name not in ("oo_destroy", "oo_last_error"):
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _np_ptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+class OctaOctree:
+    """One context on one CUDA device.  Methods mirror the C entry points (oo_upload_tree, oo_upload_mlp, oo_encode,
+    oo_query, oo_sort_queries, oo_query_host); tensors are torch CUDA tensors, trees/weights are numpy arrays."""
+
+    def __init__(self, device: int = 0):
+        import torch  # device memory and streams only
+        self._torch = torch
+        self._L = load_library()
+        self._ctx = C.c_void_p()
+        st = self._L.oo_create(C.byref(self._ctx), device)
+        if st:
+            raise OOError(st, "oo_create(device=%d) failed: needs a CUDA device of compute capability 10.x (B200); there is no CPU fallback" % device)
+        self.device = torch.device("cuda", device)
+        self.n_levels = self.n_features = 0
+        self.dtype = None
+        self.out_dim = 3
+
+    def close(self):
+        if self._ctx:
+            self._L.oo_destroy(self._ctx)
+            self._ctx = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st: int):
+        if st:
+            raise OOError(st, self._L.oo_last_error(self._ctx).decode())
+
+    def _stream(self):
+        return C.c_void_p(self._torch.cuda.current_stream(self.device).cuda_stream)
+
+    # ---------------------------------------------------------------- uploads
+    def oo_upload_tree(self, tree, atlas_levels: Sequence, dtype: str):
+        """tree: object with n_nodes, max_depth, child, depth, map_slot, level_depth, level_res, level_slots (numpy / lists).
+        atlas_levels: per level a numpy array or a torch CUDA tensor [slots][R][R][F]."""
+        import numpy as np
+        torch = self._torch
+        child = np.ascontiguousarray(tree.child, np.int32)
+        depth = np.ascontiguousarray(tree.depth, np.uint8)
+        slot = np.ascontiguousarray(tree.map_slot, np.int32)
+        ld = np.ascontiguousarray(tree.level_depth, np.uint32)
+        lr = np.ascontiguousarray(tree.level_res, np.uint32)
+        ls = np.ascontiguousarray(tree.level_slots, np.uint32)
+        tdt = {"f16": torch.float16, "f32": torch.float32}[dtype]
+        dev = []
+        for a in atlas_levels:
+            t = a if isinstance(a, torch.Tensor) else torch.from_numpy(np.ascontiguousarray(a))
+            t = t.to(device=self.device, dtype=tdt).contiguous()
+            dev.append(t)
+        F = int(dev[0].shape[-1])
+        ptrs = (C.c_void_p * len(dev))(*[t.data_ptr() if t.numel() else None for t in dev])
+        d = _TreeDesc(child.shape[0], int(tree.max_depth), _np_ptr(child), _np_ptr(depth), _np_ptr(slot), len(dev), _np_ptr(ld),
+                      _np_ptr(lr), _np_ptr(ls), F, OO_F16 if dtype == "f16" else OO_F32, C.cast(ptrs, C.c_void_p))
+        self._check(self._L.oo_upload_tree(self._ctx, C.byref(d), self._stream()))
+        self.n_levels, self.n_features, self.dtype = len(dev), F, dtype
+        del dev
+
+    def oo_upload_mlp(self, weights: Sequence, out_act: str = "exp"):
+        import numpy as np
+        ws = [np.ascontiguousarray(w, np.float16) for w in weights]
+        ptrs = (C.c_void_p * len(ws))(*[w.ctypes.data for w in ws])
+        d = _MlpDesc(ws[0].shape[1], ws[0].shape[0], len(ws) - 1, ws[-1].shape[0], C.cast(ptrs, C.c_void_p),
+                     {"none": OO_ACT_NONE, "exp": OO_ACT_EXP}[out_act])
+        self._check(self._L.oo_upload_mlp(self._ctx, C.byref(d), self._stream()))
+        self.out_dim = int(ws[-1].shape[0])
+
+    def oo_reserve(self, n: int):
+        self._check(self._L.oo_reserve(self._ctx, int(n)))
+
+    def oo_set_path(self, path: int):
+        self._check(self._L.oo_set_path(self._ctx, int(path)))
+
+    def oo_get_info(self) -> dict:
+        info = _Info()
+        self._check(self._L.oo_get_info(self._ctx, C.byref(info)))
+        return {k: int(getattr(info, k)) for k, _ in _Info._fields_}
+
+    # ---------------------------------------------------------------- queries
+    def _queries(self, x, nrm, wo, extra, perm):
+        torch = self._torch
+        for t in (x, nrm, wo, extra, perm):
+            if t is not None:
+                assert t.is_cuda and t.is_contiguous(), "queries must be contiguous CUDA tensors"
+        assert x.dtype == torch.float32 and wo.dtype == torch.float32
+        n = int(x.shape[0])
+        ne = 0 if extra is None else int(extra.numel() // max(n, 1))
+        q = _Queries(n, x.data_ptr(), nrm.data_ptr() if nrm is not None else None, wo.data_ptr(),
+                     extra.data_ptr() if extra is not None else None, ne, perm.data_ptr() if perm is not None else None)
+        return q, n
+
+    def oo_sort_queries(self, x, perm_out=None):
+        torch = self._torch
+        n = int(x.shape[0])
+        if perm_out is None:
+            perm_out = torch.empty(n, dtype=torch.int32, device=self.device)
+        q = _Queries(n, x.data_ptr(), None, x.data_ptr(), None, 0, None)
+        self._check(self._L.oo_sort_queries(self._ctx, C.byref(q), C.c_void_p(perm_out.data_ptr()), self._stream()))
+        return perm_out
+
+    def oo_encode(self, x, wo, perm=None, features=None, want_debug: bool = False):
+        torch = self._torch
+        q, n = self._queries(x, None, wo, None, perm)
+        LF = self.n_levels * self.n_features
+        if features is None:
+            features = torch.empty((n, LF), dtype=torch.float16 if self.dtype == "f16" else torch.float32, device=self.device)
+        slot = texel = None
+        if want_debug:
+            slot = torch.empty((n, self.n_levels), dtype=torch.int32, device=self.device)
+            texel = torch.empty((n, self.n_levels, 2), dtype=torch.int16, device=self.device)
+        self._check(self._L.oo_encode(self._ctx, C.byref(q), C.c_void_p(features.data_ptr()),
+                                      C.c_void_p(slot.data_ptr()) if want_debug else None,
+                                      C.c_void_p(texel.data_ptr()) if want_debug else None, self._stream()))
+        return (features, slot, texel) if want_debug else features
+
+    def oo_query(self, x, nrm, wo, extra=None, perm=None, rgb=None):
+        torch = self._torch
+        q, n = self._queries(x, nrm, wo, extra, perm)
+        if rgb is None:
+            rgb = torch.empty((n, self.out_dim), dtype=torch.float32, device=self.device)
+        self._check(self._L.oo_query(self._ctx, C.byref(q), C.c_void_p(rgb.data_ptr()), self._stream()))
+        return rgb
+
+    def oo_query_host(self, x, nrm, wo, extra=None, rgb=None):
+        """x, nrm, wo, extra, rgb: CPU tensors (pinned for asynchronous copies) or numpy arrays.  Synchronous."""
+        torch = self._torch
+        n = int(x.shape[0])
+
+        def ptr(a):
+            if a is None:
+                return None
+            return a.data_ptr() if isinstance(a, torch.Tensor) else a.ctypes.data
+        ne = 0 if extra is None else int((extra.numel() if isinstance(extra, torch.Tensor) else extra.size) // max(n, 1))
+        if rgb is None:
+            rgb = torch.empty((n, self.out_dim), dtype=torch.float32).pin_memory()
+        q = _Queries(n, ptr(x), ptr(nrm), ptr(wo), ptr(extra), ne, None)
+        self._check(self._L.oo_query_host(self._ctx, C.byref(q), C.c_void_p(ptr(rgb)), self._stream()))
+        return rgb
+
+    def oo_read_padded_map(self, level: int, slot: int, R: int):
+        import numpy as np
+        out = np.empty((R + 2, R + 2, self.n_features), np.float16 if self.dtype == "f16" else np.float32)
+        self._check(self._L.oo_read_padded_map(self._ctx, level, slot, _np_ptr(out)))
+        return out
+
+    # convenience: upload a gen.Workload
+    def upload_workload(self, w):
+        self.oo_upload_tree(w.tree, w.atlas.levels, w.atlas.dtype)
+        self.oo_upload_mlp(w.mlp.weights, w.mlp.out_act)
+        return self

@@ -1,0 +1,617 @@
+// oo_api.cu — host side of liboo: the C ABI of include/oo.h.  Owns the device layouts (border-padded level-major
+// atlases, dense + hop descent tables, the padded decoder image), validates what is uploaded, and dispatches kernels.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "oo_internal.h"
+
+using namespace oo;
+
+struct oo_ctx {
+    int device = 0;
+    int n_sms = 148;
+    std::string err;
+    cudaError_t sticky = cudaSuccess;
+    oo_path path = OO_PATH_AUTO;
+    oo_info info{};
+
+    // tree
+    bool have_tree = false;
+    bool plan_ok = false;
+    uint32_t tree_max_depth = 0;
+    TreeParams T{};
+    std::vector<void*> atlas_dev;          // library-owned padded atlases (unshifted base pointers)
+    std::vector<uint64_t> level_slots;
+    void* d_dense = nullptr;
+    std::vector<void*> d_hop;
+    void* d_child = nullptr;
+    void* d_map_slot = nullptr;
+
+    // mlp
+    bool have_mlp = false;
+    MlpParams M{};
+    void* d_image = nullptr;
+
+    // scratch
+    uint64_t reserved = 0;
+    void* d_feat = nullptr;    uint64_t feat_bytes = 0;
+    uint32_t *d_keys_a = nullptr, *d_keys_b = nullptr, *d_idx_a = nullptr, *d_hist = nullptr;
+    float *d_qx = nullptr, *d_qn = nullptr, *d_qw = nullptr, *d_qe = nullptr, *d_rgb = nullptr;
+};
+
+namespace {
+
+oo_status fail(oo_ctx* c, oo_status st, const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    if (c) c->err = buf;
+    return st;
+}
+
+#define OO_CUDA(c, call)                                                                                      \
+    do {                                                                                                      \
+        cudaError_t e_ = (call);                                                                              \
+        if (e_ != cudaSuccess) {                                                                              \
+            (c)->sticky = e_;                                                                                 \
+            return fail((c), e_ == cudaErrorMemoryAllocation ? OO_ERR_OOM : OO_ERR_CUDA, "%s: %s", #call,     \
+                        cudaGetErrorString(e_));                                                              \
+        }                                                                                                     \
+    } while (0)
+
+struct DeviceGuard {
+    int prev = -1;
+    explicit DeviceGuard(int dev) {
+        cudaGetDevice(&prev);
+        if (prev != dev) cudaSetDevice(dev);
+        else prev = -1;
+    }
+    ~DeviceGuard() {
+        if (prev >= 0) cudaSetDevice(prev);
+    }
+};
+
+void free_dev(void*& p) {
+    if (p) cudaFree(p);
+    p = nullptr;
+}
+
+void free_tree(oo_ctx* c) {
+    for (void*& p : c->atlas_dev) free_dev(p);
+    c->atlas_dev.clear();
+    for (void*& p : c->d_hop) free_dev(p);
+    c->d_hop.clear();
+    free_dev(c->d_dense);
+    free_dev(c->d_child);
+    free_dev(c->d_map_slot);
+    c->have_tree = false;
+    c->plan_ok = false;
+    c->info.node_table_bytes = c->info.atlas_bytes = 0;
+}
+
+void free_scratch(oo_ctx* c) {
+    free_dev(c->d_feat);
+    c->feat_bytes = 0;
+    void** ps[] = {(void**)&c->d_keys_a, (void**)&c->d_keys_b, (void**)&c->d_idx_a, (void**)&c->d_hist, (void**)&c->d_qx,
+                   (void**)&c->d_qn,     (void**)&c->d_qw,     (void**)&c->d_qe,    (void**)&c->d_rgb};
+    for (void** p : ps) free_dev(*p);
+    c->reserved = 0;
+}
+
+bool is_pow2(uint32_t v) { return v && !(v & (v - 1)); }
+
+oo_status check_async(oo_ctx* c) {
+    if (c->sticky != cudaSuccess) return fail(c, OO_ERR_CUDA, "earlier CUDA failure: %s", cudaGetErrorString(c->sticky));
+    cudaError_t e = cudaPeekAtLastError();
+    if (e != cudaSuccess) {
+        c->sticky = e;
+        return fail(c, OO_ERR_CUDA, "asynchronous CUDA failure: %s", cudaGetErrorString(e));
+    }
+    return OO_OK;
+}
+
+oo_status check_queries(oo_ctx* c, const oo_queries* q, bool need_nrm) {
+    if (!q) return fail(c, OO_ERR_INVALID_ARG, "queries is NULL");
+    if (q->n == 0) return OO_OK;
+    if (!q->x || !q->wo) return fail(c, OO_ERR_INVALID_ARG, "queries.x / queries.wo is NULL");
+    if (need_nrm && !q->nrm) return fail(c, OO_ERR_INVALID_ARG, "queries.nrm is NULL");
+    if (q->n_extra > OO_MAX_EXTRA) return fail(c, OO_ERR_INVALID_ARG, "n_extra %u > %d", q->n_extra, OO_MAX_EXTRA);
+    if (need_nrm && q->n_extra && !q->extra) return fail(c, OO_ERR_INVALID_ARG, "n_extra > 0 but queries.extra is NULL");
+    if (q->n >= (1ull << 32)) return fail(c, OO_ERR_UNSUPPORTED, "more than 2^32-1 queries per call");
+    return OO_OK;
+}
+
+QueryParams make_qp(const oo_queries* q) {
+    QueryParams Q{};
+    Q.n = q->n; Q.x = q->x; Q.nrm = q->nrm; Q.wo = q->wo; Q.extra = q->extra; Q.n_extra = q->n_extra; Q.perm = q->perm;
+    return Q;
+}
+
+void count(oo_ctx* c, int launches) {
+    if (launches > 0) {
+        c->info.launches += (uint64_t)launches;
+        c->info.query_launches += (uint64_t)launches;
+    }
+}
+
+}  // namespace
+
+// =====================================================================================================================
+
+extern "C" OO_API oo_status oo_create(oo_ctx** out, int cuda_device) {
+    if (!out) return OO_ERR_INVALID_ARG;
+    *out = nullptr;
+    oo_ctx* c = new (std::nothrow) oo_ctx();
+    if (!c) return OO_ERR_OOM;
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || cuda_device < 0 || cuda_device >= n) {
+        delete c;
+        return OO_ERR_CUDA;
+    }
+    cudaDeviceProp prop{};
+    e = cudaGetDeviceProperties(&prop, cuda_device);
+    if (e != cudaSuccess || prop.major != 10) {   // kernels are sm_100a only
+        delete c;
+        return OO_ERR_CUDA;
+    }
+    c->device = cuda_device;
+    c->n_sms = prop.multiProcessorCount;
+    c->info.n_sms = (uint32_t)c->n_sms;
+    *out = c;
+    return OO_OK;
+}
+
+extern "C" OO_API void oo_destroy(oo_ctx* c) {
+    if (!c) return;
+    {
+        DeviceGuard g(c->device);
+        free_tree(c);
+        free_dev(c->d_image);
+        free_scratch(c);
+    }
+    delete c;
+}
+
+extern "C" OO_API const char* oo_last_error(const oo_ctx* c) { return c ? c->err.c_str() : "context is NULL"; }
+
+extern "C" OO_API oo_status oo_set_path(oo_ctx* c, oo_path path) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if ((int)path < 0 || (int)path > (int)OO_PATH_FUSED_TC) return fail(c, OO_ERR_INVALID_ARG, "unknown path %d", (int)path);
+    c->path = path;
+    return OO_OK;
+}
+
+extern "C" OO_API oo_status oo_get_info(const oo_ctx* c, oo_info* out) {
+    if (!c || !out) return OO_ERR_INVALID_ARG;
+    *out = c->info;
+    out->hop_plan_ok = c->plan_ok ? 1u : 0u;
+    return OO_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// oo_upload_tree
+// ---------------------------------------------------------------------------------------------------------------------
+extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, void* cuda_stream) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (!t) return fail(c, OO_ERR_INVALID_ARG, "tree is NULL");
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    DeviceGuard g(c->device);
+    // ---- validate the description
+    if (t->n_nodes == 0 || !t->child || !t->depth || !t->map_slot) return fail(c, OO_ERR_INVALID_ARG, "empty tree or NULL node arrays");
+    if (t->max_depth == 0 || t->max_depth > OO_MAX_DEPTH) return fail(c, OO_ERR_INVALID_ARG, "max_depth %u outside 1..%d", t->max_depth, OO_MAX_DEPTH);
+    if (t->n_levels == 0 || t->n_levels > OO_MAX_LEVELS) return fail(c, OO_ERR_INVALID_ARG, "n_levels %u outside 1..%d", t->n_levels, OO_MAX_LEVELS);
+    if (!t->level_depth || !t->level_res || !t->level_slots || !t->atlas) return fail(c, OO_ERR_INVALID_ARG, "NULL level arrays");
+    if (t->dtype != OO_F16 && t->dtype != OO_F32) return fail(c, OO_ERR_INVALID_ARG, "unknown dtype");
+    const uint32_t esize = t->dtype == OO_F32 ? 4 : 2;
+    const uint32_t texel_bytes = t->n_features * esize;
+    if (texel_bytes != 16 && texel_bytes != 32 && texel_bytes != 64)
+        return fail(c, OO_ERR_INVALID_ARG, "F*sizeof(dtype) = %u bytes; must be 16, 32 or 64", texel_bytes);
+    const uint32_t L = t->n_levels;
+    for (uint32_t l = 0; l < L; ++l) {
+        if (t->level_depth[l] < 1 || t->level_depth[l] > t->max_depth) return fail(c, OO_ERR_INVALID_ARG, "level_depth[%u] = %u outside 1..max_depth", l, t->level_depth[l]);
+        if (l && t->level_depth[l] <= t->level_depth[l - 1]) return fail(c, OO_ERR_INVALID_ARG, "level_depth must be strictly increasing");
+        if (!is_pow2(t->level_res[l]) || t->level_res[l] < 2 || t->level_res[l] > 256) return fail(c, OO_ERR_INVALID_ARG, "level_res[%u] = %u: need a power of two in 2..256", l, t->level_res[l]);
+        if (t->level_slots[l] && !t->atlas[l]) return fail(c, OO_ERR_INVALID_ARG, "atlas[%u] is NULL", l);
+        if (((uintptr_t)t->atlas[l]) & 15) return fail(c, OO_ERR_INVALID_ARG, "atlas[%u] is not 16-byte aligned", l);
+    }
+    // ---- validate the nodes; per-depth local indices (used depth: map_slot; otherwise running count)
+    const uint32_t N = t->n_nodes, D = t->max_depth;
+    int level_of_depth[OO_MAX_DEPTH + 1];
+    for (uint32_t d = 0; d <= D; ++d) level_of_depth[d] = -1;
+    for (uint32_t l = 0; l < L; ++l) level_of_depth[t->level_depth[l]] = (int)l;
+    if (t->depth[0] != 0) return fail(c, OO_ERR_INVALID_ARG, "node 0 must be the root (depth 0)");
+    std::vector<int32_t> local(N);
+    std::vector<uint32_t> depth_count(D + 1, 0);
+    std::vector<std::vector<uint8_t>> seen(L);
+    for (uint32_t l = 0; l < L; ++l) seen[l].assign(t->level_slots[l], 0);
+    std::vector<uint8_t> has_parent(N, 0);
+    for (uint32_t i = 0; i < N; ++i) {
+        const uint32_t d = t->depth[i];
+        if (d > D) return fail(c, OO_ERR_INVALID_ARG, "node %u: depth %u > max_depth", i, d);
+        if (i && d == 0) return fail(c, OO_ERR_INVALID_ARG, "node %u: a second root", i);
+        const int l = level_of_depth[d];
+        if (l >= 0) {
+            const int32_t s = t->map_slot[i];
+            if (s < 0 || (uint32_t)s >= t->level_slots[l]) return fail(c, OO_ERR_INVALID_ARG, "node %u: map_slot %d outside level %d (%u slots)", i, s, l, t->level_slots[l]);
+            if (seen[l][s]) return fail(c, OO_ERR_INVALID_ARG, "node %u: map_slot %d used twice in level %d", i, s, l);
+            seen[l][s] = 1;
+            local[i] = s;
+        } else {
+            if (t->map_slot[i] != -1) return fail(c, OO_ERR_INVALID_ARG, "node %u: map_slot must be -1 at an unused depth", i);
+            local[i] = (int32_t)depth_count[d];
+        }
+        depth_count[d]++;
+        for (int o = 0; o < 8; ++o) {
+            const int32_t ch = t->child[(size_t)i * 8 + o];
+            if (ch == -1) continue;
+            if (ch <= 0 || (uint32_t)ch >= N) return fail(c, OO_ERR_INVALID_ARG, "node %u: child %d out of range", i, ch);
+            if (t->depth[ch] != d + 1) return fail(c, OO_ERR_INVALID_ARG, "node %u (depth %u): child %d has depth %u", i, d, ch, (uint32_t)t->depth[ch]);
+            if (has_parent[ch]) return fail(c, OO_ERR_INVALID_ARG, "node %d has two parents", ch);
+            has_parent[ch] = 1;
+        }
+    }
+    for (uint32_t i = 1; i < N; ++i)
+        if (!has_parent[i]) return fail(c, OO_ERR_INVALID_ARG, "node %u is unreachable", i);
+
+    // ---- replace the previous tree
+    free_tree(c);
+    TreeParams T{};
+    T.n_levels = L; T.F = t->n_features; T.f32 = t->dtype == OO_F32; T.texel_bytes = texel_bytes;
+    T.depth_eff = t->level_depth[L - 1];
+    T.scale_eff = (float)(1u << T.depth_eff);
+    c->tree_max_depth = D;
+    c->level_slots.assign(t->level_slots, t->level_slots + L);
+
+    // ---- atlases: padded copies
+    c->atlas_dev.assign(L, nullptr);
+    uint64_t atlas_bytes = 0;
+    int launches = 0;
+    for (uint32_t l = 0; l < L; ++l) {
+        const uint32_t R = t->level_res[l], Rp = R + 2;
+        const uint64_t slots = std::max<uint64_t>(t->level_slots[l], 1);      // at least one (zero) map, so that the branch-free gather has an address
+        const uint64_t bytes = slots * Rp * Rp * texel_bytes;
+        OO_CUDA(c, cudaMalloc(&c->atlas_dev[l], bytes));
+        atlas_bytes += bytes;
+        if (t->level_slots[l] == 0) OO_CUDA(c, cudaMemsetAsync(c->atlas_dev[l], 0, bytes, stream));
+        else launches += launch_pad_atlas(t->atlas[l], c->atlas_dev[l], t->level_slots[l], R, texel_bytes, stream);
+        LevelParams& lv = T.lv[l];
+        lv.atlas = (const uint8_t*)c->atlas_dev[l] + (uint64_t)(Rp + 1) * texel_bytes;
+        lv.half_r = 0.5f * (float)R;
+        lv.off = 0.5f * (float)R - 0.5f;
+        lv.R = R; lv.Rp = Rp;
+        lv.map_bytes = Rp * Rp * texel_bytes;
+        lv.row_bytes = Rp * texel_bytes;
+        lv.depth = t->level_depth[l];
+        lv.shift = T.depth_eff - lv.depth;
+    }
+    c->info.atlas_bytes = atlas_bytes;
+
+    // ---- plain tables for the generic kernels
+    uint64_t table_bytes = 0;
+    OO_CUDA(c, cudaMalloc(&c->d_child, (size_t)N * 8 * 4));
+    OO_CUDA(c, cudaMalloc(&c->d_map_slot, (size_t)N * 4));
+    OO_CUDA(c, cudaMemcpyAsync(c->d_child, t->child, (size_t)N * 8 * 4, cudaMemcpyHostToDevice, stream));
+    OO_CUDA(c, cudaMemcpyAsync(c->d_map_slot, t->map_slot, (size_t)N * 4, cudaMemcpyHostToDevice, stream));
+    table_bytes += (uint64_t)N * 36;
+    T.child = (const int32_t*)c->d_child;
+    T.map_slot = (const int32_t*)c->d_map_slot;
+
+    // ---- hop plan.  Stations: dense tables for every used depth <= Td and for Td = min(4, depth_eff) itself; each used
+    // level deeper than Td must be within 3 depths of the previous station (else only the generic path is available).
+    const uint32_t Td = std::min<uint32_t>(4, T.depth_eff);
+    bool plan_ok = true;
+    {
+        uint32_t prev = Td;
+        for (uint32_t l = 0; l < L; ++l) {
+            const uint32_t d = t->level_depth[l];
+            if (d <= Td) continue;
+            if (d - prev > 3) plan_ok = false;
+            prev = d;
+        }
+    }
+    std::vector<std::vector<int32_t>> hop_host;    // kept alive until the stream sync below
+    std::vector<int32_t> dense;
+    if (plan_ok) {
+        // node ids per depth and the integer cell coordinates of every node (by walking from the root)
+        std::vector<uint32_t> cx(N), cy(N), cz(N);
+        std::vector<std::vector<uint32_t>> by_depth(D + 1);
+        cx[0] = cy[0] = cz[0] = 0;
+        // parents precede children is NOT required by the ABI: do a BFS
+        std::vector<uint32_t> queue;
+        queue.reserve(N);
+        queue.push_back(0);
+        for (size_t h = 0; h < queue.size(); ++h) {
+            const uint32_t i = queue[h];
+            by_depth[t->depth[i]].push_back(i);
+            for (int o = 0; o < 8; ++o) {
+                const int32_t ch = t->child[(size_t)i * 8 + o];
+                if (ch < 0) continue;
+                cx[ch] = cx[i] * 2 + (o & 1); cy[ch] = cy[i] * 2 + ((o >> 1) & 1); cz[ch] = cz[i] * 2 + ((o >> 2) & 1);
+                queue.push_back((uint32_t)ch);
+            }
+        }
+        auto add_dense = [&](uint32_t d) -> uint32_t {
+            const uint32_t off = (uint32_t)dense.size();
+            dense.resize(off + (1u << (3 * d)), -1);
+            for (uint32_t i : by_depth[d]) dense[off + ((cz[i] << (2 * d)) | (cy[i] << d) | cx[i])] = local[i];
+            return off;
+        };
+        bool t_done = false;
+        for (uint32_t l = 0; l < L; ++l) {
+            LevelParams& lv = T.lv[l];
+            if (lv.depth <= Td) {
+                lv.dense = 1;
+                lv.dense_off = add_dense(lv.depth);
+                if (lv.depth == Td) { T.t_dense_off = lv.dense_off; t_done = true; }
+            }
+        }
+        if (!t_done) T.t_dense_off = add_dense(Td);
+        T.t_depth = Td;
+        T.t_shift = T.depth_eff - Td;
+        while (dense.size() % 4) dense.push_back(-1);
+        T.dense_ints = (uint32_t)dense.size();
+        OO_CUDA(c, cudaMalloc(&c->d_dense, dense.size() * 4));
+        OO_CUDA(c, cudaMemcpyAsync(c->d_dense, dense.data(), dense.size() * 4, cudaMemcpyHostToDevice, stream));
+        T.dense = (const int32_t*)c->d_dense;
+        table_bytes += dense.size() * 4;
+        // hop tables
+        uint32_t prev_depth = Td;
+        for (uint32_t l = 0; l < L; ++l) {
+            LevelParams& lv = T.lv[l];
+            if (lv.depth <= Td) continue;
+            const uint32_t gdep = lv.depth - prev_depth;
+            lv.dense = 0;
+            lv.gap = gdep;
+            // one row of 8^gap entries per local index at the previous station (a used level's local index is its
+            // map_slot, which ranges over level_slots; an unused depth's is a running count over its nodes)
+            size_t rows = std::max<size_t>(by_depth[prev_depth].size(), 1);
+            const int pl = level_of_depth[prev_depth];
+            if (pl >= 0) rows = std::max<size_t>(t->level_slots[pl], 1);
+            hop_host.emplace_back(rows << (3 * gdep), -1);
+            std::vector<int32_t>& tab = hop_host.back();
+            const uint32_t m = (1u << gdep) - 1;
+            // for every node at the previous station enumerate its descendants `gap` levels below
+            std::vector<std::pair<uint32_t, uint32_t>> frontier, next;   // (node, ancestor local index)
+            for (uint32_t a : by_depth[prev_depth]) frontier.emplace_back(a, (uint32_t)local[a]);
+            for (uint32_t s = 0; s < gdep; ++s) {
+                next.clear();
+                for (auto& pr : frontier)
+                    for (int o = 0; o < 8; ++o) {
+                        const int32_t ch = t->child[(size_t)pr.first * 8 + o];
+                        if (ch >= 0) next.emplace_back((uint32_t)ch, pr.second);
+                    }
+                frontier.swap(next);
+            }
+            for (auto& pr : frontier) {
+                const uint32_t i = pr.first;
+                const uint32_t idx = ((cz[i] & m) << (2 * gdep)) | ((cy[i] & m) << gdep) | (cx[i] & m);
+                tab[((size_t)pr.second << (3 * gdep)) + idx] = local[i];
+            }
+            void* dptr = nullptr;
+            OO_CUDA(c, cudaMalloc(&dptr, tab.size() * 4));
+            c->d_hop.push_back(dptr);
+            OO_CUDA(c, cudaMemcpyAsync(dptr, tab.data(), tab.size() * 4, cudaMemcpyHostToDevice, stream));
+            lv.hop = (const int32_t*)dptr;
+            table_bytes += tab.size() * 4;
+            prev_depth = lv.depth;
+        }
+    }
+    c->info.node_table_bytes = table_bytes;
+    c->info.launches += (uint64_t)launches;
+    OO_CUDA(c, cudaStreamSynchronize(stream));
+    OO_CUDA(c, cudaGetLastError());
+    c->T = T;
+    c->plan_ok = plan_ok;
+    c->have_tree = true;
+    if (c->have_mlp) c->M.feat_dim = L * T.F;
+    return OO_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// oo_upload_mlp
+// ---------------------------------------------------------------------------------------------------------------------
+extern "C" OO_API oo_status oo_upload_mlp(oo_ctx* c, const oo_mlp_desc* m, void* cuda_stream) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (!m || !m->weights) return fail(c, OO_ERR_INVALID_ARG, "mlp or mlp.weights is NULL");
+    if (m->width != 64) return fail(c, OO_ERR_UNSUPPORTED, "hidden width %u: only 64 is implemented", m->width);
+    if (m->n_hidden < 1 || m->n_hidden > OO_MAX_HIDDEN) return fail(c, OO_ERR_INVALID_ARG, "n_hidden %u outside 1..%d", m->n_hidden, OO_MAX_HIDDEN);
+    if (m->out_dim < 1 || m->out_dim > 8) return fail(c, OO_ERR_INVALID_ARG, "out_dim %u outside 1..8", m->out_dim);
+    if (m->in_dim < 7 || m->in_dim > OO_MAX_LEVELS * 32 + 6 + OO_MAX_EXTRA) return fail(c, OO_ERR_INVALID_ARG, "in_dim %u out of range", m->in_dim);
+    if (m->out_act != OO_ACT_NONE && m->out_act != OO_ACT_EXP) return fail(c, OO_ERR_INVALID_ARG, "unknown out_act");
+    for (uint32_t k = 0; k <= m->n_hidden; ++k)
+        if (!m->weights[k]) return fail(c, OO_ERR_INVALID_ARG, "weights[%u] is NULL", k);
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    DeviceGuard g(c->device);
+    const uint32_t k1 = (m->in_dim + 15) & ~15u;
+    const uint32_t s0 = k1 + 8, s1 = 72;
+    const size_t halves = (size_t)64 * s0 + (size_t)(m->n_hidden - 1) * 64 * s1 + (size_t)16 * s1;
+    std::vector<uint16_t> img(halves, 0);
+    const uint16_t* w0 = (const uint16_t*)m->weights[0];
+    for (uint32_t o = 0; o < 64; ++o)
+        for (uint32_t i = 0; i < m->in_dim; ++i) img[(size_t)o * s0 + i] = w0[(size_t)o * m->in_dim + i];
+    size_t off = (size_t)64 * s0;
+    for (uint32_t k = 1; k < m->n_hidden; ++k) {
+        const uint16_t* w = (const uint16_t*)m->weights[k];
+        for (uint32_t o = 0; o < 64; ++o)
+            for (uint32_t i = 0; i < 64; ++i) img[off + (size_t)o * s1 + i] = w[(size_t)o * 64 + i];
+        off += (size_t)64 * s1;
+    }
+    const uint16_t* wl = (const uint16_t*)m->weights[m->n_hidden];
+    for (uint32_t o = 0; o < m->out_dim; ++o)
+        for (uint32_t i = 0; i < 64; ++i) img[off + (size_t)o * s1 + i] = wl[(size_t)o * 64 + i];
+    free_dev(c->d_image);
+    c->have_mlp = false;
+    OO_CUDA(c, cudaMalloc(&c->d_image, halves * 2));
+    OO_CUDA(c, cudaMemcpyAsync(c->d_image, img.data(), halves * 2, cudaMemcpyHostToDevice, stream));
+    OO_CUDA(c, cudaStreamSynchronize(stream));
+    MlpParams M{};
+    M.image = (const uint16_t*)c->d_image;
+    M.image_bytes = (uint32_t)(halves * 2);
+    M.in_dim = m->in_dim; M.k1 = k1; M.n_hidden = m->n_hidden; M.out_dim = m->out_dim; M.out_act = (uint32_t)m->out_act;
+    M.feat_dim = c->have_tree ? c->T.n_levels * c->T.F : 0;
+    c->M = M;
+    c->have_mlp = true;
+    return OO_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// scratch
+// ---------------------------------------------------------------------------------------------------------------------
+extern "C" OO_API oo_status oo_reserve(oo_ctx* c, uint64_t n) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (n <= c->reserved) return OO_OK;
+    DeviceGuard g(c->device);
+    free_scratch(c);
+    OO_CUDA(c, cudaMalloc((void**)&c->d_keys_a, n * 4));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_keys_b, n * 4));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_idx_a, n * 4));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_hist, morton_sort_hist_ints(n) * 4));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_qx, n * 12));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_qn, n * 12));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_qw, n * 12));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_qe, n * 4 * OO_MAX_EXTRA));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_rgb, n * 4 * 8));
+    c->reserved = n;
+    return OO_OK;
+}
+
+static oo_status ensure_feat(oo_ctx* c, uint64_t bytes) {
+    if (bytes <= c->feat_bytes) return OO_OK;
+    free_dev(c->d_feat);
+    c->feat_bytes = 0;
+    OO_CUDA(c, cudaMalloc(&c->d_feat, bytes));
+    c->feat_bytes = bytes;
+    return OO_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// oo_sort_queries
+// ---------------------------------------------------------------------------------------------------------------------
+extern "C" OO_API oo_status oo_sort_queries(oo_ctx* c, const oo_queries* q, uint32_t* d_perm_out, void* cuda_stream) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (!q || (q->n && (!q->x || !d_perm_out))) return fail(c, OO_ERR_INVALID_ARG, "NULL argument");
+    if (q->n >= (1ull << 32)) return fail(c, OO_ERR_UNSUPPORTED, "more than 2^32-1 queries per call");
+    if (q->n > c->reserved) return fail(c, OO_ERR_NOT_READY, "call oo_reserve(%llu) first", (unsigned long long)q->n);
+    if (oo_status st = check_async(c)) return st;
+    DeviceGuard g(c->device);
+    count(c, launch_morton_sort(q->x, q->n, c->d_keys_a, c->d_keys_b, c->d_idx_a, d_perm_out, c->d_hist, (cudaStream_t)cuda_stream));
+    return check_async(c);
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// oo_encode / oo_query
+// ---------------------------------------------------------------------------------------------------------------------
+static oo_path resolve_encode_path(oo_ctx* c) {
+    const bool fast = c->plan_ok && fast_shape_supported(c->T.n_levels, c->T.F, c->T.f32 != 0);
+    if (c->path == OO_PATH_GENERIC) return OO_PATH_GENERIC;
+    if (c->path == OO_PATH_AUTO) return fast ? OO_PATH_UNFUSED : OO_PATH_GENERIC;
+    return fast ? OO_PATH_UNFUSED : (oo_path)-1;
+}
+
+extern "C" OO_API oo_status oo_encode(oo_ctx* c, const oo_queries* q, void* d_features, int32_t* d_slot, int16_t* d_texel,
+                               void* cuda_stream) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "no tree uploaded");
+    if (oo_status st = check_queries(c, q, false)) return st;
+    if (oo_status st = check_async(c)) return st;
+    if (q->n == 0) return OO_OK;
+    DeviceGuard g(c->device);
+    const oo_path p = resolve_encode_path(c);
+    if ((int)p < 0) return fail(c, OO_ERR_UNSUPPORTED, "no specialised kernel for L=%u F=%u (or the tree has no hop plan); use OO_PATH_GENERIC/AUTO", c->T.n_levels, c->T.F);
+    QueryParams Q = make_qp(q);
+    EncodeOut O{d_features, d_slot, d_texel};
+    int n = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Q, O, c->tree_max_depth, (cudaStream_t)cuda_stream)
+                                 : launch_encode_fast(c->T, Q, O, c->n_sms, (cudaStream_t)cuda_stream);
+    if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "encode kernel missing");
+    count(c, n);
+    c->info.path_last_encode = (uint32_t)p;
+    return check_async(c);
+}
+
+static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cudaStream_t stream) {
+    if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "no tree uploaded");
+    if (!c->have_mlp) return fail(c, OO_ERR_NOT_READY, "no MLP uploaded");
+    if (oo_status st = check_queries(c, q, true)) return st;
+    if (q->n && !d_rgb) return fail(c, OO_ERR_INVALID_ARG, "rgb is NULL");
+    const uint32_t feat = c->T.n_levels * c->T.F;
+    if (c->M.in_dim != feat + 6 + q->n_extra)
+        return fail(c, OO_ERR_NOT_READY, "MLP in_dim %u != L*F + 6 + n_extra = %u", c->M.in_dim, feat + 6 + q->n_extra);
+    if (oo_status st = check_async(c)) return st;
+    if (q->n == 0) return OO_OK;
+    c->M.feat_dim = feat;
+    const bool fast = c->plan_ok && fast_shape_supported(c->T.n_levels, c->T.F, c->T.f32 != 0);
+    oo_path p = c->path;
+    if (p == OO_PATH_AUTO) p = fast ? OO_PATH_FUSED_MMA : OO_PATH_GENERIC;
+    if (p != OO_PATH_GENERIC && !fast)
+        return fail(c, OO_ERR_UNSUPPORTED, "no specialised kernel for L=%u F=%u (or the tree has no hop plan); use OO_PATH_GENERIC/AUTO", c->T.n_levels, c->T.F);
+    QueryParams Q = make_qp(q);
+    int n = 0;
+    if (p == OO_PATH_GENERIC || p == OO_PATH_UNFUSED) {
+        const uint64_t bytes = q->n * (uint64_t)feat * (c->T.f32 ? 4 : 2);
+        if (oo_status st = ensure_feat(c, bytes)) return st;
+        EncodeOut O{c->d_feat, nullptr, nullptr};
+        // features are indexed by the query's own index, so perm only changes the processing order
+        n = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Q, O, c->tree_max_depth, stream)
+                                 : launch_encode_fast(c->T, Q, O, c->n_sms, stream);
+        if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "encode kernel missing");
+        count(c, n);
+        n = launch_mlp_rows(c->T, c->M, Q, c->d_feat, d_rgb, c->n_sms, stream);
+    } else if (p == OO_PATH_FUSED_MMA) {
+        n = launch_fused_mma(c->T, c->M, Q, d_rgb, c->n_sms, stream);
+    } else {
+        n = launch_fused_tc(c->T, c->M, Q, d_rgb, c->n_sms, stream);
+    }
+    if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "requested kernel path %d is not available for this shape", (int)p);
+    count(c, n);
+    c->info.path_last_query = (uint32_t)p;
+    return check_async(c);
+}
+
+extern "C" OO_API oo_status oo_query(oo_ctx* c, const oo_queries* q, float* d_rgb, void* cuda_stream) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    DeviceGuard g(c->device);
+    return query_device(c, q, d_rgb, (cudaStream_t)cuda_stream);
+}
+
+extern "C" OO_API oo_status oo_query_host(oo_ctx* c, const oo_queries* q, float* h_rgb, void* cuda_stream) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (!q) return fail(c, OO_ERR_INVALID_ARG, "queries is NULL");
+    if (q->perm) return fail(c, OO_ERR_INVALID_ARG, "oo_query_host: perm must be NULL");
+    if (q->n > c->reserved) return fail(c, OO_ERR_NOT_READY, "call oo_reserve(%llu) first", (unsigned long long)q->n);
+    if (oo_status st = check_queries(c, q, true)) return st;
+    if (q->n == 0) return OO_OK;
+    if (!h_rgb) return fail(c, OO_ERR_INVALID_ARG, "rgb is NULL");
+    if (!c->have_mlp) return fail(c, OO_ERR_NOT_READY, "no MLP uploaded");
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    DeviceGuard g(c->device);
+    OO_CUDA(c, cudaMemcpyAsync(c->d_qx, q->x, q->n * 12, cudaMemcpyHostToDevice, stream));
+    OO_CUDA(c, cudaMemcpyAsync(c->d_qn, q->nrm, q->n * 12, cudaMemcpyHostToDevice, stream));
+    OO_CUDA(c, cudaMemcpyAsync(c->d_qw, q->wo, q->n * 12, cudaMemcpyHostToDevice, stream));
+    if (q->n_extra) OO_CUDA(c, cudaMemcpyAsync(c->d_qe, q->extra, q->n * 4 * q->n_extra, cudaMemcpyHostToDevice, stream));
+    oo_queries dq = *q;
+    dq.x = c->d_qx; dq.nrm = c->d_qn; dq.wo = c->d_qw; dq.extra = q->n_extra ? c->d_qe : nullptr;
+    if (oo_status st = query_device(c, &dq, c->d_rgb, stream)) return st;
+    OO_CUDA(c, cudaMemcpyAsync(h_rgb, c->d_rgb, q->n * 4 * c->M.out_dim, cudaMemcpyDeviceToHost, stream));
+    OO_CUDA(c, cudaStreamSynchronize(stream));
+    return OO_OK;
+}
+
+extern "C" OO_API oo_status oo_read_padded_map(oo_ctx* c, uint32_t level, uint32_t slot, void* h_out) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "no tree uploaded");
+    if (level >= c->T.n_levels || slot >= c->level_slots[level] || !h_out) return fail(c, OO_ERR_INVALID_ARG, "bad level/slot/pointer");
+    DeviceGuard g(c->device);
+    const LevelParams& lv = c->T.lv[level];
+    OO_CUDA(c, cudaMemcpy(h_out, (const uint8_t*)c->atlas_dev[level] + (uint64_t)slot * lv.map_bytes, lv.map_bytes, cudaMemcpyDeviceToHost));
+    return OO_OK;
+}

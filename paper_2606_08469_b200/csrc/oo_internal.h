@@ -1,0 +1,97 @@
+// oo_internal.h — structures shared by the host side of liboo (oo_api.cu) and its kernels (oo_kernels.cu).
+// Not part of the ABI.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "oo.h"
+
+namespace oo {
+
+// ---------------------------------------------------------------------------------------------------------------
+// Device-side view of one used level.  The library's atlas layout is level-major and BORDER-PADDED: every map is
+// (R+2) x (R+2) texels, the one-texel border pre-filled by the octahedral wrap, so the four bilinear taps of any
+// base texel (i0, j0) in [-1, R-1]^2 are plain neighbours and the hot loop has no wrap logic.  `atlas` is pre-offset by
+// one row and one texel, so tap (i0, j0) is at  atlas + slot*map_bytes + (j0*Rp + i0)*texel_bytes  for i0, j0 >= -1.
+struct LevelParams {
+    const uint8_t* atlas;
+    const int32_t* hop;     // hop table from the previous station: [n_prev][8^gap] -> slot at this depth (-1 = absent)
+    float half_r;           // R/2
+    float off;              // R/2 - 1/2
+    uint32_t R;
+    uint32_t Rp;            // R + 2
+    uint32_t map_bytes;     // Rp*Rp*texel_bytes
+    uint32_t row_bytes;     // Rp*texel_bytes
+    uint32_t depth;
+    uint32_t shift;         // depth_eff - depth
+    uint32_t dense;         // 1: slot = dense table lookup (depth <= 4); 0: hop from the previous station
+    uint32_t dense_off;     // offset (ints) of this level's dense table inside the dense block
+    uint32_t gap;           // depth - previous station depth (1..3) when !dense
+    uint32_t pad_;
+};
+
+struct TreeParams {
+    LevelParams lv[OO_MAX_LEVELS];
+    uint32_t n_levels;
+    uint32_t F;
+    uint32_t f32;            // texel dtype is fp32
+    uint32_t texel_bytes;
+    uint32_t depth_eff;      // deepest used depth: positions are quantised to 2^depth_eff cells per axis
+    float scale_eff;         // 2^depth_eff
+    // top station: dense table at depth T = min(4, depth_eff) giving the local node index at that depth
+    uint32_t t_depth, t_shift, t_dense_off;
+    uint32_t dense_ints;     // total ints of the dense block (staged into shared memory by the fast kernels)
+    const int32_t* dense;    // global copy of the dense block
+    // plain representation for the generic kernels
+    const int32_t* child;    // [n_nodes][8]
+    const int32_t* map_slot; // [n_nodes]
+};
+
+struct QueryParams {
+    uint64_t n;
+    const float* x;
+    const float* nrm;
+    const float* wo;
+    const float* extra;
+    uint32_t n_extra;
+    const uint32_t* perm;
+};
+
+// Decoder image: the padded, shared-memory-ready copy of the weights (built by oo_upload_mlp).
+//   layer 0:        [64][K1 + 8] halves, K1 = in_dim rounded up to 16 (extra columns zero)
+//   layers 1..H-1:  [64][72]
+//   output layer:   [16][72] (rows >= out_dim zero)      -- 16 rows so that the same image also serves a N=16 UMMA
+struct MlpParams {
+    const uint16_t* image;   // global
+    uint32_t image_bytes;
+    uint32_t in_dim, k1, n_hidden, out_dim, out_act;
+    uint32_t feat_dim;       // L*F
+};
+
+struct EncodeOut {
+    void* features;          // [n][L*F] tree dtype, or nullptr
+    int32_t* slot;           // [n][L] or nullptr
+    int16_t* texel;          // [n][L][2] or nullptr
+};
+
+// ---------------------------------------------------------------------------------------------------------------
+// Launchers (oo_kernels.cu / oo_sort.cu).  Each returns the number of kernels it launched, or -1 if the requested
+// specialisation does not exist.  All launches go to `stream`.
+int launch_pad_atlas(const void* src, void* dst, uint64_t slots, uint32_t R, uint32_t texel_bytes, cudaStream_t stream);
+int launch_encode_generic(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, uint32_t tree_max_depth,
+                          cudaStream_t stream);
+int launch_encode_fast(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, int n_sms, cudaStream_t stream);
+int launch_mlp_rows(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const void* features, float* rgb,
+                    int n_sms, cudaStream_t stream);
+int launch_fused_mma(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
+                     cudaStream_t stream);
+int launch_fused_tc(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
+                    cudaStream_t stream);
+bool fast_shape_supported(uint32_t L, uint32_t F, bool f32);
+int launch_morton_sort(const float* x, uint64_t n, uint32_t* keys_a, uint32_t* keys_b, uint32_t* idx_a, uint32_t* perm_out,
+                       uint32_t* hist, cudaStream_t stream);
+size_t morton_sort_hist_ints(uint64_t n);
+
+}  // namespace oo

@@ -1,0 +1,263 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element, on the same seeded inputs.
+
+Bars (BASELINE.json north_star): slots and base texels bit-exact; features within 1e-3; RGB max-abs 2e-2 / mean-abs
+2e-3 on outputs in [0,4] (A23 above 4).  Every available kernel path is checked, and the paths against each other."""
+import numpy as np
+import pytest
+
+import gen
+from oracle import c as OC
+from oracle import oo_oracle as O
+from parity import check_features, check_indices, check_rgb
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2606_08469_b200 as P
+    return P
+
+
+def _dev(q):
+    cu = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    return cu(q.x), cu(q.nrm), cu(q.wo), cu(q.extra)
+
+
+def _paths(P, ctx):
+    out = [P.PATH_GENERIC]
+    if ctx.oo_get_info()["hop_plan_ok"]:
+        out += [P.PATH_UNFUSED, P.PATH_FUSED_MMA, P.PATH_FUSED_TC]
+    return out
+
+
+def _run_all(P, w, ref_feat, ref_slot, ref_tex, ref_rgb, expect_fast=True):
+    ctx = P.OctaOctree(0).upload_workload(w)
+    x, n, wo, ex = _dev(w.queries)
+    results = {}
+    for path in _paths(P, ctx):
+        ctx.oo_set_path(path)
+        try:
+            rgb = ctx.oo_query(x, n, wo, ex)
+        except P.OOError as e:
+            if e.status == 3 and path == P.PATH_FUSED_TC:      # tcgen05 variant not available for this shape
+                continue
+            raise
+        torch.cuda.synchronize()
+        results[path] = rgb.cpu().numpy()
+        check_rgb(results[path], ref_rgb)
+        if path in (P.PATH_GENERIC, P.PATH_UNFUSED):
+            f, s, t = ctx.oo_encode(x, wo, want_debug=True)
+            torch.cuda.synchronize()
+            check_indices(s.cpu().numpy(), t.cpu().numpy(), ref_slot, ref_tex)
+            check_features(f.float().cpu().numpy(), ref_feat)
+    if expect_fast:
+        assert P.PATH_FUSED_MMA in results
+        # same arithmetic in the same order: the fused and unfused specialised paths agree bit for bit
+        assert np.array_equal(results[P.PATH_FUSED_MMA], results[P.PATH_UNFUSED])
+    ctx.oo_set_path(P.PATH_AUTO)
+    rgb = ctx.oo_query(x, n, wo, ex).cpu().numpy()
+    info = ctx.oo_get_info()
+    assert info["path_last_query"] == (P.PATH_FUSED_MMA if expect_fast else P.PATH_GENERIC)
+    check_rgb(rgb, ref_rgb)
+    assert info["query_launches"] > 0
+    ctx.close()
+    return results
+
+
+@pytest.mark.parametrize("variant", ["cfg0", "cfg0_root0"])
+def test_config0(P, variant):
+    w = gen.config0(root0_variant=(variant == "cfg0_root0"))
+    q = w.queries
+    f, s, t = O.encode(w.tree, w.atlas.levels, q.x, q.wo)
+    rgb = O.query(w.tree, w.atlas.levels, w.mlp.weights, q.x, q.nrm, q.wo)
+    _run_all(P, w, f, s, t, rgb)
+
+
+@pytest.mark.parametrize("cfg,width,height,max_depth", [(1, 192, 160, None), (2, 160, 90, None), (1, 97, 61, 6),
+                                                        (3, 128, 96, 8), (3, 96, 64, 6)])
+def test_scene_configs_reduced(P, cfg, width, height, max_depth):
+    """configs 1-3 recipes at reduced frame size (and, for config 3, reduced depth): several 32-query tiles + a ragged tail."""
+    w = gen.scene_workload(cfg, width=width, height=height, max_depth=max_depth)
+    q = w.queries
+    co = OC.from_workload(w)
+    f, s, t = co.encode(q.x, q.wo)
+    rgb = co.query(q.x, q.nrm, q.wo, q.extra)
+    _run_all(P, w, f, s, t, rgb)
+
+
+def test_absent_cells_and_out_of_cube_positions(P):
+    """A17/A16: random positions in a sparse tree (most fine cells absent -> zero features), positions outside the cube."""
+    w = gen.scene_workload(1, width=64, height=64)
+    q = gen.random_queries(5003, 5)
+    q.x[:200] = q.x[:200] * 3.0 - 1.0                # outside [0,1]^3: clamped
+    q.x[200] = [1.0, 1.0, 1.0]
+    q.x[201] = [0.0, 0.0, 0.0]
+    q.wo[:6] = [[1, 0, 0], [-1, 0, 0], [0, 1, 0], [0, -1, 0], [0, 0, 1], [0, 0, -1]]     # axis directions: border taps
+    q.wo[6] = [-0.0, 0.0, -1.0]
+    q.wo[7:300] *= 7.5                               # not normalised (A22)
+    w.queries = q
+    co = OC.from_workload(w)
+    f, s, t = co.encode(q.x, q.wo)
+    assert (s < 0).mean() > 0.3
+    rgb = co.query(q.x, q.nrm, q.wo)
+    _run_all(P, w, f, s, t, rgb)
+
+
+def test_non_canonical_levels_fall_back_to_generic(P):
+    """Used depths {1, 6}: the gap of 5 has no hop plan; AUTO must run the generic kernels and still match."""
+    scene = gen.make_scene("three", 0)
+    tree = gen.build_tree(scene, 6).set_levels([1, 6], [16, 4])
+    atlas = gen.make_atlas(tree, 8, "f16", 0)
+    mlp = gen.make_mlp(2 * 8 + 6, 2, 0)
+    cam = gen.make_camera(80, 60, 0)
+    w = gen.Workload("odd", tree, atlas, mlp, gen.raycast(scene, cam), scene, cam)
+    co = OC.from_workload(w)
+    q = w.queries
+    f, s, t = co.encode(q.x, q.wo)
+    rgb = co.query(q.x, q.nrm, q.wo)
+    _run_all(P, w, f, s, t, rgb, expect_fast=False)
+
+
+def test_unspecialised_shape_falls_back_to_generic(P):
+    """L=6 levels of F=8 has no template instance: AUTO -> generic; also out_act = none and out_dim = 5."""
+    tree = gen.build_tree(None, 3, uniform=True)
+    tree = gen.build_tree(gen.make_scene("three", 1), 6).set_levels([1, 2, 3, 4, 5, 6], [8, 8, 4, 4, 2, 2])
+    atlas = gen.make_atlas(tree, 8, "f16", 1)
+    mlp = gen.make_mlp(6 * 8 + 6, 3, 1, out_dim=5, out_act="none")
+    scene = gen.make_scene("three", 1)
+    w = gen.Workload("L6", tree, atlas, mlp, gen.raycast(scene, gen.make_camera(70, 50, 1)), scene)
+    co = OC.from_workload(w)
+    q = w.queries
+    f, s, t = co.encode(q.x, q.wo)
+    rgb = co.query(q.x, q.nrm, q.wo)
+    ctx = P.OctaOctree(0).upload_workload(w)
+    x, n, wo, _ = _dev(q)
+    got = ctx.oo_query(x, n, wo).cpu().numpy()
+    assert ctx.oo_get_info()["path_last_query"] == P.PATH_GENERIC
+    assert got.shape == (q.n, 5)
+    assert np.abs(got - rgb).max() < 2e-2
+    fe, sl, tx = ctx.oo_encode(x, wo, want_debug=True)
+    check_indices(sl.cpu().numpy(), tx.cpu().numpy(), s, t)
+    check_features(fe.float().cpu().numpy(), f)
+
+
+def test_padded_atlas_is_the_octahedral_wrap(P, ):
+    """a5, bit-exact: the library's border-padded map equals the oracle's wrap applied to the uploaded map."""
+    w = gen.config0()
+    ctx = P.OctaOctree(0).upload_workload(w)
+    for level, slot in [(0, 3), (1, 41)]:
+        R = w.tree.level_res[level]
+        pad = ctx.oo_read_padded_map(level, slot, R)
+        jj, ii = np.meshgrid(np.arange(-1, R + 1), np.arange(-1, R + 1), indexing="ij")
+        wi, wj = O.wrap(ii.ravel(), jj.ravel(), R)
+        expect = w.atlas.levels[level][slot][wj, wi].reshape(R + 2, R + 2, -1)
+        assert np.array_equal(pad, expect)
+    w1 = gen.scene_workload(1, width=32, height=32)
+    ctx.upload_workload(w1)                            # a second upload replaces the first
+    for level in range(4):
+        R = w1.tree.level_res[level]
+        slot = w1.tree.level_slots[level] - 1
+        pad = ctx.oo_read_padded_map(level, slot, R)
+        jj, ii = np.meshgrid(np.arange(-1, R + 1), np.arange(-1, R + 1), indexing="ij")
+        wi, wj = O.wrap(ii.ravel(), jj.ravel(), R)
+        expect = w1.atlas.levels[level][slot][wj, wi].reshape(R + 2, R + 2, -1)
+        assert np.array_equal(pad.view(np.uint16), expect.view(np.uint16))
+
+
+@pytest.mark.parametrize("n", [0, 1, 31, 32, 33, 255, 257])
+def test_ragged_sizes(P, n):
+    w = gen.config0(n=max(n, 1))
+    ctx = P.OctaOctree(0).upload_workload(w)
+    q = w.queries.take(slice(0, n))
+    x, nn, wo, _ = _dev(q)
+    if n == 0:
+        x = torch.empty((0, 3), device="cuda"); nn = x.clone(); wo = x.clone()
+    ref = O.query(w.tree, w.atlas.levels, w.mlp.weights, q.x, q.nrm, q.wo) if n else np.zeros((0, 3))
+    for path in (P.PATH_GENERIC, P.PATH_UNFUSED, P.PATH_FUSED_MMA):
+        ctx.oo_set_path(path)
+        guard = torch.full((n + 8, 3), -7.0, device="cuda")
+        ctx.oo_query(x, nn, wo, rgb=guard[:n])
+        torch.cuda.synchronize()
+        got = guard.cpu().numpy()
+        assert np.all(got[n:] == -7.0)                 # nothing written past the end
+        if n:
+            check_rgb(got[:n], ref)
+
+
+def test_morton_sort_and_permuted_query(P):
+    """a1: the permutation is the unique stable Morton order (bit-exact vs the oracle); processing in any order leaves
+    the outputs in the caller's order, bit for bit."""
+    w = gen.scene_workload(2, width=160, height=90)
+    q = w.queries
+    ctx = P.OctaOctree(0).upload_workload(w)
+    ctx.oo_reserve(q.n)
+    x, n, wo, ex = _dev(q)
+    perm = ctx.oo_sort_queries(x)
+    torch.cuda.synchronize()
+    assert np.array_equal(perm.cpu().numpy().astype(np.int64), O.morton_order(q.x))
+    base = ctx.oo_query(x, n, wo, ex).cpu().numpy()
+    shuf = torch.from_numpy(gen.shuffle_perm(q.n, 0).astype(np.int32)).cuda()
+    for path in (P.PATH_GENERIC, P.PATH_UNFUSED, P.PATH_FUSED_MMA):
+        ctx.oo_set_path(path)
+        ref = ctx.oo_query(x, n, wo, ex).cpu().numpy()
+        assert np.array_equal(ref, base)
+        for pm in (perm, shuf):
+            got = ctx.oo_query(x, n, wo, ex, perm=pm).cpu().numpy()
+            assert np.array_equal(got, ref)
+    # a random cloud of positions incl. out-of-range ones (keys clamp), several radix chunks and a ragged tail
+    xs = torch.from_numpy((gen.u01(3, 1, 3 * 70001).reshape(-1, 3) * 1.2 - 0.1).astype(np.float32)).cuda()
+    ctx.oo_reserve(70001)
+    perm = ctx.oo_sort_queries(xs).cpu().numpy().astype(np.int64)
+    assert np.array_equal(perm, O.morton_order(xs.cpu().numpy()))
+
+
+def test_query_host_equals_query(P):
+    w = gen.scene_workload(2, width=96, height=64)
+    q = w.queries
+    ctx = P.OctaOctree(0).upload_workload(w)
+    ctx.oo_reserve(q.n)
+    x, n, wo, ex = _dev(q)
+    dev = ctx.oo_query(x, n, wo, ex).cpu().numpy()
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    host = ctx.oo_query_host(pin(q.x), pin(q.nrm), pin(q.wo), pin(q.extra))
+    assert np.array_equal(host.numpy(), dev)
+    host2 = ctx.oo_query_host(q.x, q.nrm, q.wo, q.extra, rgb=np.empty((q.n, 3), np.float32))   # pageable numpy
+    assert np.array_equal(host2, dev)
+
+
+def test_error_codes(P):
+    w = gen.config0()
+    ctx = P.OctaOctree(0)
+    x, n, wo, _ = _dev(w.queries)
+    with pytest.raises(P.OOError) as e:
+        ctx.oo_query(x, n, wo)
+    assert e.value.status == 2                                     # nothing uploaded
+    ctx.oo_upload_tree(w.tree, w.atlas.levels, "f32")
+    ctx.oo_upload_mlp(gen.make_mlp(15, 2, 0).weights)
+    with pytest.raises(P.OOError) as e:
+        ctx.oo_query(x, n, wo)
+    assert e.value.status == 2 and "in_dim" in str(e.value)        # MLP width does not match the tree
+    with pytest.raises(P.OOError) as e:
+        ctx.oo_upload_mlp([np.zeros((32, 14), np.float16), np.zeros((3, 32), np.float16)])
+    assert e.value.status == 3                                     # width 32 unsupported
+    bad = gen.config0().tree
+    bad.child = bad.child.copy()
+    bad.child[0, 0] = 50                                           # a depth-2 node as child of the root
+    with pytest.raises(P.OOError) as e:
+        ctx.oo_upload_tree(bad, w.atlas.levels, "f32")
+    assert e.value.status == 1
+    bad = gen.config0().tree
+    bad.map_slot = bad.map_slot.copy()
+    bad.map_slot[2] = bad.map_slot[1]                              # duplicate slot
+    with pytest.raises(P.OOError) as e:
+        ctx.oo_upload_tree(bad, w.atlas.levels, "f32")
+    assert e.value.status == 1
+    ctx.upload_workload(w)                                         # the context is still usable
+    ref = O.query(w.tree, w.atlas.levels, w.mlp.weights, w.queries.x, w.queries.nrm, w.queries.wo)
+    check_rgb(ctx.oo_query(x, n, wo).cpu().numpy(), ref)
+    with pytest.raises(P.OOError) as e:
+        ctx.oo_sort_queries(x)
+    assert e.value.status == 2                                     # oo_reserve not called
