@@ -147,17 +147,16 @@ static void encode_one(const oracle_tree* t, const float x[3], const float wo[3]
     }
 }
 
-/* O8 */
-static void mlp_one(const oracle_mlp* m, const double* in, double* rgb) {
+/* O8.  W[layer] = the fp16 weights widened exactly to double (done once per call, see oracle_query). */
+static void mlp_one(const oracle_mlp* m, double* const* W, const double* in, double* rgb) {
     double a[MAX_DIM], b[MAX_DIM];
     int n_in = (int)m->in_dim;
     for (int k = 0; k < n_in; ++k) a[k] = in[k];
     for (uint32_t layer = 0; layer <= m->n_hidden; ++layer) {
         int n_out = layer == m->n_hidden ? (int)m->out_dim : (int)m->width;
-        const uint16_t* W = m->weights[layer];
         for (int o = 0; o < n_out; ++o) {
             double acc = 0.0;
-            for (int k = 0; k < n_in; ++k) acc += half_to_double(W[(size_t)o * n_in + k]) * a[k];
+            for (int k = 0; k < n_in; ++k) acc += W[layer][(size_t)o * n_in + k] * a[k];
             if (layer < m->n_hidden) acc = acc > 0.0 ? acc : 0.0;
             b[o] = acc;
         }
@@ -197,6 +196,13 @@ ORACLE_API int oracle_query(const oracle_tree* t, const oracle_mlp* m, uint64_t 
     int L = (int)t->n_levels, F = (int)t->n_features, used = 1;
     if (L > MAX_LEVELS || m->n_hidden + 1 > MAX_LAYERS || m->in_dim > MAX_DIM || m->width > MAX_DIM) return -1;
     if ((uint32_t)(L * F) + 6 + n_extra != m->in_dim) return -2;
+    double* W[MAX_LAYERS];
+    for (uint32_t layer = 0; layer <= m->n_hidden; ++layer) {
+        size_t n_in = layer == 0 ? m->in_dim : m->width, n_out = layer == m->n_hidden ? m->out_dim : m->width;
+        W[layer] = (double*)malloc(n_in * n_out * sizeof(double));
+        if (!W[layer]) return -3;
+        for (size_t k = 0; k < n_in * n_out; ++k) W[layer][k] = half_to_double(m->weights[layer][k]);
+    }
 #ifdef _OPENMP
     if (n_threads <= 0) n_threads = omp_get_max_threads();
     used = n_threads;
@@ -210,7 +216,8 @@ ORACLE_API int oracle_query(const oracle_tree* t, const oracle_mlp* m, uint64_t 
         for (int a = 0; a < 3; ++a) in[p++] = (double)nrm[3 * k + a];
         for (int a = 0; a < 3; ++a) in[p++] = (double)wo[3 * k + a];
         for (uint32_t e = 0; e < n_extra; ++e) in[p++] = (double)extra[(size_t)k * n_extra + e];
-        mlp_one(m, in, rgb + (size_t)k * m->out_dim);
+        mlp_one(m, W, in, rgb + (size_t)k * m->out_dim);
     }
+    for (uint32_t layer = 0; layer <= m->n_hidden; ++layer) free(W[layer]);
     return used;
 }

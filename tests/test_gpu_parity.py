@@ -107,9 +107,10 @@ def test_absent_cells_and_out_of_cube_positions(P):
 
 
 def test_non_canonical_levels_fall_back_to_generic(P):
-    """Used depths {1, 6}: the gap of 5 has no hop plan; AUTO must run the generic kernels and still match."""
+    """Used depths {1, 8}: 8 is more than 3 levels below the top station (depth 4), so there is no hop plan; AUTO must
+    run the generic kernels and still match."""
     scene = gen.make_scene("three", 0)
-    tree = gen.build_tree(scene, 6).set_levels([1, 6], [16, 4])
+    tree = gen.build_tree(scene, 8).set_levels([1, 8], [16, 4])
     atlas = gen.make_atlas(tree, 8, "f16", 0)
     mlp = gen.make_mlp(2 * 8 + 6, 2, 0)
     cam = gen.make_camera(80, 60, 0)
