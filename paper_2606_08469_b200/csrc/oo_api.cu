@@ -38,6 +38,7 @@ struct oo_ctx {
     bool have_mlp = false;
     MlpParams M{};
     void* d_image = nullptr;
+    void* d_image_tc = nullptr;
 
     // scratch
     uint64_t reserved = 0;
@@ -177,6 +178,7 @@ extern "C" OO_API void oo_destroy(oo_ctx* c) {
         DeviceGuard g(c->device);
         free_tree(c);
         free_dev(c->d_image);
+        free_dev(c->d_image_tc);
         free_scratch(c);
     }
     delete c;
@@ -449,16 +451,38 @@ extern "C" OO_API oo_status oo_upload_mlp(oo_ctx* c, const oo_mlp_desc* m, void*
     const uint16_t* wl = (const uint16_t*)m->weights[m->n_hidden];
     for (uint32_t o = 0; o < m->out_dim; ++o)
         for (uint32_t i = 0; i < 64; ++i) img[off + (size_t)o * s1 + i] = wl[(size_t)o * 64 + i];
+    // tensor-core image: chunk-major [K/8][N][8] per layer
+    const size_t tc_halves = (size_t)k1 * 64 + (size_t)(m->n_hidden - 1) * 64 * 64 + (size_t)64 * 16;
+    std::vector<uint16_t> tc(tc_halves, 0);
+    {
+        auto put = [&](size_t base, uint32_t N, uint32_t n, uint32_t k, uint16_t v) { tc[base + ((size_t)(k / 8) * N + n) * 8 + (k % 8)] = v; };
+        for (uint32_t o = 0; o < 64; ++o)
+            for (uint32_t i = 0; i < m->in_dim; ++i) put(0, 64, o, i, w0[(size_t)o * m->in_dim + i]);
+        size_t base = (size_t)k1 * 64;
+        for (uint32_t k = 1; k < m->n_hidden; ++k) {
+            const uint16_t* w = (const uint16_t*)m->weights[k];
+            for (uint32_t o = 0; o < 64; ++o)
+                for (uint32_t i = 0; i < 64; ++i) put(base, 64, o, i, w[(size_t)o * 64 + i]);
+            base += (size_t)64 * 64;
+        }
+        for (uint32_t o = 0; o < m->out_dim; ++o)
+            for (uint32_t i = 0; i < 64; ++i) put(base, 16, o, i, wl[(size_t)o * 64 + i]);
+    }
     free_dev(c->d_image);
+    free_dev(c->d_image_tc);
     c->have_mlp = false;
     OO_CUDA(c, cudaMalloc(&c->d_image, halves * 2));
     OO_CUDA(c, cudaMemcpyAsync(c->d_image, img.data(), halves * 2, cudaMemcpyHostToDevice, stream));
+    OO_CUDA(c, cudaMalloc(&c->d_image_tc, tc_halves * 2));
+    OO_CUDA(c, cudaMemcpyAsync(c->d_image_tc, tc.data(), tc_halves * 2, cudaMemcpyHostToDevice, stream));
     OO_CUDA(c, cudaStreamSynchronize(stream));
     MlpParams M{};
     M.image = (const uint16_t*)c->d_image;
     M.image_bytes = (uint32_t)(halves * 2);
     M.in_dim = m->in_dim; M.k1 = k1; M.n_hidden = m->n_hidden; M.out_dim = m->out_dim; M.out_act = (uint32_t)m->out_act;
     M.feat_dim = c->have_tree ? c->T.n_levels * c->T.F : 0;
+    M.image_tc = (const uint16_t*)c->d_image_tc;
+    M.image_tc_bytes = (uint32_t)(tc_halves * 2);
     c->M = M;
     c->have_mlp = true;
     return OO_OK;
@@ -551,7 +575,7 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
     c->M.feat_dim = feat;
     const bool fast = c->plan_ok && fast_shape_supported(c->T.n_levels, c->T.F, c->T.f32 != 0);
     oo_path p = c->path;
-    if (p == OO_PATH_AUTO) p = fast ? OO_PATH_FUSED_MMA : OO_PATH_GENERIC;
+    if (p == OO_PATH_AUTO) p = !fast ? OO_PATH_GENERIC : (tc_shape_supported(c->T.n_levels, c->T.F, c->T.f32 != 0) && c->M.out_dim <= 4 ? OO_PATH_FUSED_TC : OO_PATH_FUSED_MMA);
     if (p != OO_PATH_GENERIC && !fast)
         return fail(c, OO_ERR_UNSUPPORTED, "no specialised kernel for L=%u F=%u (or the tree has no hop plan); use OO_PATH_GENERIC/AUTO", c->T.n_levels, c->T.F);
     QueryParams Q = make_qp(q);

@@ -1,10 +1,299 @@
-// oo_fused_tc.cu — fused encode + MLP on tcgen05.mma with TMEM accumulators (OO_PATH_FUSED_TC).
+// oo_fused_tc.cu — fused encode + MLP on 5th-generation tensor cores (OO_PATH_FUSED_TC).
+//
+// One warpgroup (128 threads) owns a tile of 128 queries end to end; thread t is query row t and TMEM lane t.
+//   gather (registers, fp32)  ->  fp16 row into the A tile in shared memory (UMMA K-major canonical layout)
+//   -> tcgen05.mma.kind::f16 M=128 N=64 K=16 steps issued by ONE thread, accumulator in TMEM (64 fp32 columns)
+//   -> tcgen05.commit -> mbarrier -> every thread tcgen05.ld's its own row -> ReLU -> fp16 -> back into the A tile
+//   -> next layer ... -> output layer (N=16) -> exp -> RGB.
+// Features and activations never touch HBM.  A block holds two such warpgroups sharing the descent tables and the weight
+// image; several blocks per SM overlap the memory-bound gather of one tile with the tensor/epilogue phase of others.
+//
+// Shared-memory operand layout (no swizzle, K-major): 16-byte chunk c (8 consecutive K) of row r is at
+//   base + c * (rows*16) + r*16,  i.e. core matrices (8 rows x 16 B) are contiguous, SBO = 128 B, LBO = rows*16 B.
+// A warp writing chunk c of its 32 rows therefore writes 512 contiguous bytes (no bank conflicts).
 #include "oo_device.cuh"
 
 namespace oo {
 
-int launch_fused_tc(const TreeParams&, const MlpParams&, const QueryParams&, float*, int, cudaStream_t) {
-    return -1;   // not built yet: oo_query reports OO_ERR_UNSUPPORTED for OO_PATH_FUSED_TC
+namespace {
+
+constexpr int kTcThreads = 256;      // two warpgroups
+constexpr int kTileRows = 128;
+
+// ------------------------------------------------------------------------------------------------- PTX wrappers
+__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void tmem_relinquish() {
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+__device__ __forceinline__ void fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void named_bar(uint32_t id, uint32_t threads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
+}
+__device__ __forceinline__ void mbar_init(uint32_t mbar, uint32_t count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
+}
+__device__ __forceinline__ uint32_t mbar_try_wait(uint32_t mbar, uint32_t parity) {
+    uint32_t ok;
+    asm volatile(
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+        : "=r"(ok)
+        : "r"(mbar), "r"(parity)
+        : "memory");
+    return ok;
+}
+// bounded wait: a protocol bug traps instead of hanging the GPU
+__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
+    for (uint32_t spin = 0; !mbar_try_wait(mbar, parity); ++spin)
+        if (spin > (1u << 26)) __trap();
+}
+// D[tmem] (+)= A[smem] * B[smem]^T ; kind::f16, fp32 accumulate
+__device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+    asm volatile(
+        "{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n" ::"r"(d_tmem),
+        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void umma_commit(uint32_t mbar) {
+    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(mbar) : "memory");
+}
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+
+// 32 lanes x 32 consecutive fp32 columns: thread i of the warp receives row (lane base + i)
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+          "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]),
+          "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]),
+          "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+        : "r"(taddr)
+        : "memory");
+}
+__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t (&r)[4]) {
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+                 : "r"(taddr)
+                 : "memory");
+}
+
+// shared-memory matrix descriptor, K-major, SWIZZLE_NONE: start address, LBO (between the two 16-byte K chunks of one
+// K=16 step), SBO (between 8-row groups), descriptor version 1 (sm_100)
+__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
+    return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16) |
+           ((uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32) | (1ull << 46);
+}
+// instruction descriptor: D = fp32, A = B = fp16, both K-major, M x N
+__host__ __device__ constexpr uint32_t instr_desc(uint32_t M, uint32_t N) { return (1u << 4) | ((N >> 3) << 17) | ((M >> 4) << 24); }
+
+}  // namespace
+
+// The tensor-core weight image (built by oo_upload_mlp, MlpParams::image_tc): per layer chunk-major [K/8][N][8] halves:
+//   layer 0: K = k1, N = 64;  layers 1..H-1: K = 64, N = 64;  output: K = 64, N = 16 (rows >= out_dim zero).
+template <int L, int F, bool F32>
+__global__ void __launch_bounds__(kTcThreads, 3) fused_tc_kernel(const __grid_constant__ TreeParams T,
+                                                                 const __grid_constant__ MlpParams M,
+                                                                 const __grid_constant__ QueryParams Q,
+                                                                 float* __restrict__ rgb, uint32_t n_tiles) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    const uint32_t dense_bytes = (T.dense_ints * 4 + 127) & ~127u;
+    const uint32_t a_chunks = (M.k1 > 64 ? M.k1 : 64) / 8;
+    const uint32_t a_bytes = a_chunks * kTileRows * 16;
+    int32_t* s_dense = (int32_t*)smem;
+    uint8_t* s_w = smem + dense_bytes;
+    uint8_t* s_a0 = s_w + ((M.image_tc_bytes + 127) & ~127u);
+    uint64_t* s_bar = (uint64_t*)(s_a0 + 2 * a_bytes);
+    uint32_t* s_tmem = (uint32_t*)(s_bar + 2);
+
+    const uint32_t wg = threadIdx.x >> 7, row = threadIdx.x & 127, warp = threadIdx.x >> 5;
+    {
+        const uint4* s = (const uint4*)T.dense;
+        uint4* d = (uint4*)s_dense;
+        for (uint32_t i = threadIdx.x; i < T.dense_ints / 4; i += kTcThreads) d[i] = __ldg(s + i);
+        s = (const uint4*)M.image_tc;
+        d = (uint4*)s_w;
+        for (uint32_t i = threadIdx.x; i < M.image_tc_bytes / 16; i += kTcThreads) d[i] = __ldg(s + i);
+    }
+    if (threadIdx.x == 0) {
+        mbar_init(smem_u32(&s_bar[0]), 1);
+        mbar_init(smem_u32(&s_bar[1]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    if (warp == 0) {
+        tmem_alloc(smem_u32(s_tmem), 128);
+        tmem_relinquish();
+    }
+    fence_async_smem();          // the weight image was written with generic stores and is read by the tensor core
+    fence_before_sync();
+    __syncthreads();
+    fence_after_sync();
+    const uint32_t tmem_d = *s_tmem + wg * 64;                       // this warpgroup's 64 accumulator columns
+    const uint32_t tmem_lane = tmem_d + ((row & ~31u) << 16);        // this warp's 32 lanes
+    uint8_t* s_a = s_a0 + wg * a_bytes;
+    const uint32_t a_addr = smem_u32(s_a), w_addr = smem_u32(s_w), bar = smem_u32(&s_bar[wg]);
+    const uint32_t a_lbo = kTileRows * 16;                           // 2048 B between K chunks of the A tile
+    uint32_t phase = 0;
+    const bool leader = row == 0;
+    constexpr uint32_t idesc_h = instr_desc(128, 64), idesc_o = instr_desc(128, 16);
+
+    for (uint32_t tile = blockIdx.x * 2 + wg; tile < n_tiles; tile += gridDim.x * 2) {
+        // ------------------------------------------------------------------ gather: one query per thread
+        const uint64_t t = (uint64_t)tile * kTileRows + row;
+        const bool valid = t < Q.n;
+        const uint64_t tt = valid ? t : Q.n - 1;
+        const uint64_t qi = Q.perm ? Q.perm[tt] : tt;
+        float x[3], n[3], w[3];
+        load3(Q.x, qi, x);
+        load3(Q.nrm, qi, n);
+        load3(Q.wo, qi, w);
+        Encoded<L, F, F32> e;
+        locate<L, F, F32>(T, s_dense, x, w, e);
+        uint8_t* a_row = s_a + row * 16;
+#pragma unroll
+        for (int l = 0; l < L; ++l) {
+            const LevelParams& lv = T.lv[l];
+            const Tap tp = level_tap(e.uv, lv.half_r, lv.off);
+            float h[F];
+            gather_level<F, F32>(lv, e.slot[l], tp, h);
+            if constexpr (F % 8 == 0) {
+#pragma unroll
+                for (int v = 0; v < F / 8; ++v)
+                    *(uint4*)(a_row + (l * (F / 8) + v) * a_lbo) =
+                        make_uint4(pack_half2(h[8 * v], h[8 * v + 1]), pack_half2(h[8 * v + 2], h[8 * v + 3]),
+                                   pack_half2(h[8 * v + 4], h[8 * v + 5]), pack_half2(h[8 * v + 6], h[8 * v + 7]));
+            } else {   // F == 4: half a chunk
+                *(uint2*)(a_row + ((l * 4) / 8) * a_lbo + ((l * 4) % 8) * 2) = make_uint2(pack_half2(h[0], h[1]), pack_half2(h[2], h[3]));
+            }
+        }
+        {   // attributes + zero padding up to k1
+            float v[24];
+#pragma unroll
+            for (int k = 0; k < 24; ++k) v[k] = 0.0f;
+            constexpr int lead = (L * F) % 8;            // 0 or 4: position of n inside its chunk
+            v[lead + 0] = n[0]; v[lead + 1] = n[1]; v[lead + 2] = n[2];
+            v[lead + 3] = w[0]; v[lead + 4] = w[1]; v[lead + 5] = w[2];
+#pragma unroll
+            for (int k = 0; k < OO_MAX_EXTRA; ++k)
+                if ((uint32_t)k < Q.n_extra) v[lead + 6 + k] = __ldg(Q.extra + qi * Q.n_extra + k);
+            constexpr int c0 = (L * F) / 8;
+            const uint32_t c_end = M.k1 / 8;
+            if constexpr (lead == 0) {
+                *(uint4*)(a_row + c0 * a_lbo) = make_uint4(pack_half2(v[0], v[1]), pack_half2(v[2], v[3]), pack_half2(v[4], v[5]), pack_half2(v[6], v[7]));
+            } else {
+                *(uint2*)(a_row + c0 * a_lbo + 8) = make_uint2(pack_half2(v[4], v[5]), pack_half2(v[6], v[7]));
+            }
+            if (c0 + 1 < c_end)
+                *(uint4*)(a_row + (c0 + 1) * a_lbo) = make_uint4(pack_half2(v[8], v[9]), pack_half2(v[10], v[11]), pack_half2(v[12], v[13]), pack_half2(v[14], v[15]));
+            if (c0 + 2 < c_end)
+                *(uint4*)(a_row + (c0 + 2) * a_lbo) = make_uint4(pack_half2(v[16], v[17]), pack_half2(v[18], v[19]), pack_half2(v[20], v[21]), pack_half2(v[22], v[23]));
+        }
+        // ------------------------------------------------------------------ hidden layers
+        uint32_t w_off = 0;
+        for (uint32_t layer = 0; layer < M.n_hidden; ++layer) {
+            const uint32_t kt_n = (layer == 0 ? M.k1 : 64u) >> 4;
+            fence_async_smem();          // my A-tile stores -> visible to the tensor core
+            fence_before_sync();
+            named_bar(1 + wg, 128);
+            if (leader) {
+                fence_after_sync();
+                for (uint32_t kt = 0; kt < kt_n; ++kt)
+                    umma_f16(tmem_d, smem_desc(a_addr + kt * 2 * a_lbo, a_lbo, 128),
+                             smem_desc(w_addr + w_off + kt * 2 * 1024, 1024, 128), idesc_h, kt);
+                umma_commit(bar);
+            }
+            w_off += kt_n * 2 * 1024;
+            mbar_wait(bar, phase);
+            phase ^= 1;
+            fence_after_sync();
+            // epilogue: my row of D -> ReLU -> fp16 -> my row of the next A tile
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                uint32_t r[32];
+                tmem_ld32(tmem_lane + half * 32, r);
+                tmem_wait_ld();
+#pragma unroll
+                for (int c = 0; c < 4; ++c)
+                    *(uint4*)(a_row + (half * 4 + c) * a_lbo) =
+                        make_uint4(pack_half2_relu(__uint_as_float(r[8 * c]), __uint_as_float(r[8 * c + 1])),
+                                   pack_half2_relu(__uint_as_float(r[8 * c + 2]), __uint_as_float(r[8 * c + 3])),
+                                   pack_half2_relu(__uint_as_float(r[8 * c + 4]), __uint_as_float(r[8 * c + 5])),
+                                   pack_half2_relu(__uint_as_float(r[8 * c + 6]), __uint_as_float(r[8 * c + 7])));
+            }
+        }
+        // ------------------------------------------------------------------ output layer (N = 16, K = 64)
+        fence_async_smem();
+        fence_before_sync();
+        named_bar(1 + wg, 128);
+        if (leader) {
+            fence_after_sync();
+#pragma unroll
+            for (uint32_t kt = 0; kt < 4; ++kt)
+                umma_f16(tmem_d, smem_desc(a_addr + kt * 2 * a_lbo, a_lbo, 128), smem_desc(w_addr + w_off + kt * 2 * 256, 256, 128),
+                         idesc_o, kt);
+            umma_commit(bar);
+        }
+        mbar_wait(bar, phase);
+        phase ^= 1;
+        fence_after_sync();
+        uint32_t o[4];
+        tmem_ld4(tmem_lane, o);
+        tmem_wait_ld();
+        if (valid) {
+#pragma unroll
+            for (uint32_t c = 0; c < 4; ++c)
+                if (c < M.out_dim) {
+                    const float z = __uint_as_float(o[c]);
+                    rgb[qi * M.out_dim + c] = M.out_act == OO_ACT_EXP ? fast_exp(z) : z;
+                }
+        }
+        // the next tile's MMA overwrites D: make sure every thread's TMEM loads are ordered before the next barrier
+        fence_before_sync();
+    }
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(*s_tmem, 128);
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+#define OO_TC_SHAPES(X)                                                        \
+    X(1, 8, false) X(2, 8, false) X(3, 8, false) X(4, 8, false) X(5, 8, false) \
+    X(2, 16, false) X(3, 16, false) X(4, 16, false) X(5, 16, false)            \
+    X(2, 4, true) X(4, 4, true)
+
+bool tc_shape_supported(uint32_t L, uint32_t F, bool f32) {
+#define X(l, f, t) if (L == l && F == f && f32 == t) return true;
+    OO_TC_SHAPES(X)
+#undef X
+    return false;
+}
+
+int launch_fused_tc(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, cudaStream_t stream) {
+    if (Q.n == 0) return 0;
+    if (M.out_dim > 4 || !M.image_tc) return -1;
+    const uint32_t a_chunks = (M.k1 > 64 ? M.k1 : 64) / 8;
+    const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + 2 * a_chunks * kTileRows * 16 + 64;
+    const uint64_t n_tiles = (Q.n + kTileRows - 1) / kTileRows;
+    const uint64_t blocks = (n_tiles + 1) / 2;
+    const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms * 3 ? blocks : (uint64_t)n_sms * 3);
+#define X(l, f, t)                                                                                                  \
+    if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                                         \
+        static bool attr = false;                                                                                   \
+        if (!attr) {                                                                                                \
+            cudaFuncSetAttribute(fused_tc_kernel<l, f, t>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); \
+            attr = true;                                                                                            \
+        }                                                                                                           \
+        fused_tc_kernel<l, f, t><<<grid, kTcThreads, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles);              \
+        return 1;                                                                                                   \
+    }
+    OO_TC_SHAPES(X)
+#undef X
+    return -1;
 }
 
 }  // namespace oo

@@ -68,6 +68,10 @@ struct MlpParams {
     uint32_t image_bytes;
     uint32_t in_dim, k1, n_hidden, out_dim, out_act;
     uint32_t feat_dim;       // L*F
+    // the same weights in the UMMA K-major canonical layout for the tcgen05 kernel: per layer [K/8][N][8] halves
+    // (layer 0: K = k1, N = 64; hidden: K = N = 64; output: K = 64, N = 16 with rows >= out_dim zero)
+    const uint16_t* image_tc;
+    uint32_t image_tc_bytes;
 };
 
 struct EncodeOut {
@@ -90,6 +94,7 @@ int launch_fused_mma(const TreeParams& T, const MlpParams& M, const QueryParams&
 int launch_fused_tc(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
                     cudaStream_t stream);
 bool fast_shape_supported(uint32_t L, uint32_t F, bool f32);
+bool tc_shape_supported(uint32_t L, uint32_t F, bool f32);
 int launch_morton_sort(const float* x, uint64_t n, uint32_t* keys_a, uint32_t* keys_b, uint32_t* idx_a, uint32_t* perm_out,
                        uint32_t* hist, cudaStream_t stream);
 size_t morton_sort_hist_ints(uint64_t n);

@@ -38,19 +38,6 @@ int launch_pad_atlas(const void* src, void* dst, uint64_t slots, uint32_t R, uin
 }
 
 // =====================================================================================================================
-// Query loading
-// =====================================================================================================================
-struct QueryRegs {
-    float x[3], n[3], w[3];
-};
-
-__device__ __forceinline__ void load3(const float* __restrict__ p, uint64_t qi, float (&v)[3]) {
-    v[0] = __ldg(p + qi * 3);
-    v[1] = __ldg(p + qi * 3 + 1);
-    v[2] = __ldg(p + qi * 3 + 2);
-}
-
-// =====================================================================================================================
 // Generic encode: any tree, any (F, dtype) with 16/32/64-byte texels.  Plain child-table descent per level.
 // One thread per query.  Slow by design; it is the fallback and a cross-check of the specialised kernels.
 // =====================================================================================================================
@@ -115,34 +102,6 @@ int launch_encode_generic(const TreeParams& T, const QueryParams& Q, const Encod
     const unsigned grid = (unsigned)((Q.n + 255) / 256);
     encode_generic_kernel<<<grid, 256, 0, stream>>>(T, Q, O, tree_max_depth);
     return 1;
-}
-
-// =====================================================================================================================
-// Shared pieces of the specialised kernels
-// =====================================================================================================================
-
-// stage `bytes` (multiple of 16) from global to shared with all threads of the block
-__device__ __forceinline__ void stage_to_smem(void* dst, const void* src, uint32_t bytes) {
-    const uint4* s = (const uint4*)src;
-    uint4* d = (uint4*)dst;
-    for (uint32_t i = threadIdx.x; i < bytes / 16; i += blockDim.x) d[i] = __ldg(s + i);
-}
-
-template <int L, int F, bool F32>
-struct Encoded {
-    int slot[L];
-    OctaUV uv;
-};
-
-// a2 + a3 + a4 for one query
-template <int L, int F, bool F32>
-__device__ __forceinline__ void locate(const TreeParams& T, const int32_t* s_dense, const float (&x)[3],
-                                       const float (&w)[3], Encoded<L, F, F32>& e) {
-    const int qmax = (int)(1u << T.depth_eff) - 1;
-    const int qx = quantise(x[0], T.scale_eff, qmax), qy = quantise(x[1], T.scale_eff, qmax),
-              qz = quantise(x[2], T.scale_eff, qmax);
-    descend_plan<L>(T, s_dense, qx, qy, qz, e.slot);
-    e.uv = octa_project(w[0], w[1], w[2]);
 }
 
 // =====================================================================================================================
