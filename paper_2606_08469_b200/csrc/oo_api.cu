@@ -594,6 +594,10 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
         n = launch_fused_mma(c->T, c->M, Q, d_rgb, c->n_sms, stream);
     } else {
         n = launch_fused_tc(c->T, c->M, Q, d_rgb, c->n_sms, stream);
+        if (n < 0 && c->path == OO_PATH_AUTO) {      // e.g. shared memory does not fit: the mma.sync kernel always does
+            p = OO_PATH_FUSED_MMA;
+            n = launch_fused_mma(c->T, c->M, Q, d_rgb, c->n_sms, stream);
+        }
     }
     if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "requested kernel path %d is not available for this shape", (int)p);
     count(c, n);

@@ -17,7 +17,6 @@ namespace oo {
 
 namespace {
 
-constexpr int kTcThreads = 256;      // two warpgroups
 constexpr int kTileRows = 128;
 
 // ------------------------------------------------------------------------------------------------- PTX wrappers
@@ -42,16 +41,20 @@ __device__ __forceinline__ void mbar_init(uint32_t mbar, uint32_t count) {
 __device__ __forceinline__ uint32_t mbar_try_wait(uint32_t mbar, uint32_t parity) {
     uint32_t ok;
     asm volatile(
-        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}\n"
+        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n selp.u32 %0, 1, 0, p;\n}\n"
         : "=r"(ok)
-        : "r"(mbar), "r"(parity)
+        : "r"(mbar), "r"(parity), "r"(20000u)
         : "memory");
     return ok;
 }
-// bounded wait: a protocol bug traps instead of hanging the GPU
+// The hardware suspends the thread inside try_wait (up to the hint, in ns), so the loop rarely iterates.  Bounded: a
+// protocol bug traps instead of hanging the GPU.
 __device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
     for (uint32_t spin = 0; !mbar_try_wait(mbar, parity); ++spin)
-        if (spin > (1u << 26)) __trap();
+        if (spin > (1u << 22)) __trap();
+}
+__device__ __forceinline__ void cp_async4(uint32_t saddr, const void* gptr) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(saddr), "l"(gptr) : "memory");
 }
 // D[tmem] (+)= A[smem] * B[smem]^T ; kind::f16, fp32 accumulate
 __device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
@@ -97,37 +100,42 @@ __host__ __device__ constexpr uint32_t instr_desc(uint32_t M, uint32_t N) { retu
 
 // The tensor-core weight image (built by oo_upload_mlp, MlpParams::image_tc): per layer chunk-major [K/8][N][8] halves:
 //   layer 0: K = k1, N = 64;  layers 1..H-1: K = 64, N = 64;  output: K = 64, N = 16 (rows >= out_dim zero).
-template <int L, int F, bool F32>
-__global__ void __launch_bounds__(kTcThreads, 3) fused_tc_kernel(const __grid_constant__ TreeParams T,
-                                                                 const __grid_constant__ MlpParams M,
-                                                                 const __grid_constant__ QueryParams Q,
-                                                                 float* __restrict__ rgb, uint32_t n_tiles) {
+//
+// ONE persistent block per SM with NWG warpgroups: the descent tables and the weight image are staged once per SM and
+// shared; every warpgroup owns an A tile, 64 TMEM columns, an mbarrier and a query staging buffer into which the NEXT
+// tile's (x, n, wo, extra, index) are prefetched with cp.async while the current tile is gathered and decoded, so the
+// cold HBM latency of the query stream is hidden behind the previous tile.
+template <int L, int F, bool F32, int NWG>
+__global__ void __launch_bounds__(NWG * 128, 1) fused_tc_kernel(const __grid_constant__ TreeParams T,
+                                                                const __grid_constant__ MlpParams M,
+                                                                const __grid_constant__ QueryParams Q,
+                                                                float* __restrict__ rgb, uint32_t n_tiles) {
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t dense_bytes = (T.dense_ints * 4 + 127) & ~127u;
     const uint32_t a_chunks = (M.k1 > 64 ? M.k1 : 64) / 8;
     const uint32_t a_bytes = a_chunks * kTileRows * 16;
+    const uint32_t q_words = 10 + Q.n_extra;                         // x3 n3 wo3 index extras, each [128] words
+    const uint32_t q_bytes = q_words * kTileRows * 4;
     int32_t* s_dense = (int32_t*)smem;
     uint8_t* s_w = smem + dense_bytes;
-    uint8_t* s_a0 = s_w + ((M.image_tc_bytes + 127) & ~127u);
-    uint64_t* s_bar = (uint64_t*)(s_a0 + 2 * a_bytes);
-    uint32_t* s_tmem = (uint32_t*)(s_bar + 2);
+    uint8_t* s_tiles = s_w + ((M.image_tc_bytes + 127) & ~127u);
+    uint64_t* s_bar = (uint64_t*)(s_tiles + NWG * (a_bytes + q_bytes));
+    uint32_t* s_tmem = (uint32_t*)(s_bar + NWG);
 
     const uint32_t wg = threadIdx.x >> 7, row = threadIdx.x & 127, warp = threadIdx.x >> 5;
     {
         const uint4* s = (const uint4*)T.dense;
         uint4* d = (uint4*)s_dense;
-        for (uint32_t i = threadIdx.x; i < T.dense_ints / 4; i += kTcThreads) d[i] = __ldg(s + i);
+        for (uint32_t i = threadIdx.x; i < T.dense_ints / 4; i += NWG * 128) d[i] = __ldg(s + i);
         s = (const uint4*)M.image_tc;
         d = (uint4*)s_w;
-        for (uint32_t i = threadIdx.x; i < M.image_tc_bytes / 16; i += kTcThreads) d[i] = __ldg(s + i);
+        for (uint32_t i = threadIdx.x; i < M.image_tc_bytes / 16; i += NWG * 128) d[i] = __ldg(s + i);
     }
-    if (threadIdx.x == 0) {
-        mbar_init(smem_u32(&s_bar[0]), 1);
-        mbar_init(smem_u32(&s_bar[1]), 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
+    if (threadIdx.x < NWG) mbar_init(smem_u32(&s_bar[threadIdx.x]), 1);
+    if (threadIdx.x == 0) asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    constexpr uint32_t kTmemCols = NWG * 64 <= 64 ? 64 : NWG * 64 <= 128 ? 128 : NWG * 64 <= 256 ? 256 : 512;
     if (warp == 0) {
-        tmem_alloc(smem_u32(s_tmem), 128);
+        tmem_alloc(smem_u32(s_tmem), kTmemCols);
         tmem_relinquish();
     }
     fence_async_smem();          // the weight image was written with generic stores and is read by the tensor core
@@ -136,23 +144,48 @@ __global__ void __launch_bounds__(kTcThreads, 3) fused_tc_kernel(const __grid_co
     fence_after_sync();
     const uint32_t tmem_d = *s_tmem + wg * 64;                       // this warpgroup's 64 accumulator columns
     const uint32_t tmem_lane = tmem_d + ((row & ~31u) << 16);        // this warp's 32 lanes
-    uint8_t* s_a = s_a0 + wg * a_bytes;
-    const uint32_t a_addr = smem_u32(s_a), w_addr = smem_u32(s_w), bar = smem_u32(&s_bar[wg]);
+    uint8_t* s_a = s_tiles + wg * (a_bytes + q_bytes);
+    float* s_q = (float*)(s_a + a_bytes) + row;                      // word k of my row: s_q[k * 128]
+    const uint32_t a_addr = smem_u32(s_a), w_addr = smem_u32(s_w), bar = smem_u32(&s_bar[wg]), q_addr = smem_u32(s_q);
     const uint32_t a_lbo = kTileRows * 16;                           // 2048 B between K chunks of the A tile
     uint32_t phase = 0;
     const bool leader = row == 0;
     constexpr uint32_t idesc_h = instr_desc(128, 64), idesc_o = instr_desc(128, 16);
+    const uint32_t tile_stride = gridDim.x * NWG;
 
-    for (uint32_t tile = blockIdx.x * 2 + wg; tile < n_tiles; tile += gridDim.x * 2) {
-        // ------------------------------------------------------------------ gather: one query per thread
+    // prefetch one tile's query rows into the staging buffer: 4-byte cp.async per word (rows are 12-byte packed)
+    auto prefetch = [&](uint32_t tile) {
         const uint64_t t = (uint64_t)tile * kTileRows + row;
-        const bool valid = t < Q.n;
-        const uint64_t tt = valid ? t : Q.n - 1;
-        const uint64_t qi = Q.perm ? Q.perm[tt] : tt;
-        float x[3], n[3], w[3];
-        load3(Q.x, qi, x);
-        load3(Q.nrm, qi, n);
-        load3(Q.wo, qi, w);
+        const uint64_t tt = t < Q.n ? t : Q.n - 1;
+        const uint32_t qi = Q.perm ? __ldg(Q.perm + tt) : (uint32_t)tt;
+        const float* px = Q.x + (size_t)qi * 3;
+        const float* pn = Q.nrm + (size_t)qi * 3;
+        const float* pw = Q.wo + (size_t)qi * 3;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            cp_async4(q_addr + (k) * 512, px + k);
+            cp_async4(q_addr + (3 + k) * 512, pn + k);
+            cp_async4(q_addr + (6 + k) * 512, pw + k);
+        }
+        for (uint32_t k = 0; k < Q.n_extra; ++k) cp_async4(q_addr + (10 + k) * 512, Q.extra + (size_t)qi * Q.n_extra + k);
+        s_q[9 * 128] = __uint_as_float(qi);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    uint32_t tile = blockIdx.x * NWG + wg;
+    if (tile < n_tiles) prefetch(tile);
+    for (; tile < n_tiles; tile += tile_stride) {
+        // ------------------------------------------------------------------ this tile's query (prefetched), next tile's prefetch
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        float x[3], n[3], w[3], ex[OO_MAX_EXTRA];
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { x[k] = s_q[k * 128]; n[k] = s_q[(3 + k) * 128]; w[k] = s_q[(6 + k) * 128]; }
+        const uint32_t qi = __float_as_uint(s_q[9 * 128]);
+#pragma unroll
+        for (int k = 0; k < OO_MAX_EXTRA; ++k) ex[k] = (uint32_t)k < Q.n_extra ? s_q[(10 + k) * 128] : 0.0f;
+        const bool valid = (uint64_t)tile * kTileRows + row < Q.n;
+        if (tile + tile_stride < n_tiles) prefetch(tile + tile_stride);
+        // ------------------------------------------------------------------ gather: one query per thread
         Encoded<L, F, F32> e;
         locate<L, F, F32>(T, s_dense, x, w, e);
         uint8_t* a_row = s_a + row * 16;
@@ -180,8 +213,7 @@ __global__ void __launch_bounds__(kTcThreads, 3) fused_tc_kernel(const __grid_co
             v[lead + 0] = n[0]; v[lead + 1] = n[1]; v[lead + 2] = n[2];
             v[lead + 3] = w[0]; v[lead + 4] = w[1]; v[lead + 5] = w[2];
 #pragma unroll
-            for (int k = 0; k < OO_MAX_EXTRA; ++k)
-                if ((uint32_t)k < Q.n_extra) v[lead + 6 + k] = __ldg(Q.extra + qi * Q.n_extra + k);
+            for (int k = 0; k < OO_MAX_EXTRA; ++k) v[lead + 6 + k] = ex[k];
             constexpr int c0 = (L * F) / 8;
             const uint32_t c_end = M.k1 / 8;
             if constexpr (lead == 0) {
@@ -250,14 +282,15 @@ __global__ void __launch_bounds__(kTcThreads, 3) fused_tc_kernel(const __grid_co
             for (uint32_t c = 0; c < 4; ++c)
                 if (c < M.out_dim) {
                     const float z = __uint_as_float(o[c]);
-                    rgb[qi * M.out_dim + c] = M.out_act == OO_ACT_EXP ? fast_exp(z) : z;
+                    rgb[(size_t)qi * M.out_dim + c] = M.out_act == OO_ACT_EXP ? fast_exp(z) : z;
                 }
         }
-        // the next tile's MMA overwrites D: make sure every thread's TMEM loads are ordered before the next barrier
+        // the next tile's MMA overwrites D: order every thread's TMEM loads before the next barrier
         fence_before_sync();
     }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
-    if (warp == 0) tmem_dealloc(*s_tmem, 128);
+    if (warp == 0) tmem_dealloc(*s_tmem, kTmemCols);
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -273,26 +306,37 @@ bool tc_shape_supported(uint32_t L, uint32_t F, bool f32) {
     return false;
 }
 
+template <int NWG>
+static int launch_tc_nwg(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, uint32_t smem,
+                         cudaStream_t stream) {
+    const uint64_t n_tiles = (Q.n + kTileRows - 1) / kTileRows;
+    const uint64_t blocks = (n_tiles + NWG - 1) / NWG;
+    const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms ? blocks : (uint64_t)n_sms);
+#define X(l, f, t)                                                                                                        \
+    if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                                               \
+        static bool attr = false;                                                                                         \
+        if (!attr) {                                                                                                      \
+            cudaFuncSetAttribute(fused_tc_kernel<l, f, t, NWG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); \
+            attr = true;                                                                                                  \
+        }                                                                                                                 \
+        fused_tc_kernel<l, f, t, NWG><<<grid, NWG * 128, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles);                \
+        return 1;                                                                                                         \
+    }
+    OO_TC_SHAPES(X)
+#undef X
+    return -1;
+}
+
+// Largest warpgroup count per SM-resident block whose shared memory fits (6, else 4); -1 if the shape has no instance.
 int launch_fused_tc(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, cudaStream_t stream) {
     if (Q.n == 0) return 0;
     if (M.out_dim > 4 || !M.image_tc) return -1;
     const uint32_t a_chunks = (M.k1 > 64 ? M.k1 : 64) / 8;
-    const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + 2 * a_chunks * kTileRows * 16 + 64;
-    const uint64_t n_tiles = (Q.n + kTileRows - 1) / kTileRows;
-    const uint64_t blocks = (n_tiles + 1) / 2;
-    const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms * 3 ? blocks : (uint64_t)n_sms * 3);
-#define X(l, f, t)                                                                                                  \
-    if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                                         \
-        static bool attr = false;                                                                                   \
-        if (!attr) {                                                                                                \
-            cudaFuncSetAttribute(fused_tc_kernel<l, f, t>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); \
-            attr = true;                                                                                            \
-        }                                                                                                           \
-        fused_tc_kernel<l, f, t><<<grid, kTcThreads, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles);              \
-        return 1;                                                                                                   \
-    }
-    OO_TC_SHAPES(X)
-#undef X
+    const uint32_t per_wg = a_chunks * kTileRows * 16 + (10 + Q.n_extra) * kTileRows * 4;
+    const uint32_t fixed = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + 64 + 64;
+    const uint32_t limit = 227 * 1024;
+    if (fixed + 6 * per_wg <= limit) return launch_tc_nwg<6>(T, M, Q, rgb, n_sms, fixed + 6 * per_wg, stream);
+    if (fixed + 4 * per_wg <= limit) return launch_tc_nwg<4>(T, M, Q, rgb, n_sms, fixed + 4 * per_wg, stream);
     return -1;
 }
 
