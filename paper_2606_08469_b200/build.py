@@ -13,7 +13,7 @@ BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liboo.so")
 SOURCES = ["oo_api.cu", "oo_kernels.cu", "oo_fused_tc.cu", "oo_sort.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
-              "-Xcompiler", "-fvisibility=hidden", "-I", os.path.join(ROOT, "include"), "-I", CSRC]
+              "-Xcompiler", "-fvisibility=hidden", "-I", os.path.join(ROOT, "include"), "-I", CSRC] + os.environ.get("OO_NVCC_EXTRA", "").split()
 
 
 def _nvcc() -> str:

@@ -11,6 +11,9 @@
 // Shared-memory operand layout (no swizzle, K-major): 16-byte chunk c (8 consecutive K) of row r is at
 //   base + c * (rows*16) + r*16,  i.e. core matrices (8 rows x 16 B) are contiguous, SBO = 128 B, LBO = rows*16 B.
 // A warp writing chunk c of its 32 rows therefore writes 512 contiguous bytes (no bank conflicts).
+#include <cstdio>
+#include <cstdlib>
+
 #include "oo_device.cuh"
 
 namespace oo {
@@ -105,8 +108,8 @@ __host__ __device__ constexpr uint32_t instr_desc(uint32_t M, uint32_t N) { retu
 // shared; every warpgroup owns an A tile, 64 TMEM columns, an mbarrier and a query staging buffer into which the NEXT
 // tile's (x, n, wo, extra, index) are prefetched with cp.async while the current tile is gathered and decoded, so the
 // cold HBM latency of the query stream is hidden behind the previous tile.
-template <int L, int F, bool F32, int NWG>
-__global__ void __launch_bounds__(NWG * 128, 1) fused_tc_kernel(const __grid_constant__ TreeParams T,
+template <int L, int F, bool F32, int NWG, int MINB>
+__global__ void __launch_bounds__(NWG * 128, MINB) fused_tc_kernel(const __grid_constant__ TreeParams T,
                                                                 const __grid_constant__ MlpParams M,
                                                                 const __grid_constant__ QueryParams Q,
                                                                 float* __restrict__ rgb, uint32_t n_tiles) {
@@ -174,46 +177,69 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tc_kernel(const __grid_con
 
     uint32_t tile = blockIdx.x * NWG + wg;
     if (tile < n_tiles) prefetch(tile);
+#ifdef OO_PROFILE_PHASES
+    long long t_gather = 0, t_mlp = 0, t_wait = 0, t_q = 0; int n_done = 0;
+    const long long t_begin = clock64();
+#endif
     for (; tile < n_tiles; tile += tile_stride) {
-        // ------------------------------------------------------------------ this tile's query (prefetched), next tile's prefetch
-        asm volatile("cp.async.wait_group 0;" ::: "memory");
-        float x[3], n[3], w[3], ex[OO_MAX_EXTRA];
-#pragma unroll
-        for (int k = 0; k < 3; ++k) { x[k] = s_q[k * 128]; n[k] = s_q[(3 + k) * 128]; w[k] = s_q[(6 + k) * 128]; }
-        const uint32_t qi = __float_as_uint(s_q[9 * 128]);
-#pragma unroll
-        for (int k = 0; k < OO_MAX_EXTRA; ++k) ex[k] = (uint32_t)k < Q.n_extra ? s_q[(10 + k) * 128] : 0.0f;
+        // ------------------------------------------------------------------ this tile's query (prefetched into s_q)
+        float x[3], w[3];
         const bool valid = (uint64_t)tile * kTileRows + row < Q.n;
-        if (tile + tile_stride < n_tiles) prefetch(tile + tile_stride);
+#ifdef OO_PROFILE_PHASES
+        const long long t0 = clock64();
+#endif
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+#ifdef OO_PROFILE_PHASES
+        const long long t0b = clock64();
+#endif
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { x[k] = s_q[k * 128]; w[k] = s_q[(6 + k) * 128]; }
         // ------------------------------------------------------------------ gather: one query per thread
         Encoded<L, F, F32> e;
         locate<L, F, F32>(T, s_dense, x, w, e);
         uint8_t* a_row = s_a + row * 16;
+        constexpr int NB = (F * (F32 ? 4 : 2) == 16) ? (L < 4 ? L : 4) : (F * (F32 ? 4 : 2) == 32 ? 2 : 1);   // levels per load batch (<= 64 data registers)
 #pragma unroll
-        for (int l = 0; l < L; ++l) {
-            const LevelParams& lv = T.lv[l];
-            const Tap tp = level_tap(e.uv, lv.half_r, lv.off);
-            float h[F];
-            gather_level<F, F32>(lv, e.slot[l], tp, h);
-            if constexpr (F % 8 == 0) {
+        for (int l0 = 0; l0 < L; l0 += NB) {
+            float h[NB][F];
+            if (l0 + NB <= L) {
+                gather_levels<F, F32, NB>(&T.lv[l0], &e.slot[l0], e.uv, h);
+            } else {     // ragged last batch: one level at a time
 #pragma unroll
-                for (int v = 0; v < F / 8; ++v)
-                    *(uint4*)(a_row + (l * (F / 8) + v) * a_lbo) =
-                        make_uint4(pack_half2(h[8 * v], h[8 * v + 1]), pack_half2(h[8 * v + 2], h[8 * v + 3]),
-                                   pack_half2(h[8 * v + 4], h[8 * v + 5]), pack_half2(h[8 * v + 6], h[8 * v + 7]));
-            } else {   // F == 4: half a chunk
-                *(uint2*)(a_row + ((l * 4) / 8) * a_lbo + ((l * 4) % 8) * 2) = make_uint2(pack_half2(h[0], h[1]), pack_half2(h[2], h[3]));
+                for (int b = 0; b < NB; ++b)
+                    if (l0 + b < L) {
+                        const Tap tp = level_tap(e.uv, T.lv[l0 + b].half_r, T.lv[l0 + b].off);
+                        gather_level<F, F32>(T.lv[l0 + b], e.slot[l0 + b], tp, h[b]);
+                    }
+            }
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                const int l = l0 + b;
+                if (l >= L) break;
+                if constexpr (F % 8 == 0) {
+#pragma unroll
+                    for (int v = 0; v < F / 8; ++v)
+                        *(uint4*)(a_row + (l * (F / 8) + v) * a_lbo) =
+                            make_uint4(pack_half2(h[b][8 * v], h[b][8 * v + 1]), pack_half2(h[b][8 * v + 2], h[b][8 * v + 3]),
+                                       pack_half2(h[b][8 * v + 4], h[b][8 * v + 5]), pack_half2(h[b][8 * v + 6], h[b][8 * v + 7]));
+                } else {   // F == 4: half a chunk
+                    *(uint2*)(a_row + ((l * 4) / 8) * a_lbo + ((l * 4) % 8) * 2) = make_uint2(pack_half2(h[b][0], h[b][1]), pack_half2(h[b][2], h[b][3]));
+                }
             }
         }
-        {   // attributes + zero padding up to k1
+        uint32_t qi;
+        {   // attributes + zero padding up to k1 (n, extras and the query index are read from the staging buffer only now,
+            // so that they do not occupy registers during the gather)
             float v[24];
 #pragma unroll
             for (int k = 0; k < 24; ++k) v[k] = 0.0f;
             constexpr int lead = (L * F) % 8;            // 0 or 4: position of n inside its chunk
-            v[lead + 0] = n[0]; v[lead + 1] = n[1]; v[lead + 2] = n[2];
-            v[lead + 3] = w[0]; v[lead + 4] = w[1]; v[lead + 5] = w[2];
 #pragma unroll
-            for (int k = 0; k < OO_MAX_EXTRA; ++k) v[lead + 6 + k] = ex[k];
+            for (int k = 0; k < 3; ++k) { v[lead + k] = s_q[(3 + k) * 128]; v[lead + 3 + k] = w[k]; }
+#pragma unroll
+            for (int k = 0; k < OO_MAX_EXTRA; ++k)
+                if ((uint32_t)k < Q.n_extra) v[lead + 6 + k] = s_q[(10 + k) * 128];
+            qi = __float_as_uint(s_q[9 * 128]);
             constexpr int c0 = (L * F) / 8;
             const uint32_t c_end = M.k1 / 8;
             if constexpr (lead == 0) {
@@ -226,6 +252,12 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tc_kernel(const __grid_con
             if (c0 + 2 < c_end)
                 *(uint4*)(a_row + (c0 + 2) * a_lbo) = make_uint4(pack_half2(v[16], v[17]), pack_half2(v[18], v[19]), pack_half2(v[20], v[21]), pack_half2(v[22], v[23]));
         }
+        // the staging buffer is free again: prefetch the next tile's queries behind this tile's MLP phase
+        if (tile + tile_stride < n_tiles) prefetch(tile + tile_stride);
+#ifdef OO_PROFILE_PHASES
+        const long long t1 = clock64();
+        long long tw = 0;
+#endif
         // ------------------------------------------------------------------ hidden layers
         uint32_t w_off = 0;
         for (uint32_t layer = 0; layer < M.n_hidden; ++layer) {
@@ -241,7 +273,13 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tc_kernel(const __grid_con
                 umma_commit(bar);
             }
             w_off += kt_n * 2 * 1024;
+#ifdef OO_PROFILE_PHASES
+            const long long tw0 = clock64();
             mbar_wait(bar, phase);
+            tw += clock64() - tw0;
+#else
+            mbar_wait(bar, phase);
+#endif
             phase ^= 1;
             fence_after_sync();
             // epilogue: my row of D -> ReLU -> fp16 -> my row of the next A tile
@@ -287,7 +325,16 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tc_kernel(const __grid_con
         }
         // the next tile's MMA overwrites D: order every thread's TMEM loads before the next barrier
         fence_before_sync();
+#ifdef OO_PROFILE_PHASES
+        const long long t2 = clock64();
+        t_q += t0b - t0; t_gather += t1 - t0b; t_mlp += t2 - t1; t_wait += tw; ++n_done;
+#endif
     }
+#ifdef OO_PROFILE_PHASES
+    if (blockIdx.x == 3 && (threadIdx.x & 31) == 0 && n_done)
+        printf("wg %u warp %u tiles %d total %lld qwait %lld gather %lld mlp %lld (mma-wait %lld) per tile\n", wg, warp & 3, n_done,
+               (clock64() - t_begin) / n_done, t_q / n_done, t_gather / n_done, t_mlp / n_done, t_wait / n_done);
+#endif
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     __syncthreads();
     if (warp == 0) tmem_dealloc(*s_tmem, kTmemCols);
@@ -306,20 +353,20 @@ bool tc_shape_supported(uint32_t L, uint32_t F, bool f32) {
     return false;
 }
 
-template <int NWG>
+template <int NWG, int MINB>
 static int launch_tc_nwg(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, uint32_t smem,
                          cudaStream_t stream) {
     const uint64_t n_tiles = (Q.n + kTileRows - 1) / kTileRows;
     const uint64_t blocks = (n_tiles + NWG - 1) / NWG;
-    const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms ? blocks : (uint64_t)n_sms);
+    const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms * MINB ? blocks : (uint64_t)n_sms * MINB);
 #define X(l, f, t)                                                                                                        \
     if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                                               \
         static bool attr = false;                                                                                         \
         if (!attr) {                                                                                                      \
-            cudaFuncSetAttribute(fused_tc_kernel<l, f, t, NWG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); \
+            cudaFuncSetAttribute(fused_tc_kernel<l, f, t, NWG, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); \
             attr = true;                                                                                                  \
         }                                                                                                                 \
-        fused_tc_kernel<l, f, t, NWG><<<grid, NWG * 128, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles);                \
+        fused_tc_kernel<l, f, t, NWG, MINB><<<grid, NWG * 128, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles);                \
         return 1;                                                                                                         \
     }
     OO_TC_SHAPES(X)
@@ -335,8 +382,10 @@ int launch_fused_tc(const TreeParams& T, const MlpParams& M, const QueryParams& 
     const uint32_t per_wg = a_chunks * kTileRows * 16 + (10 + Q.n_extra) * kTileRows * 4;
     const uint32_t fixed = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + 64 + 64;
     const uint32_t limit = 227 * 1024;
-    if (fixed + 6 * per_wg <= limit) return launch_tc_nwg<6>(T, M, Q, rgb, n_sms, fixed + 6 * per_wg, stream);
-    if (fixed + 4 * per_wg <= limit) return launch_tc_nwg<4>(T, M, Q, rgb, n_sms, fixed + 4 * per_wg, stream);
+    // residency: measured on config 1 (B200): 3 warpgroups x 2 blocks/SM 72.9 us, 6 x 1 75.4 us, 5 x 1 78.6 us, 4 x 1 80.7 us
+    if (2 * (fixed + 3 * per_wg + 1024) <= 228 * 1024) return launch_tc_nwg<3, 2>(T, M, Q, rgb, n_sms, fixed + 3 * per_wg, stream);
+    if (fixed + 6 * per_wg <= limit) return launch_tc_nwg<6, 1>(T, M, Q, rgb, n_sms, fixed + 6 * per_wg, stream);
+    if (fixed + 4 * per_wg <= limit) return launch_tc_nwg<4, 1>(T, M, Q, rgb, n_sms, fixed + 4 * per_wg, stream);
     return -1;
 }
 
