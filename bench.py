@@ -152,7 +152,7 @@ def run_ours(args):
     w, desc = workload_for(args.config, rank)
     q = w.queries
     ctx = P.OctaOctree(local_rank).upload_workload(w)
-    path = {"auto": P.PATH_AUTO, "mma": P.PATH_FUSED_MMA, "tc": P.PATH_FUSED_TC, "unfused": P.PATH_UNFUSED, "generic": P.PATH_GENERIC}[args.path]
+    path = {"auto": P.PATH_AUTO, "mma": P.PATH_FUSED_MMA, "tc": P.PATH_FUSED_TC, "tm": P.PATH_FUSED_TC_TMEM, "unfused": P.PATH_UNFUSED, "generic": P.PATH_GENERIC}[args.path]
     ctx.oo_set_path(path)
     ctx.oo_reserve(q.n)
     cu = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
@@ -234,7 +234,7 @@ def run_ours(args):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": mx_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16",
         "data": "synthetic",
-        "config": dict(desc, l2="flushed between steps (256 MB memset)", path={0: "auto", 1: "generic", 2: "unfused", 3: "fused_mma", 4: "fused_tcgen05"}[info["path_last_query"]],
+        "config": dict(desc, l2="flushed between steps (256 MB memset)", path={0: "auto", 1: "generic", 2: "unfused", 3: "fused_mma", 4: "fused_tcgen05", 5: "fused_tcgen05_tmem_a"}[info["path_last_query"]],
                        ms_per_frame_warm_l2=mx_warm, frames_per_rank=1, parallelism="replicated cache, one frame per GPU, no collective"),
         "clocks": clocks,
         "e2e": {"value": tot_q / (mx_e2e * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": int((36 + 4 * (0 if q.extra is None else q.extra.shape[1])) * q.n),
@@ -260,7 +260,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=1, choices=[1, 2, 3])
-    ap.add_argument("--path", default="auto", choices=["auto", "mma", "tc", "unfused", "generic"])
+    ap.add_argument("--path", default="auto", choices=["auto", "mma", "tc", "tm", "unfused", "generic"])
     ap.add_argument("--ref-sample", type=int, default=131072, help="queries in the CPU-oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--quick", action="store_true", help="timed region only (no warm-L2 / e2e / CPU legs): the command ncu wraps")

@@ -66,7 +66,8 @@ typedef enum {
     OO_PATH_GENERIC = 1,     /* any tree: plain child-table descent; encode -> features in HBM -> MLP kernel */
     OO_PATH_UNFUSED = 2,     /* hop-table descent, specialised gather; features round-trip HBM; MLP kernel */
     OO_PATH_FUSED_MMA = 3,   /* one kernel: gather -> shared memory -> mma.sync MLP -> RGB */
-    OO_PATH_FUSED_TC = 4     /* one kernel: gather -> shared memory -> tcgen05.mma (TMEM accumulators) -> RGB */
+    OO_PATH_FUSED_TC = 4,    /* one kernel: gather -> shared memory -> tcgen05.mma (TMEM accumulators) -> RGB */
+    OO_PATH_FUSED_TC_TMEM = 5 /* the same with the activations (A operand) kept in tensor memory: no shared-memory A tile */
 } oo_path;
 
 /* The octree and its feature atlases ("every non-empty cell stores a learnable octahedral feature map").

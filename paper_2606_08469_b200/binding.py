@@ -8,7 +8,7 @@ from typing import List, Optional, Sequence
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "liboo.so")
 
-PATH_AUTO, PATH_GENERIC, PATH_UNFUSED, PATH_FUSED_MMA, PATH_FUSED_TC = 0, 1, 2, 3, 4
+PATH_AUTO, PATH_GENERIC, PATH_UNFUSED, PATH_FUSED_MMA, PATH_FUSED_TC, PATH_FUSED_TC_TMEM = 0, 1, 2, 3, 4, 5
 OO_F16, OO_F32 = 0, 1
 OO_ACT_NONE, OO_ACT_EXP = 0, 1
 _STATUS = {0: "OO_OK", 1: "OO_ERR_INVALID_ARG", 2: "OO_ERR_NOT_READY", 3: "OO_ERR_UNSUPPORTED", 4: "OO_ERR_CUDA", 5: "OO_ERR_OOM"}

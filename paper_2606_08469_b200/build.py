@@ -11,7 +11,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liboo.so")
-SOURCES = ["oo_api.cu", "oo_kernels.cu", "oo_fused_tc.cu", "oo_sort.cu"]
+SOURCES = ["oo_api.cu", "oo_kernels.cu", "oo_fused_tc.cu", "oo_fused_tm.cu", "oo_sort.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
               "-Xcompiler", "-fvisibility=hidden", "-I", os.path.join(ROOT, "include"), "-I", CSRC] + os.environ.get("OO_NVCC_EXTRA", "").split()
 

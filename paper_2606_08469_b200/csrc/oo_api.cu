@@ -188,7 +188,7 @@ extern "C" OO_API const char* oo_last_error(const oo_ctx* c) { return c ? c->err
 
 extern "C" OO_API oo_status oo_set_path(oo_ctx* c, oo_path path) {
     if (!c) return OO_ERR_INVALID_ARG;
-    if ((int)path < 0 || (int)path > (int)OO_PATH_FUSED_TC) return fail(c, OO_ERR_INVALID_ARG, "unknown path %d", (int)path);
+    if ((int)path < 0 || (int)path > (int)OO_PATH_FUSED_TC_TMEM) return fail(c, OO_ERR_INVALID_ARG, "unknown path %d", (int)path);
     c->path = path;
     return OO_OK;
 }
@@ -575,7 +575,9 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
     c->M.feat_dim = feat;
     const bool fast = c->plan_ok && fast_shape_supported(c->T.n_levels, c->T.F, c->T.f32 != 0);
     oo_path p = c->path;
-    if (p == OO_PATH_AUTO) p = !fast ? OO_PATH_GENERIC : (tc_shape_supported(c->T.n_levels, c->T.F, c->T.f32 != 0) && c->M.out_dim <= 4 ? OO_PATH_FUSED_TC : OO_PATH_FUSED_MMA);
+    if (p == OO_PATH_AUTO)
+        p = !fast ? OO_PATH_GENERIC
+                  : (tm_shape_supported(c->T.n_levels, c->T.F, c->T.f32 != 0) && c->M.out_dim <= 4 ? OO_PATH_FUSED_TC_TMEM : OO_PATH_FUSED_MMA);
     if (p != OO_PATH_GENERIC && !fast)
         return fail(c, OO_ERR_UNSUPPORTED, "no specialised kernel for L=%u F=%u (or the tree has no hop plan); use OO_PATH_GENERIC/AUTO", c->T.n_levels, c->T.F);
     QueryParams Q = make_qp(q);
@@ -592,11 +594,17 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
         n = launch_mlp_rows(c->T, c->M, Q, c->d_feat, d_rgb, c->n_sms, stream);
     } else if (p == OO_PATH_FUSED_MMA) {
         n = launch_fused_mma(c->T, c->M, Q, d_rgb, c->n_sms, stream);
-    } else {
+    } else if (p == OO_PATH_FUSED_TC) {
         n = launch_fused_tc(c->T, c->M, Q, d_rgb, c->n_sms, stream);
-        if (n < 0 && c->path == OO_PATH_AUTO) {      // e.g. shared memory does not fit: the mma.sync kernel always does
-            p = OO_PATH_FUSED_MMA;
-            n = launch_fused_mma(c->T, c->M, Q, d_rgb, c->n_sms, stream);
+    } else {
+        n = launch_fused_tm(c->T, c->M, Q, d_rgb, c->n_sms, stream);
+        if (n < 0 && c->path == OO_PATH_AUTO) {      // e.g. a first layer wider than TMEM allows: try shared-memory A, then mma.sync
+            p = OO_PATH_FUSED_TC;
+            n = launch_fused_tc(c->T, c->M, Q, d_rgb, c->n_sms, stream);
+            if (n < 0) {
+                p = OO_PATH_FUSED_MMA;
+                n = launch_fused_mma(c->T, c->M, Q, d_rgb, c->n_sms, stream);
+            }
         }
     }
     if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "requested kernel path %d is not available for this shape", (int)p);

@@ -15,89 +15,13 @@
 #include <cstdlib>
 
 #include "oo_device.cuh"
+#include "oo_tc_ptx.cuh"
 
 namespace oo {
 
 namespace {
 
 constexpr int kTileRows = 128;
-
-// ------------------------------------------------------------------------------------------------- PTX wrappers
-__device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_dst), "r"(ncols) : "memory");
-}
-__device__ __forceinline__ void tmem_relinquish() {
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
-}
-__device__ __forceinline__ void fence_before_sync() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void fence_after_sync() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
-__device__ __forceinline__ void fence_async_smem() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
-__device__ __forceinline__ void named_bar(uint32_t id, uint32_t threads) {
-    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(threads) : "memory");
-}
-__device__ __forceinline__ void mbar_init(uint32_t mbar, uint32_t count) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(mbar), "r"(count) : "memory");
-}
-__device__ __forceinline__ uint32_t mbar_try_wait(uint32_t mbar, uint32_t parity) {
-    uint32_t ok;
-    asm volatile(
-        "{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n selp.u32 %0, 1, 0, p;\n}\n"
-        : "=r"(ok)
-        : "r"(mbar), "r"(parity), "r"(20000u)
-        : "memory");
-    return ok;
-}
-// The hardware suspends the thread inside try_wait (up to the hint, in ns), so the loop rarely iterates.  Bounded: a
-// protocol bug traps instead of hanging the GPU.
-__device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
-    for (uint32_t spin = 0; !mbar_try_wait(mbar, parity); ++spin)
-        if (spin > (1u << 22)) __trap();
-}
-__device__ __forceinline__ void cp_async4(uint32_t saddr, const void* gptr) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(saddr), "l"(gptr) : "memory");
-}
-// D[tmem] (+)= A[smem] * B[smem]^T ; kind::f16, fp32 accumulate
-__device__ __forceinline__ void umma_f16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
-    asm volatile(
-        "{\n .reg .pred p;\n setp.ne.b32 p, %4, 0;\n tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n" ::"r"(d_tmem),
-        "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate)
-        : "memory");
-}
-__device__ __forceinline__ void umma_commit(uint32_t mbar) {
-    asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(mbar) : "memory");
-}
-__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-
-// 32 lanes x 32 consecutive fp32 columns: thread i of the warp receives row (lane base + i)
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
-    asm volatile(
-        "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-        "{%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31}, [%32];"
-        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
-          "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]), "=r"(r[17]), "=r"(r[18]),
-          "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]),
-          "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-        : "r"(taddr)
-        : "memory");
-}
-__device__ __forceinline__ void tmem_ld4(uint32_t taddr, uint32_t (&r)[4]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];"
-                 : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
-                 : "r"(taddr)
-                 : "memory");
-}
-
-// shared-memory matrix descriptor, K-major, SWIZZLE_NONE: start address, LBO (between the two 16-byte K chunks of one
-// K=16 step), SBO (between 8-row groups), descriptor version 1 (sm_100)
-__device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-    return (uint64_t)((saddr >> 4) & 0x3FFF) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16) |
-           ((uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32) | (1ull << 46);
-}
-// instruction descriptor: D = fp32, A = B = fp16, both K-major, M x N
-__host__ __device__ constexpr uint32_t instr_desc(uint32_t M, uint32_t N) { return (1u << 4) | ((N >> 3) << 17) | ((M >> 4) << 24); }
 
 }  // namespace
 
@@ -152,7 +76,7 @@ __global__ void __launch_bounds__(NWG * 128, MINB) fused_tc_kernel(const __grid_
     const uint32_t a_addr = smem_u32(s_a), w_addr = smem_u32(s_w), bar = smem_u32(&s_bar[wg]), q_addr = smem_u32(s_q);
     const uint32_t a_lbo = kTileRows * 16;                           // 2048 B between K chunks of the A tile
     uint32_t phase = 0;
-    const bool leader = row == 0;
+    const bool leader_warp = row < 32;                               // warp 0 of the warpgroup issues the MMAs (one elected lane)
     constexpr uint32_t idesc_h = instr_desc(128, 64), idesc_o = instr_desc(128, 16);
     const uint32_t tile_stride = gridDim.x * NWG;
 
@@ -265,12 +189,10 @@ __global__ void __launch_bounds__(NWG * 128, MINB) fused_tc_kernel(const __grid_
             fence_async_smem();          // my A-tile stores -> visible to the tensor core
             fence_before_sync();
             named_bar(1 + wg, 128);
-            if (leader) {
+            if (leader_warp) {
                 fence_after_sync();
-                for (uint32_t kt = 0; kt < kt_n; ++kt)
-                    umma_f16(tmem_d, smem_desc(a_addr + kt * 2 * a_lbo, a_lbo, 128),
-                             smem_desc(w_addr + w_off + kt * 2 * 1024, 1024, 128), idesc_h, kt);
-                umma_commit(bar);
+                umma_group<8>(tmem_d, smem_desc(a_addr, a_lbo, 128), (2 * a_lbo) >> 4, smem_desc(w_addr + w_off, 1024, 128), 2048 >> 4, idesc_h,
+                              kt_n, bar);
             }
             w_off += kt_n * 2 * 1024;
 #ifdef OO_PROFILE_PHASES
@@ -301,13 +223,9 @@ __global__ void __launch_bounds__(NWG * 128, MINB) fused_tc_kernel(const __grid_
         fence_async_smem();
         fence_before_sync();
         named_bar(1 + wg, 128);
-        if (leader) {
+        if (leader_warp) {
             fence_after_sync();
-#pragma unroll
-            for (uint32_t kt = 0; kt < 4; ++kt)
-                umma_f16(tmem_d, smem_desc(a_addr + kt * 2 * a_lbo, a_lbo, 128), smem_desc(w_addr + w_off + kt * 2 * 256, 256, 128),
-                         idesc_o, kt);
-            umma_commit(bar);
+            umma_group<4>(tmem_d, smem_desc(a_addr, a_lbo, 128), (2 * a_lbo) >> 4, smem_desc(w_addr + w_off, 256, 128), 512 >> 4, idesc_o, 4u, bar);
         }
         mbar_wait(bar, phase);
         phase ^= 1;

@@ -95,6 +95,9 @@ int launch_fused_tc(const TreeParams& T, const MlpParams& M, const QueryParams& 
                     cudaStream_t stream);
 bool fast_shape_supported(uint32_t L, uint32_t F, bool f32);
 bool tc_shape_supported(uint32_t L, uint32_t F, bool f32);
+int launch_fused_tm(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
+                     cudaStream_t stream);
+bool tm_shape_supported(uint32_t L, uint32_t F, bool f32);
 int launch_morton_sort(const float* x, uint64_t n, uint32_t* keys_a, uint32_t* keys_b, uint32_t* idx_a, uint32_t* perm_out,
                        uint32_t* hist, cudaStream_t stream);
 size_t morton_sort_hist_ints(uint64_t n);

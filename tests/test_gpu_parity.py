@@ -29,7 +29,7 @@ def _dev(q):
 def _paths(P, ctx):
     out = [P.PATH_GENERIC]
     if ctx.oo_get_info()["hop_plan_ok"]:
-        out += [P.PATH_UNFUSED, P.PATH_FUSED_MMA, P.PATH_FUSED_TC]
+        out += [P.PATH_UNFUSED, P.PATH_FUSED_MMA, P.PATH_FUSED_TC, P.PATH_FUSED_TC_TMEM]
     return out
 
 
@@ -42,7 +42,7 @@ def _run_all(P, w, ref_feat, ref_slot, ref_tex, ref_rgb, expect_fast=True):
         try:
             rgb = ctx.oo_query(x, n, wo, ex)
         except P.OOError as e:
-            if e.status == 3 and path == P.PATH_FUSED_TC:      # tcgen05 variant not available for this shape
+            if e.status == 3 and path in (P.PATH_FUSED_TC, P.PATH_FUSED_TC_TMEM):      # tcgen05 variant not available for this shape
                 continue
             raise
         torch.cuda.synchronize()
@@ -54,7 +54,7 @@ def _run_all(P, w, ref_feat, ref_slot, ref_tex, ref_rgb, expect_fast=True):
             check_indices(s.cpu().numpy(), t.cpu().numpy(), ref_slot, ref_tex)
             check_features(f.float().cpu().numpy(), ref_feat)
     if expect_fast:
-        assert P.PATH_FUSED_MMA in results and P.PATH_FUSED_TC in results
+        assert P.PATH_FUSED_MMA in results and P.PATH_FUSED_TC in results and P.PATH_FUSED_TC_TMEM in results
         # same arithmetic in the same order: the fused and unfused specialised paths agree bit for bit
         assert np.array_equal(results[P.PATH_FUSED_MMA], results[P.PATH_UNFUSED])
     ctx.oo_set_path(P.PATH_AUTO)
@@ -177,7 +177,7 @@ def test_ragged_sizes(P, n):
     if n == 0:
         x = torch.empty((0, 3), device="cuda"); nn = x.clone(); wo = x.clone()
     ref = O.query(w.tree, w.atlas.levels, w.mlp.weights, q.x, q.nrm, q.wo) if n else np.zeros((0, 3))
-    for path in (P.PATH_GENERIC, P.PATH_UNFUSED, P.PATH_FUSED_MMA, P.PATH_FUSED_TC):
+    for path in (P.PATH_GENERIC, P.PATH_UNFUSED, P.PATH_FUSED_MMA, P.PATH_FUSED_TC, P.PATH_FUSED_TC_TMEM):
         ctx.oo_set_path(path)
         guard = torch.full((n + 8, 3), -7.0, device="cuda")
         ctx.oo_query(x, nn, wo, rgb=guard[:n])
@@ -202,10 +202,10 @@ def test_morton_sort_and_permuted_query(P):
     ctx.oo_set_path(P.PATH_FUSED_MMA)
     base_mma = ctx.oo_query(x, n, wo, ex).cpu().numpy()
     shuf = torch.from_numpy(gen.shuffle_perm(q.n, 0).astype(np.int32)).cuda()
-    for path in (P.PATH_GENERIC, P.PATH_UNFUSED, P.PATH_FUSED_MMA, P.PATH_FUSED_TC):
+    for path in (P.PATH_GENERIC, P.PATH_UNFUSED, P.PATH_FUSED_MMA, P.PATH_FUSED_TC, P.PATH_FUSED_TC_TMEM):
         ctx.oo_set_path(path)
         ref = ctx.oo_query(x, n, wo, ex).cpu().numpy()
-        if path != P.PATH_FUSED_TC:                      # the tcgen05 path sums in a different order
+        if path in (P.PATH_UNFUSED, P.PATH_FUSED_MMA):               # same arithmetic in the same order: bit for bit
             assert np.array_equal(ref, base_mma)
         else:
             assert np.abs(ref - base_mma).max() < 5e-3
