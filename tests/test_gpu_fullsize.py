@@ -28,7 +28,7 @@ def test_config1_full_frame_all_queries():
     x, n, wo = _dev(q.x), _dev(q.nrm), _dev(q.wo)
     got = ctx.oo_query(x, n, wo)
     torch.cuda.synchronize()
-    assert ctx.oo_get_info()["path_last_query"] == P.PATH_FUSED_TC
+    assert ctx.oo_get_info()["path_last_query"] == P.PATH_FUSED_TC_TMEM
     mx, mean = check_rgb(got.cpu().numpy(), ref)
     fe, sl, tx = ctx.oo_encode(x, wo, want_debug=True)
     check_indices(sl.cpu().numpy(), tx.cpu().numpy(), s, t)

@@ -60,7 +60,7 @@ def _run_all(P, w, ref_feat, ref_slot, ref_tex, ref_rgb, expect_fast=True):
     ctx.oo_set_path(P.PATH_AUTO)
     rgb = ctx.oo_query(x, n, wo, ex).cpu().numpy()
     info = ctx.oo_get_info()
-    assert info["path_last_query"] == (P.PATH_FUSED_TC if expect_fast else P.PATH_GENERIC)
+    assert info["path_last_query"] == (P.PATH_FUSED_TC_TMEM if expect_fast else P.PATH_GENERIC)
     check_rgb(rgb, ref_rgb)
     assert info["query_launches"] > 0
     ctx.close()
