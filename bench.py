@@ -253,6 +253,96 @@ def run_ours(args):
     return 0
 
 
+def run_sweep(args):
+    """BASELINE.json configs[2] / configs[4] side measurements (not the headline line): one JSON line with a table.
+
+    --sweep 2: config 2's frame in scanline order, Morton-sorted (oo_sort_queries; sort cost separate and included) and
+               seeded-shuffled order.  --sweep 4: config 3's tree and MLP, batch sizes 2^16..2^24, coherent (screen-order
+               hits of a 4096x4096 frame) and incoherent (area-weighted surface points, random order): encode-only and
+               fused Mqueries/s against the roofline.  CUDA events on the launching stream, L2 flushed between launches."""
+    import numpy as np
+    import torch
+    import gen
+    import paper_2606_08469_b200 as P
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    hbm, tf, which = peaks()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+    cu = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+
+    def timed(fn, reps):
+        for _ in range(3):
+            flush.zero_()
+            fn()
+        evs = []
+        for _ in range(reps):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+            evs.append((e0, e1))
+        torch.cuda.synchronize(dev)
+        t = sorted(a.elapsed_time(b) for a, b in evs)
+        return t[len(t) // 2]
+
+    rows = []
+    if args.sweep == 2:
+        w, desc = workload_for(2)
+        q = w.queries
+        ctx = P.OctaOctree(0).upload_workload(w)
+        ctx.oo_reserve(q.n)
+        x, nrm, wo, ex = cu(q.x), cu(q.nrm), cu(q.wo), cu(q.extra)
+        rgb = torch.empty((q.n, 3), dtype=torch.float32, device=dev)
+        perm = torch.empty(q.n, dtype=torch.int32, device=dev)
+        shuf = cu(gen.shuffle_perm(q.n, 0).astype(np.int32))
+        bq = desc["bytes_per_query"]
+        t_scan = timed(lambda: ctx.oo_query(x, nrm, wo, ex, rgb=rgb), args.steps)
+        t_sort = timed(lambda: ctx.oo_sort_queries(x, perm_out=perm), args.steps)
+        t_sorted = timed(lambda: ctx.oo_query(x, nrm, wo, ex, perm=perm, rgb=rgb), args.steps)
+        t_both = timed(lambda: (ctx.oo_sort_queries(x, perm_out=perm), ctx.oo_query(x, nrm, wo, ex, perm=perm, rgb=rgb)), args.steps)
+        t_shuf = timed(lambda: ctx.oo_query(x, nrm, wo, ex, perm=shuf, rgb=rgb), args.steps)
+        for name, t in (("scanline order", t_scan), ("morton-sorted (query only)", t_sorted), ("morton sort alone", t_sort),
+                        ("sort + query, output in caller order", t_both), ("seeded random shuffle", t_shuf)):
+            rows.append({"order": name, "ms": t, "Mqueries_per_s": q.n / t / 1e3, "roofline_frac": bq * q.n / (t * 1e-3) / 1e9 / hbm})
+        out = {"sweep": "BASELINE.json configs[2]: query order on the 1280x720 frame", "workload": desc["workload"], "rows": rows}
+    else:
+        w = gen.scene_workload(3, seed=0, width=64, height=64)          # config 3's scene, tree, atlas and MLP
+        L, F = len(w.tree.level_depth), w.atlas.F
+        bq_fused = L * 4 * F * 2 + 48
+        bq_enc = L * 4 * F * 2 + 24 + L * F * 2                           # x, wo in; features out
+        ctx = P.OctaOctree(0).upload_workload(w)
+        n_max = 1 << args.sweep_max_log2
+        side = 1 << ((args.sweep_max_log2 + 1) // 2)
+        cam = gen.make_camera(side, n_max // side, 0)
+        dists = {"coherent": gen.raycast(w.scene, cam), "incoherent": gen.incoherent_queries(w.scene, n_max, 0)}
+        ctx.oo_reserve(n_max)
+        feat = torch.empty((n_max, L * F), dtype=torch.float16, device=dev)
+        rgb = torch.empty((n_max, 3), dtype=torch.float32, device=dev)
+        for dname, q in dists.items():
+            X, Nn, W = cu(q.x), cu(q.nrm), cu(q.wo)
+            for lg in range(16, args.sweep_max_log2 + 1):
+                n = 1 << lg
+                x, nrm, wo = X[:n], Nn[:n], W[:n]
+                reps = max(5, min(args.steps, (1 << 26) // n))
+                t_f = timed(lambda: ctx.oo_query(x, nrm, wo, rgb=rgb[:n]), reps)
+                t_e = timed(lambda: ctx.oo_encode(x, wo, features=feat[:n]), reps)
+                rows.append({"distribution": dname, "n": n, "fused_ms": t_f, "fused_Mqueries_per_s": n / t_f / 1e3,
+                             "fused_roofline_frac": bq_fused * n / (t_f * 1e-3) / 1e9 / hbm,
+                             "encode_ms": t_e, "encode_Mqueries_per_s": n / t_e / 1e3,
+                             "encode_roofline_frac": bq_enc * n / (t_e * 1e-3) / 1e9 / hbm})
+        out = {"sweep": "BASELINE.json configs[4]: batch size x query distribution on the config-3 tree and MLP",
+               "tree_nodes": w.tree.n_nodes, "atlas_bytes": w.atlas.nbytes, "bytes_per_query": {"fused": bq_fused, "encode": bq_enc},
+               "rows": rows}
+    out.update({"unit": UNIT, "l2": "flushed between launches (256 MB memset)", "timing": "median of CUDA-event times",
+                "peak_gbs": hbm, "peak_source": which, "data": "synthetic"})
+    print(json.dumps(out))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -263,11 +353,15 @@ def main():
     ap.add_argument("--path", default="auto", choices=["auto", "mma", "tc", "tm", "unfused", "generic"])
     ap.add_argument("--ref-sample", type=int, default=131072, help="queries in the CPU-oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", type=int, default=0, choices=[0, 2, 4], help="side measurements of configs[2] / configs[4] (a table, not the headline line)")
+    ap.add_argument("--sweep-max-log2", type=int, default=24)
     ap.add_argument("--quick", action="store_true", help="timed region only (no warm-L2 / e2e / CPU legs): the command ncu wraps")
     args = ap.parse_args()
     # the reference arm is a CPU program: keep each step bounded whatever K the driver passes
     args.steps_ref = max(1, min(args.steps, 5))
     args.warmup_ref = max(0, min(args.warmup, 1))
+    if args.sweep:
+        return run_sweep(args)
     return run_reference(args) if args.impl == "reference" else run_ours(args)
 
 

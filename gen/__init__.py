@@ -28,6 +28,7 @@ STREAM_ATLAS = 100      # + level
 STREAM_WEIGHTS = 200    # + layer
 STREAM_POS, STREAM_NRM, STREAM_DIR, STREAM_ROUGH = 3, 4, 5, 6
 STREAM_SCENE, STREAM_CAMERA, STREAM_INCOH, STREAM_SHUFFLE = 7, 8, 9, 10
+STREAM_DISPARITY, STREAM_ALBEDO = 11, 12
 
 
 def build_lib(force: bool = False) -> str:
@@ -261,6 +262,47 @@ def make_atlas(tree: Tree, F: int, dtype: str, seed: int, std: float = 0.1, leve
             raise ValueError(dtype)
         out.append(a.reshape(S, R, R, F))
     return Atlas(F, dtype, out)
+
+
+def tie_vertex_map_borders(a: np.ndarray) -> np.ndarray:
+    """In place: give the boundary vertices of vertex-stored octahedral maps [..][n+1][n+1][F] the values of the vertices
+    they coincide with on the sphere ("the edge vertices are shared along adjacent faces", Fig. 3 caption):
+    (i, 0) = (n-i, 0), (i, n) = (n-i, n), (0, j) = (0, n-j), (n, j) = (n, n-j); the four corners are all the -z pole.
+    Input structure only (which stored entries are one and the same vertex), no interpolation arithmetic."""
+    n = a.shape[-2] - 1
+    for i in range(n // 2 + 1, n + 1):
+        a[..., 0, i, :] = a[..., 0, n - i, :]
+        a[..., n, i, :] = a[..., n, n - i, :]
+        a[..., i, 0, :] = a[..., n - i, 0, :]
+        a[..., i, n, :] = a[..., n - i, n, :]
+    a[..., 0, n, :] = a[..., 0, 0, :]
+    a[..., n, 0, :] = a[..., 0, 0, :]
+    a[..., n, n, :] = a[..., 0, 0, :]
+    return a
+
+
+def make_vertex_atlas(tree: Tree, F: int, dtype: str, seed: int, std: float = 0.1) -> Atlas:
+    """Vertex-stored maps (PAPER.md "features are stored at map vertices", vertex resolution n_l + 1 with n_l =
+    tree.level_res[l] intervals per axis): per used level [slots][n+1][n+1][F], same value distributions as make_atlas,
+    boundary vertices tied (tie_vertex_map_borders)."""
+    out = []
+    for l, (R, S) in enumerate(zip(tree.level_res, tree.level_slots)):
+        n = S * (R + 1) * (R + 1) * F
+        a = normal_f16(seed, STREAM_ATLAS + l, n, std) if dtype == "f16" else uniform_f32(seed, STREAM_ATLAS + l, n, -1.0, 1.0)
+        out.append(tie_vertex_map_borders(a.reshape(S, R + 1, R + 1, F)))
+    return Atlas(F, dtype, out)
+
+
+def disparity(n: int, seed: int, lo: float = 0.25, hi: float = 4.0) -> np.ndarray:
+    """Per-query disparity d^ (Eq. 7 output) as a synthetic input: U(lo, hi), i.e. virtual reflected points
+    0.25 .. 4 scene units away along the mirror direction."""
+    return uniform_f32(seed, STREAM_DISPARITY, n, lo, hi)
+
+
+def albedo_roughness(n: int, seed: int) -> np.ndarray:
+    """[n][4] = diffuse albedo a ~ U(0,1)^3 and roughness alpha ~ U(0.05,1): the extras of PAPER.md Eq. 12."""
+    a = uniform_f32(seed, STREAM_ALBEDO, 3 * n, 0.0, 1.0).reshape(n, 3)
+    return np.ascontiguousarray(np.concatenate([a, roughness(n, seed)], 1))
 
 
 def make_mlp(in_dim: int, n_hidden: int, seed: int, width: int = 64, out_dim: int = 3, out_act: str = "exp") -> MLP:
