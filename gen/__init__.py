@@ -444,3 +444,28 @@ def scene_workload(cfg: int, seed: int = 0, width: Optional[int] = None, height:
     mlp = make_mlp(len(depths) * F + 6 + n_extra, H, seed)
     return Workload("cfg%d" % cfg, tree, atlas, mlp, q, scene, cam,
                     {"width": width, "height": height, "n_extra": n_extra})
+
+
+def paper_workload(seed: int = 0, width: int = 1024, height: int = 1024, depths=None, res=None, F: int = 4,
+                   dtype: str = "f32", width_mlp: int = 128, n_hidden: int = 4, incoherent_n: int = 0) -> Workload:
+    """The paper's own shapes (PAPER.md "Implementation details": K = 8 consecutive levels with spatial resolution
+    (2^2)^3 .. (2^9)^3, vertex resolution 2^8+1 .. 2^1+1, C = 4 features per vertex; decoder 4 hidden layers x 128) on the
+    three-sphere stand-in scene of config 1: used depths 2..9, R_l = 256 .. 2 intervals (vertex maps, fp32 as Table 2's
+    16 bytes per entry implies), queries = the primary hits of a width x height frame plus the attributes of Eq. 12
+    (albedo, roughness as extras) and a synthetic per-query disparity (Eq. 7's output).  ``depths``/``res`` give reduced
+    variants of the same recipe for tests.  meta["disparity"] holds d^, meta["dirmap"] = "vertex"."""
+    depths = list(range(2, 10)) if depths is None else [int(d) for d in depths]
+    res = [1 << (10 - d) for d in depths] if res is None else [int(r) for r in res]
+    scene = make_scene("three", seed)
+    tree = build_tree(scene, depths[-1]).set_levels(depths, res)
+    atlas = make_vertex_atlas(tree, F, dtype, seed)
+    cam = None
+    if incoherent_n:
+        q = incoherent_queries(scene, incoherent_n, seed)
+    else:
+        cam = make_camera(width, height, seed)
+        q = raycast(scene, cam)
+    q.extra = albedo_roughness(q.n, seed)
+    mlp = make_mlp(len(depths) * F + 9 + 4, n_hidden, seed, width=width_mlp)
+    return Workload("paper", tree, atlas, mlp, q, scene, cam,
+                    {"width": width, "height": height, "n_extra": 4, "disparity": disparity(q.n, seed), "dirmap": "vertex"})

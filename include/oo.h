@@ -12,7 +12,10 @@
  *   3. concatenate the per-level features (Eq. 11) with the per-query attributes (Eq. 12-13);
  *   4. decode with a small MLP (hidden width 64, ReLU, no biases) to RGB.
  * This is the nearest-cell / raw-direction variant that the paper itself names as ablations; see
- * DESIGN.md §1 for the differences from the full method.
+ * DESIGN.md §1 for the differences from the full method.  The paper's full query is selected piece by piece with
+ * oo_set_mode (8-neighbour trilinear blend, Eq. 10; mirror / disparity-shifted lookup direction, Eq. 8-9; the attribute
+ * vector of Eq. 12) and oo_tree_desc.dirmap (vertex-stored maps with barycentric taps, Eq. 6); decoders of width 64 or
+ * 128.  See "The paper's full query" below.
  *
  * Conventions
  *   - Every pointer is marked HOST or DEVICE.  DEVICE pointers must belong to the context's CUDA device.
@@ -60,6 +63,32 @@ typedef enum {
 typedef enum { OO_F16 = 0, OO_F32 = 1 } oo_dtype;
 typedef enum { OO_ACT_NONE = 0, OO_ACT_EXP = 1 } oo_out_act;
 
+/* ---- The paper's full query.  All-zero = the hot path described above. ---- */
+/* f1, Eq. 10: features sit at cell centres; with p = clamp(x,0,1)*2^d - 1/2, k0 = floor(p), t = p - k0 the
+ * eight cells k0 + {0,1}^3 are blended with trilinear weights prod(t or 1-t), restricted to the non-empty cells inside
+ * the grid and renormalised by the sum of the surviving weights (none survives => zero features). */
+typedef enum { OO_SPATIAL_NEAREST = 0, OO_SPATIAL_TRILINEAR8 = 1 } oo_spatial;
+/* f2, Eq. 6: OO_DIRMAP_VERTEX stores every map as (R+1) x (R+1) VERTICES of the unfolded octahedral
+ * grid with R intervals per axis; the lookup finds the grid cell (ci, cj) = min(floor((u+1)/2*R), R-1), splits it along
+ * the anti-diagonal where u_x*u_y > 0 (cell in a same-sign quadrant) and along the main diagonal otherwise, so that the
+ * hypotenuses run parallel to the octahedron's face edges, and takes the barycentric combination of the containing
+ * triangle's three vertices.  Boundary vertices that coincide on the sphere are stored separately; the library reads
+ * them as given (tying them is the owner's concern). */
+typedef enum { OO_DIRMAP_TEXEL = 0, OO_DIRMAP_VERTEX = 1 } oo_dirmap;
+/* f3, P:135 and Eq. 8-9: the direction that indexes the maps.  WO: wo itself.  MIRROR: w_r = 2(n.wo)n - wo.
+ * SHIFTED: per cell j with centre c_j, w~_j = (x - c_j)*d^ + w_r (Eq. 9 before normalisation; Eq. 4 is scale invariant),
+ * d^ = oo_queries.disparity (the output of the disparity predictor of Eq. 7, supplied per query).  Directions are formed
+ * in fp32, one rounding per operation, in the order DESIGN.md "Index contract (full query)" fixes. */
+typedef enum { OO_LOOKUP_WO = 0, OO_LOOKUP_MIRROR = 1, OO_LOOKUP_SHIFTED = 2 } oo_lookup;
+/* f4, Eq. 12: decoder input after the features.  N_WO: [n | wo | extra].  PAPER: [x | w_r | n | extra]
+ * (extra = albedo a, roughness alpha, ... as supplied). */
+typedef enum { OO_ATTRS_N_WO = 0, OO_ATTRS_PAPER = 1 } oo_attrs;
+typedef struct {
+    oo_spatial spatial;
+    oo_lookup lookup;
+    oo_attrs attrs;
+} oo_mode;
+
 /* Which kernels oo_encode / oo_query run.  Every choice computes the same function; all are CUDA. */
 typedef enum {
     OO_PATH_AUTO = 0,        /* fastest available for the uploaded shapes */
@@ -67,7 +96,9 @@ typedef enum {
     OO_PATH_UNFUSED = 2,     /* hop-table descent, specialised gather; features round-trip HBM; MLP kernel */
     OO_PATH_FUSED_MMA = 3,   /* one kernel: gather -> shared memory -> mma.sync MLP -> RGB */
     OO_PATH_FUSED_TC = 4,    /* one kernel: gather -> shared memory -> tcgen05.mma (TMEM accumulators) -> RGB */
-    OO_PATH_FUSED_TC_TMEM = 5 /* the same with the activations (A operand) kept in tensor memory: no shared-memory A tile */
+    OO_PATH_FUSED_TC_TMEM = 5, /* the same with the activations (A operand) kept in tensor memory: no shared-memory A tile */
+    OO_PATH_FULL = 6         /* reported by oo_get_info when the full-query kernels ran (mode != 0, vertex maps or width 128);
+                                not selectable with oo_set_path */
 } oo_path;
 
 /* The octree and its feature atlases ("every non-empty cell stores a learnable octahedral feature map").
@@ -87,15 +118,17 @@ typedef struct {
     const uint32_t* level_slots; /* HOST [L] number of maps in level l (= number of nodes at that depth) */
     uint32_t n_features;         /* F; F * sizeof(dtype) must be 16, 32 or 64 bytes */
     oo_dtype dtype;              /* storage type of the texels */
-    const void* const* atlas;    /* HOST array [L] of DEVICE pointers, each [level_slots[l]][R_l][R_l][F], 16-byte aligned */
+    const void* const* atlas;    /* HOST array [L] of DEVICE pointers, each [level_slots[l]][R_l][R_l][F], 16-byte aligned
+                                    (OO_DIRMAP_VERTEX: [level_slots[l]][R_l+1][R_l+1][F]) */
+    oo_dirmap dirmap;            /* OO_DIRMAP_TEXEL (0): texel-centred maps, bilinear taps, border wrap; OO_DIRMAP_VERTEX */
 } oo_tree_desc;
 
 /* Decoder f_phi: n_hidden x (linear width x in, ReLU), then linear out_dim x width, then out_act.
  * No biases (A10).  fp16 weights, row-major [out][in].  in_dim must equal L*F + 6 + n_extra of the queries:
- * input order [h_0 .. h_{L-1} | n | wo | extra] (A7). */
+ * input order [h_0 .. h_{L-1} | n | wo | extra] (A7); with OO_ATTRS_PAPER L*F + 9 + n_extra: [h | x | w_r | n | extra]. */
 typedef struct {
     uint32_t in_dim;
-    uint32_t width;              /* must be 64 */
+    uint32_t width;              /* 64, or 128 (the paper's decoder; runs on the full-query kernels) */
     uint32_t n_hidden;           /* 1..OO_MAX_HIDDEN */
     uint32_t out_dim;            /* 1..8 (3 = RGB) */
     const void* const* weights;  /* HOST array [n_hidden+1] of HOST pointers to fp16 matrices:
@@ -114,6 +147,7 @@ typedef struct {
     uint32_t n_extra;            /* 0..OO_MAX_EXTRA (roughness: 1) */
     const uint32_t* perm;        /* optional DEVICE [n]: processing order (thread t handles query perm[t]); results are
                                     always written at the query's own index, i.e. in the caller's order.  NULL = identity */
+    const float* disparity;      /* [n] d^ of Eq. 7-9, required by OO_LOOKUP_SHIFTED, ignored otherwise (may be NULL) */
 } oo_queries;
 
 typedef struct {
@@ -146,6 +180,9 @@ OO_API oo_status oo_reserve(oo_ctx* ctx, uint64_t max_queries);
  * shapes have no such kernel. */
 OO_API oo_status oo_set_path(oo_ctx* ctx, oo_path path);
 OO_API oo_status oo_get_info(const oo_ctx* ctx, oo_info* out);
+/* Select the variant of the query (default all-zero = the hot path).  Takes effect from the next oo_encode_full /
+ * oo_query.  OO_LOOKUP_SHIFTED needs oo_queries.disparity; OO_ATTRS_PAPER changes the expected MLP in_dim. */
+OO_API oo_status oo_set_mode(oo_ctx* ctx, const oo_mode* mode);
 
 /* Row a1: d_perm_out[k] = index of the k-th query in ascending order of the 30-bit Morton key of
  * clamp(floor(x*1024), 0, 1023) (bit b of q_x -> key bit 3b, q_y -> 3b+1, q_z -> 3b+2), ties in original order
@@ -159,7 +196,18 @@ OO_API oo_status oo_sort_queries(oo_ctx* ctx, const oo_queries* q, uint32_t* d_p
 OO_API oo_status oo_encode(oo_ctx* ctx, const oo_queries* q, void* d_features, int32_t* d_slot, int16_t* d_texel,
                     void* cuda_stream);
 
-/* The whole path.  d_rgb: DEVICE [n][out_dim] fp32, written at each query's own index. */
+/* Steps 1-3 under the current oo_mode and the tree's dirmap (any combination, the all-zero mode included).
+ * d_features: DEVICE [n][L*F] fp32.  J = 8 neighbours (OO_SPATIAL_TRILINEAR8, j = a | b<<1 | c<<2 for cell k0 + (a,b,c))
+ * or 1 (nearest).  Optional debug outputs: d_slot DEVICE [n][L][J] atlas slot of each neighbour (-1 = outside the grid or
+ * empty); d_cell DEVICE [n][L][J][3] = the directional index decision for that neighbour's lookup direction: texel maps
+ * (i0, j0, 0) as in oo_encode, vertex maps (ci, cj, upper) with upper = 1 for the triangle that holds local corner (1,1)
+ * [anti-diagonal split] / (0,1) [main-diagonal split]. */
+OO_API oo_status oo_encode_full(oo_ctx* ctx, const oo_queries* q, float* d_features, int32_t* d_slot, int16_t* d_cell,
+                         void* cuda_stream);
+
+/* The whole path.  d_rgb: DEVICE [n][out_dim] fp32, written at each query's own index.  Runs the hot-path kernels when
+ * the mode is all-zero, the maps are texel maps and the decoder is 64 wide; otherwise the full-query kernel (one fused
+ * launch as well). */
 OO_API oo_status oo_query(oo_ctx* ctx, const oo_queries* q, float* d_rgb, void* cuda_stream);
 
 /* The whole path from HOST buffers: copies the queries to the device (cudaMemcpyAsync on the stream), runs oo_query,

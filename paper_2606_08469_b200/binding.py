@@ -8,13 +8,18 @@ from typing import List, Optional, Sequence
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "liboo.so")
 
-PATH_AUTO, PATH_GENERIC, PATH_UNFUSED, PATH_FUSED_MMA, PATH_FUSED_TC, PATH_FUSED_TC_TMEM = 0, 1, 2, 3, 4, 5
+PATH_AUTO, PATH_GENERIC, PATH_UNFUSED, PATH_FUSED_MMA, PATH_FUSED_TC, PATH_FUSED_TC_TMEM, PATH_FULL = 0, 1, 2, 3, 4, 5, 6
+SPATIAL = {"nearest": 0, "trilinear8": 1}
+DIRMAP = {"texel": 0, "vertex": 1}
+LOOKUP = {"wo": 0, "mirror": 1, "shifted": 2}
+ATTRS = {"n_wo": 0, "paper": 1}
 OO_F16, OO_F32 = 0, 1
 OO_ACT_NONE, OO_ACT_EXP = 0, 1
 _STATUS = {0: "OO_OK", 1: "OO_ERR_INVALID_ARG", 2: "OO_ERR_NOT_READY", 3: "OO_ERR_UNSUPPORTED", 4: "OO_ERR_CUDA", 5: "OO_ERR_OOM"}
 
 EXPORTED_SYMBOLS = ["oo_create", "oo_destroy", "oo_last_error", "oo_upload_tree", "oo_upload_mlp", "oo_reserve", "oo_set_path",
-                    "oo_get_info", "oo_sort_queries", "oo_encode", "oo_query", "oo_query_host", "oo_read_padded_map"]
+                    "oo_get_info", "oo_sort_queries", "oo_encode", "oo_query", "oo_query_host", "oo_read_padded_map", "oo_set_mode",
+                    "oo_encode_full"]
 
 
 class OOError(RuntimeError):
@@ -26,7 +31,8 @@ class OOError(RuntimeError):
 class _TreeDesc(C.Structure):
     _fields_ = [("n_nodes", C.c_uint32), ("max_depth", C.c_uint32), ("child", C.c_void_p), ("depth", C.c_void_p),
                 ("map_slot", C.c_void_p), ("n_levels", C.c_uint32), ("level_depth", C.c_void_p), ("level_res", C.c_void_p),
-                ("level_slots", C.c_void_p), ("n_features", C.c_uint32), ("dtype", C.c_int), ("atlas", C.c_void_p)]
+                ("level_slots", C.c_void_p), ("n_features", C.c_uint32), ("dtype", C.c_int), ("atlas", C.c_void_p),
+                ("dirmap", C.c_int)]
 
 
 class _MlpDesc(C.Structure):
@@ -36,7 +42,11 @@ class _MlpDesc(C.Structure):
 
 class _Queries(C.Structure):
     _fields_ = [("n", C.c_uint64), ("x", C.c_void_p), ("nrm", C.c_void_p), ("wo", C.c_void_p), ("extra", C.c_void_p),
-                ("n_extra", C.c_uint32), ("perm", C.c_void_p)]
+                ("n_extra", C.c_uint32), ("perm", C.c_void_p), ("disparity", C.c_void_p)]
+
+
+class _Mode(C.Structure):
+    _fields_ = [("spatial", C.c_int), ("lookup", C.c_int), ("attrs", C.c_int)]
 
 
 class _Info(C.Structure):
@@ -76,6 +86,8 @@ def load_library():
     L.oo_query.argtypes = [vp, C.POINTER(_Queries), vp, vp]
     L.oo_query_host.argtypes = [vp, C.POINTER(_Queries), vp, vp]
     L.oo_read_padded_map.argtypes = [vp, u32, u32, vp]
+    L.oo_set_mode.argtypes = [vp, C.POINTER(_Mode)]
+    L.oo_encode_full.argtypes = [vp, C.POINTER(_Queries), vp, vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
         if name not in ("oo_destroy", "oo_last_error"):
             getattr(L, name).restype = C.c_int
@@ -103,6 +115,7 @@ class OctaOctree:
         self.n_levels = self.n_features = 0
         self.dtype = None
         self.out_dim = 3
+        self.n_neighbours = 1
 
     def close(self):
         if self._ctx:
@@ -123,9 +136,9 @@ class OctaOctree:
         return C.c_void_p(self._torch.cuda.current_stream(self.device).cuda_stream)
 
     # ---------------------------------------------------------------- uploads
-    def oo_upload_tree(self, tree, atlas_levels: Sequence, dtype: str):
+    def oo_upload_tree(self, tree, atlas_levels: Sequence, dtype: str, dirmap: str = "texel"):
         """tree: object with n_nodes, max_depth, child, depth, map_slot, level_depth, level_res, level_slots (numpy / lists).
-        atlas_levels: per level a numpy array or a torch CUDA tensor [slots][R][R][F]."""
+        atlas_levels: per level a numpy array or a torch CUDA tensor [slots][R][R][F] (dirmap "vertex": [slots][R+1][R+1][F])."""
         import numpy as np
         torch = self._torch
         child = np.ascontiguousarray(tree.child, np.int32)
@@ -143,7 +156,7 @@ class OctaOctree:
         F = int(dev[0].shape[-1])
         ptrs = (C.c_void_p * len(dev))(*[t.data_ptr() if t.numel() else None for t in dev])
         d = _TreeDesc(child.shape[0], int(tree.max_depth), _np_ptr(child), _np_ptr(depth), _np_ptr(slot), len(dev), _np_ptr(ld),
-                      _np_ptr(lr), _np_ptr(ls), F, OO_F16 if dtype == "f16" else OO_F32, C.cast(ptrs, C.c_void_p))
+                      _np_ptr(lr), _np_ptr(ls), F, OO_F16 if dtype == "f16" else OO_F32, C.cast(ptrs, C.c_void_p), DIRMAP[dirmap])
         self._check(self._L.oo_upload_tree(self._ctx, C.byref(d), self._stream()))
         self.n_levels, self.n_features, self.dtype = len(dev), F, dtype
         del dev
@@ -163,22 +176,28 @@ class OctaOctree:
     def oo_set_path(self, path: int):
         self._check(self._L.oo_set_path(self._ctx, int(path)))
 
+    def oo_set_mode(self, spatial: str = "nearest", lookup: str = "wo", attrs: str = "n_wo"):
+        m = _Mode(SPATIAL[spatial], LOOKUP[lookup], ATTRS[attrs])
+        self._check(self._L.oo_set_mode(self._ctx, C.byref(m)))
+        self.n_neighbours = 8 if spatial == "trilinear8" else 1
+
     def oo_get_info(self) -> dict:
         info = _Info()
         self._check(self._L.oo_get_info(self._ctx, C.byref(info)))
         return {k: int(getattr(info, k)) for k, _ in _Info._fields_}
 
     # ---------------------------------------------------------------- queries
-    def _queries(self, x, nrm, wo, extra, perm):
+    def _queries(self, x, nrm, wo, extra, perm, disparity=None):
         torch = self._torch
-        for t in (x, nrm, wo, extra, perm):
+        for t in (x, nrm, wo, extra, perm, disparity):
             if t is not None:
                 assert t.is_cuda and t.is_contiguous(), "queries must be contiguous CUDA tensors"
         assert x.dtype == torch.float32 and wo.dtype == torch.float32
         n = int(x.shape[0])
         ne = 0 if extra is None else int(extra.numel() // max(n, 1))
         q = _Queries(n, x.data_ptr(), nrm.data_ptr() if nrm is not None else None, wo.data_ptr(),
-                     extra.data_ptr() if extra is not None else None, ne, perm.data_ptr() if perm is not None else None)
+                     extra.data_ptr() if extra is not None else None, ne, perm.data_ptr() if perm is not None else None,
+                     disparity.data_ptr() if disparity is not None else None)
         return q, n
 
     def oo_sort_queries(self, x, perm_out=None):
@@ -205,15 +224,29 @@ class OctaOctree:
                                       C.c_void_p(texel.data_ptr()) if want_debug else None, self._stream()))
         return (features, slot, texel) if want_debug else features
 
-    def oo_query(self, x, nrm, wo, extra=None, perm=None, rgb=None):
+    def oo_encode_full(self, x, nrm, wo, disparity=None, perm=None, want_debug: bool = False):
+        """features fp32 [n][L*F] under the current mode; with want_debug also slots [n][L][J] and cells [n][L][J][3]."""
         torch = self._torch
-        q, n = self._queries(x, nrm, wo, extra, perm)
+        q, n = self._queries(x, nrm, wo, None, perm, disparity)
+        features = torch.empty((n, self.n_levels * self.n_features), dtype=torch.float32, device=self.device)
+        slot = cell = None
+        if want_debug:
+            slot = torch.empty((n, self.n_levels, self.n_neighbours), dtype=torch.int32, device=self.device)
+            cell = torch.empty((n, self.n_levels, self.n_neighbours, 3), dtype=torch.int16, device=self.device)
+        self._check(self._L.oo_encode_full(self._ctx, C.byref(q), C.c_void_p(features.data_ptr()),
+                                           C.c_void_p(slot.data_ptr()) if want_debug else None,
+                                           C.c_void_p(cell.data_ptr()) if want_debug else None, self._stream()))
+        return (features, slot, cell) if want_debug else features
+
+    def oo_query(self, x, nrm, wo, extra=None, perm=None, rgb=None, disparity=None):
+        torch = self._torch
+        q, n = self._queries(x, nrm, wo, extra, perm, disparity)
         if rgb is None:
             rgb = torch.empty((n, self.out_dim), dtype=torch.float32, device=self.device)
         self._check(self._L.oo_query(self._ctx, C.byref(q), C.c_void_p(rgb.data_ptr()), self._stream()))
         return rgb
 
-    def oo_query_host(self, x, nrm, wo, extra=None, rgb=None):
+    def oo_query_host(self, x, nrm, wo, extra=None, rgb=None, disparity=None):
         """x, nrm, wo, extra, rgb: CPU tensors (pinned for asynchronous copies) or numpy arrays.  Synchronous."""
         torch = self._torch
         n = int(x.shape[0])
@@ -225,7 +258,7 @@ class OctaOctree:
         ne = 0 if extra is None else int((extra.numel() if isinstance(extra, torch.Tensor) else extra.size) // max(n, 1))
         if rgb is None:
             rgb = torch.empty((n, self.out_dim), dtype=torch.float32).pin_memory()
-        q = _Queries(n, ptr(x), ptr(nrm), ptr(wo), ptr(extra), ne, None)
+        q = _Queries(n, ptr(x), ptr(nrm), ptr(wo), ptr(extra), ne, None, ptr(disparity))
         self._check(self._L.oo_query_host(self._ctx, C.byref(q), C.c_void_p(ptr(rgb)), self._stream()))
         return rgb
 
@@ -236,7 +269,7 @@ class OctaOctree:
         return out
 
     # convenience: upload a gen.Workload
-    def upload_workload(self, w):
-        self.oo_upload_tree(w.tree, w.atlas.levels, w.atlas.dtype)
+    def upload_workload(self, w, dirmap: str = "texel"):
+        self.oo_upload_tree(w.tree, w.atlas.levels, w.atlas.dtype, dirmap)
         self.oo_upload_mlp(w.mlp.weights, w.mlp.out_act)
         return self

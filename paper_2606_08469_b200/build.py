@@ -11,7 +11,8 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liboo.so")
-SOURCES = ["oo_api.cu", "oo_kernels.cu", "oo_fused_tc.cu", "oo_fused_tm.cu", "oo_sort.cu"]
+SOURCES = ["oo_api.cu", "oo_kernels.cu", "oo_fused_tc.cu", "oo_fused_tm.cu", "oo_sort.cu",
+           "oo_full_encode.cu", "oo_full_fused_w64.cu", "oo_full_fused_w128.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
               "-Xcompiler", "-fvisibility=hidden", "-I", os.path.join(ROOT, "include"), "-I", CSRC] + os.environ.get("OO_NVCC_EXTRA", "").split()
 
@@ -50,7 +51,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(" ".join(cmd) + "\n" + r.stdout + r.stderr)
         if r.returncode:
             raise RuntimeError("nvcc failed: " + " ".join(cmd))
-    with ThreadPoolExecutor(max_workers=4) as ex:
+    with ThreadPoolExecutor(max_workers=8) as ex:
         list(ex.map(run, jobs))
     if force or jobs or _stale(LIB, objs):
         tmp = LIB + ".tmp%d" % os.getpid()

@@ -20,6 +20,7 @@ struct oo_ctx {
     std::string err;
     cudaError_t sticky = cudaSuccess;
     oo_path path = OO_PATH_AUTO;
+    FullModeH mode{0, 0, 0};
     oo_info info{};
 
     // tree
@@ -44,7 +45,7 @@ struct oo_ctx {
     uint64_t reserved = 0;
     void* d_feat = nullptr;    uint64_t feat_bytes = 0;
     uint32_t *d_keys_a = nullptr, *d_keys_b = nullptr, *d_idx_a = nullptr, *d_hist = nullptr;
-    float *d_qx = nullptr, *d_qn = nullptr, *d_qw = nullptr, *d_qe = nullptr, *d_rgb = nullptr;
+    float *d_qx = nullptr, *d_qn = nullptr, *d_qw = nullptr, *d_qe = nullptr, *d_rgb = nullptr, *d_qd = nullptr;
 };
 
 namespace {
@@ -103,7 +104,7 @@ void free_scratch(oo_ctx* c) {
     free_dev(c->d_feat);
     c->feat_bytes = 0;
     void** ps[] = {(void**)&c->d_keys_a, (void**)&c->d_keys_b, (void**)&c->d_idx_a, (void**)&c->d_hist, (void**)&c->d_qx,
-                   (void**)&c->d_qn,     (void**)&c->d_qw,     (void**)&c->d_qe,    (void**)&c->d_rgb};
+                   (void**)&c->d_qn,     (void**)&c->d_qw,     (void**)&c->d_qe,    (void**)&c->d_rgb, (void**)&c->d_qd};
     for (void** p : ps) free_dev(*p);
     c->reserved = 0;
 }
@@ -134,6 +135,7 @@ oo_status check_queries(oo_ctx* c, const oo_queries* q, bool need_nrm) {
 QueryParams make_qp(const oo_queries* q) {
     QueryParams Q{};
     Q.n = q->n; Q.x = q->x; Q.nrm = q->nrm; Q.wo = q->wo; Q.extra = q->extra; Q.n_extra = q->n_extra; Q.perm = q->perm;
+    Q.disparity = q->disparity;
     return Q;
 }
 
@@ -193,6 +195,18 @@ extern "C" OO_API oo_status oo_set_path(oo_ctx* c, oo_path path) {
     return OO_OK;
 }
 
+extern "C" OO_API oo_status oo_set_mode(oo_ctx* c, const oo_mode* m) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (!m) return fail(c, OO_ERR_INVALID_ARG, "mode is NULL");
+    if ((int)m->spatial < 0 || (int)m->spatial > (int)OO_SPATIAL_TRILINEAR8 || (int)m->lookup < 0 || (int)m->lookup > (int)OO_LOOKUP_SHIFTED ||
+        (int)m->attrs < 0 || (int)m->attrs > (int)OO_ATTRS_PAPER)
+        return fail(c, OO_ERR_INVALID_ARG, "unknown mode value (spatial %d, lookup %d, attrs %d)", (int)m->spatial, (int)m->lookup, (int)m->attrs);
+    c->mode.tri8 = m->spatial == OO_SPATIAL_TRILINEAR8;
+    c->mode.lookup = (uint32_t)m->lookup;
+    c->mode.attrs_paper = m->attrs == OO_ATTRS_PAPER;
+    return OO_OK;
+}
+
 extern "C" OO_API oo_status oo_get_info(const oo_ctx* c, oo_info* out) {
     if (!c || !out) return OO_ERR_INVALID_ARG;
     *out = c->info;
@@ -214,6 +228,8 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
     if (t->n_levels == 0 || t->n_levels > OO_MAX_LEVELS) return fail(c, OO_ERR_INVALID_ARG, "n_levels %u outside 1..%d", t->n_levels, OO_MAX_LEVELS);
     if (!t->level_depth || !t->level_res || !t->level_slots || !t->atlas) return fail(c, OO_ERR_INVALID_ARG, "NULL level arrays");
     if (t->dtype != OO_F16 && t->dtype != OO_F32) return fail(c, OO_ERR_INVALID_ARG, "unknown dtype");
+    if (t->dirmap != OO_DIRMAP_TEXEL && t->dirmap != OO_DIRMAP_VERTEX) return fail(c, OO_ERR_INVALID_ARG, "unknown dirmap");
+    const bool vertex = t->dirmap == OO_DIRMAP_VERTEX;
     const uint32_t esize = t->dtype == OO_F32 ? 4 : 2;
     const uint32_t texel_bytes = t->n_features * esize;
     if (texel_bytes != 16 && texel_bytes != 32 && texel_bytes != 64)
@@ -269,6 +285,7 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
     free_tree(c);
     TreeParams T{};
     T.n_levels = L; T.F = t->n_features; T.f32 = t->dtype == OO_F32; T.texel_bytes = texel_bytes;
+    T.vertex = vertex ? 1u : 0u;
     T.depth_eff = t->level_depth[L - 1];
     T.scale_eff = (float)(1u << T.depth_eff);
     c->tree_max_depth = D;
@@ -279,15 +296,17 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
     uint64_t atlas_bytes = 0;
     int launches = 0;
     for (uint32_t l = 0; l < L; ++l) {
-        const uint32_t R = t->level_res[l], Rp = R + 2;
+        // texel maps: (R+2)^2 with the wrapped border; vertex maps: the (R+1)^2 vertices as given
+        const uint32_t R = t->level_res[l], Rp = vertex ? R + 1 : R + 2;
         const uint64_t slots = std::max<uint64_t>(t->level_slots[l], 1);      // at least one (zero) map, so that the branch-free gather has an address
         const uint64_t bytes = slots * Rp * Rp * texel_bytes;
         OO_CUDA(c, cudaMalloc(&c->atlas_dev[l], bytes));
         atlas_bytes += bytes;
         if (t->level_slots[l] == 0) OO_CUDA(c, cudaMemsetAsync(c->atlas_dev[l], 0, bytes, stream));
+        else if (vertex) OO_CUDA(c, cudaMemcpyAsync(c->atlas_dev[l], t->atlas[l], bytes, cudaMemcpyDeviceToDevice, stream));
         else launches += launch_pad_atlas(t->atlas[l], c->atlas_dev[l], t->level_slots[l], R, texel_bytes, stream);
         LevelParams& lv = T.lv[l];
-        lv.atlas = (const uint8_t*)c->atlas_dev[l] + (uint64_t)(Rp + 1) * texel_bytes;
+        lv.atlas = (const uint8_t*)c->atlas_dev[l] + (vertex ? 0 : (uint64_t)(Rp + 1) * texel_bytes);
         lv.half_r = 0.5f * (float)R;
         lv.off = 0.5f * (float)R - 0.5f;
         lv.R = R; lv.Rp = Rp;
@@ -425,7 +444,8 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
 extern "C" OO_API oo_status oo_upload_mlp(oo_ctx* c, const oo_mlp_desc* m, void* cuda_stream) {
     if (!c) return OO_ERR_INVALID_ARG;
     if (!m || !m->weights) return fail(c, OO_ERR_INVALID_ARG, "mlp or mlp.weights is NULL");
-    if (m->width != 64) return fail(c, OO_ERR_UNSUPPORTED, "hidden width %u: only 64 is implemented", m->width);
+    if (m->width != 64 && m->width != 128) return fail(c, OO_ERR_UNSUPPORTED, "hidden width %u: only 64 and 128 are implemented", m->width);
+    const uint32_t W = m->width;
     if (m->n_hidden < 1 || m->n_hidden > OO_MAX_HIDDEN) return fail(c, OO_ERR_INVALID_ARG, "n_hidden %u outside 1..%d", m->n_hidden, OO_MAX_HIDDEN);
     if (m->out_dim < 1 || m->out_dim > 8) return fail(c, OO_ERR_INVALID_ARG, "out_dim %u outside 1..8", m->out_dim);
     if (m->in_dim < 7 || m->in_dim > OO_MAX_LEVELS * 32 + 6 + OO_MAX_EXTRA) return fail(c, OO_ERR_INVALID_ARG, "in_dim %u out of range", m->in_dim);
@@ -437,36 +457,37 @@ extern "C" OO_API oo_status oo_upload_mlp(oo_ctx* c, const oo_mlp_desc* m, void*
     const uint32_t k1 = (m->in_dim + 15) & ~15u;
     const uint32_t s0 = k1 + 8, s1 = 72;
     const size_t halves = (size_t)64 * s0 + (size_t)(m->n_hidden - 1) * 64 * s1 + (size_t)16 * s1;
-    std::vector<uint16_t> img(halves, 0);
+    std::vector<uint16_t> img(halves, 0);     // the mma.sync image (width 64 only; left zero otherwise and never used)
     const uint16_t* w0 = (const uint16_t*)m->weights[0];
+    if (W == 64)
     for (uint32_t o = 0; o < 64; ++o)
         for (uint32_t i = 0; i < m->in_dim; ++i) img[(size_t)o * s0 + i] = w0[(size_t)o * m->in_dim + i];
     size_t off = (size_t)64 * s0;
-    for (uint32_t k = 1; k < m->n_hidden; ++k) {
+    for (uint32_t k = 1; W == 64 && k < m->n_hidden; ++k) {
         const uint16_t* w = (const uint16_t*)m->weights[k];
         for (uint32_t o = 0; o < 64; ++o)
             for (uint32_t i = 0; i < 64; ++i) img[off + (size_t)o * s1 + i] = w[(size_t)o * 64 + i];
         off += (size_t)64 * s1;
     }
     const uint16_t* wl = (const uint16_t*)m->weights[m->n_hidden];
-    for (uint32_t o = 0; o < m->out_dim; ++o)
+    for (uint32_t o = 0; W == 64 && o < m->out_dim; ++o)
         for (uint32_t i = 0; i < 64; ++i) img[off + (size_t)o * s1 + i] = wl[(size_t)o * 64 + i];
     // tensor-core image: chunk-major [K/8][N][8] per layer
-    const size_t tc_halves = (size_t)k1 * 64 + (size_t)(m->n_hidden - 1) * 64 * 64 + (size_t)64 * 16;
+    const size_t tc_halves = (size_t)k1 * W + (size_t)(m->n_hidden - 1) * W * W + (size_t)W * 16;
     std::vector<uint16_t> tc(tc_halves, 0);
     {
         auto put = [&](size_t base, uint32_t N, uint32_t n, uint32_t k, uint16_t v) { tc[base + ((size_t)(k / 8) * N + n) * 8 + (k % 8)] = v; };
-        for (uint32_t o = 0; o < 64; ++o)
-            for (uint32_t i = 0; i < m->in_dim; ++i) put(0, 64, o, i, w0[(size_t)o * m->in_dim + i]);
-        size_t base = (size_t)k1 * 64;
+        for (uint32_t o = 0; o < W; ++o)
+            for (uint32_t i = 0; i < m->in_dim; ++i) put(0, W, o, i, w0[(size_t)o * m->in_dim + i]);
+        size_t base = (size_t)k1 * W;
         for (uint32_t k = 1; k < m->n_hidden; ++k) {
             const uint16_t* w = (const uint16_t*)m->weights[k];
-            for (uint32_t o = 0; o < 64; ++o)
-                for (uint32_t i = 0; i < 64; ++i) put(base, 64, o, i, w[(size_t)o * 64 + i]);
-            base += (size_t)64 * 64;
+            for (uint32_t o = 0; o < W; ++o)
+                for (uint32_t i = 0; i < W; ++i) put(base, W, o, i, w[(size_t)o * W + i]);
+            base += (size_t)W * W;
         }
         for (uint32_t o = 0; o < m->out_dim; ++o)
-            for (uint32_t i = 0; i < 64; ++i) put(base, 16, o, i, wl[(size_t)o * 64 + i]);
+            for (uint32_t i = 0; i < W; ++i) put(base, 16, o, i, wl[(size_t)o * W + i]);
     }
     free_dev(c->d_image);
     free_dev(c->d_image_tc);
@@ -483,6 +504,7 @@ extern "C" OO_API oo_status oo_upload_mlp(oo_ctx* c, const oo_mlp_desc* m, void*
     M.feat_dim = c->have_tree ? c->T.n_levels * c->T.F : 0;
     M.image_tc = (const uint16_t*)c->d_image_tc;
     M.image_tc_bytes = (uint32_t)(tc_halves * 2);
+    M.width = W;
     c->M = M;
     c->have_mlp = true;
     return OO_OK;
@@ -505,6 +527,7 @@ extern "C" OO_API oo_status oo_reserve(oo_ctx* c, uint64_t n) {
     OO_CUDA(c, cudaMalloc((void**)&c->d_qw, n * 12));
     OO_CUDA(c, cudaMalloc((void**)&c->d_qe, n * 4 * OO_MAX_EXTRA));
     OO_CUDA(c, cudaMalloc((void**)&c->d_rgb, n * 4 * 8));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_qd, n * 4));
     c->reserved = n;
     return OO_OK;
 }
@@ -546,6 +569,7 @@ extern "C" OO_API oo_status oo_encode(oo_ctx* c, const oo_queries* q, void* d_fe
                                void* cuda_stream) {
     if (!c) return OO_ERR_INVALID_ARG;
     if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "no tree uploaded");
+    if (c->T.vertex) return fail(c, OO_ERR_UNSUPPORTED, "oo_encode reads texel maps; use oo_encode_full for vertex maps");
     if (oo_status st = check_queries(c, q, false)) return st;
     if (oo_status st = check_async(c)) return st;
     if (q->n == 0) return OO_OK;
@@ -562,14 +586,57 @@ extern "C" OO_API oo_status oo_encode(oo_ctx* c, const oo_queries* q, void* d_fe
     return check_async(c);
 }
 
+// the full-query kernels are needed as soon as anything differs from the hot path
+static bool needs_full(const oo_ctx* c) {
+    return c->mode.tri8 || c->mode.lookup || c->mode.attrs_paper || c->T.vertex || (c->have_mlp && c->M.width != 64);
+}
+
+static oo_status check_full(oo_ctx* c, const oo_queries* q) {
+    if (!c->plan_ok) return fail(c, OO_ERR_UNSUPPORTED, "the full query needs the hop-table descent (used depths at most 3 apart below depth 4)");
+    if (c->mode.lookup != OO_LOOKUP_WO && q->n && !q->nrm) return fail(c, OO_ERR_INVALID_ARG, "queries.nrm is NULL (mirror direction)");
+    if (c->mode.lookup == OO_LOOKUP_SHIFTED && q->n && !q->disparity) return fail(c, OO_ERR_INVALID_ARG, "queries.disparity is NULL (OO_LOOKUP_SHIFTED)");
+    return OO_OK;
+}
+
+extern "C" OO_API oo_status oo_encode_full(oo_ctx* c, const oo_queries* q, float* d_features, int32_t* d_slot, int16_t* d_cell,
+                                    void* cuda_stream) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "no tree uploaded");
+    if (oo_status st = check_queries(c, q, false)) return st;
+    if (oo_status st = check_full(c, q)) return st;
+    if (oo_status st = check_async(c)) return st;
+    if (q->n == 0) return OO_OK;
+    DeviceGuard g(c->device);
+    const int n = launch_encode_full(c->T, make_qp(q), c->mode, d_features, d_slot, d_cell, c->n_sms, (cudaStream_t)cuda_stream);
+    if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "no full-query encode kernel for F=%u %s", c->T.F, c->T.f32 ? "fp32" : "fp16");
+    count(c, n);
+    c->info.path_last_encode = (uint32_t)OO_PATH_FULL;
+    return check_async(c);
+}
+
 static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cudaStream_t stream) {
     if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "no tree uploaded");
     if (!c->have_mlp) return fail(c, OO_ERR_NOT_READY, "no MLP uploaded");
     if (oo_status st = check_queries(c, q, true)) return st;
     if (q->n && !d_rgb) return fail(c, OO_ERR_INVALID_ARG, "rgb is NULL");
     const uint32_t feat = c->T.n_levels * c->T.F;
-    if (c->M.in_dim != feat + 6 + q->n_extra)
-        return fail(c, OO_ERR_NOT_READY, "MLP in_dim %u != L*F + 6 + n_extra = %u", c->M.in_dim, feat + 6 + q->n_extra);
+    const uint32_t n_attr = c->mode.attrs_paper ? 9u : 6u;
+    if (c->M.in_dim != feat + n_attr + q->n_extra)
+        return fail(c, OO_ERR_NOT_READY, "MLP in_dim %u != L*F + %u + n_extra = %u", c->M.in_dim, n_attr, feat + n_attr + q->n_extra);
+    if (needs_full(c)) {
+        if (oo_status st = check_full(c, q)) return st;
+        if (c->path != OO_PATH_AUTO) return fail(c, OO_ERR_UNSUPPORTED, "the full query has one kernel; oo_set_path(OO_PATH_AUTO)");
+        if (oo_status st = check_async(c)) return st;
+        if (q->n == 0) return OO_OK;
+        c->M.feat_dim = feat;
+        const QueryParams Q = make_qp(q);
+        const int n = c->M.width == 64 ? launch_fused_full_w64(c->T, c->M, Q, c->mode, d_rgb, c->n_sms, stream)
+                                       : launch_fused_full_w128(c->T, c->M, Q, c->mode, d_rgb, c->n_sms, stream);
+        if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "no full-query kernel for F=%u %s, in_dim %u, out_dim %u", c->T.F, c->T.f32 ? "fp32" : "fp16", c->M.in_dim, c->M.out_dim);
+        count(c, n);
+        c->info.path_last_query = (uint32_t)OO_PATH_FULL;
+        return check_async(c);
+    }
     if (oo_status st = check_async(c)) return st;
     if (q->n == 0) return OO_OK;
     c->M.feat_dim = feat;
@@ -634,8 +701,10 @@ extern "C" OO_API oo_status oo_query_host(oo_ctx* c, const oo_queries* q, float*
     OO_CUDA(c, cudaMemcpyAsync(c->d_qn, q->nrm, q->n * 12, cudaMemcpyHostToDevice, stream));
     OO_CUDA(c, cudaMemcpyAsync(c->d_qw, q->wo, q->n * 12, cudaMemcpyHostToDevice, stream));
     if (q->n_extra) OO_CUDA(c, cudaMemcpyAsync(c->d_qe, q->extra, q->n * 4 * q->n_extra, cudaMemcpyHostToDevice, stream));
+    if (q->disparity) OO_CUDA(c, cudaMemcpyAsync(c->d_qd, q->disparity, q->n * 4, cudaMemcpyHostToDevice, stream));
     oo_queries dq = *q;
     dq.x = c->d_qx; dq.nrm = c->d_qn; dq.wo = c->d_qw; dq.extra = q->n_extra ? c->d_qe : nullptr;
+    dq.disparity = q->disparity ? c->d_qd : nullptr;
     if (oo_status st = query_device(c, &dq, c->d_rgb, stream)) return st;
     OO_CUDA(c, cudaMemcpyAsync(h_rgb, c->d_rgb, q->n * 4 * c->M.out_dim, cudaMemcpyDeviceToHost, stream));
     OO_CUDA(c, cudaStreamSynchronize(stream));
@@ -646,6 +715,7 @@ extern "C" OO_API oo_status oo_read_padded_map(oo_ctx* c, uint32_t level, uint32
     if (!c) return OO_ERR_INVALID_ARG;
     if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "no tree uploaded");
     if (level >= c->T.n_levels || slot >= c->level_slots[level] || !h_out) return fail(c, OO_ERR_INVALID_ARG, "bad level/slot/pointer");
+    if (c->T.vertex) return fail(c, OO_ERR_UNSUPPORTED, "vertex maps are stored as given (no padded copy)");
     DeviceGuard g(c->device);
     const LevelParams& lv = c->T.lv[level];
     OO_CUDA(c, cudaMemcpy(h_out, (const uint8_t*)c->atlas_dev[level] + (uint64_t)slot * lv.map_bytes, lv.map_bytes, cudaMemcpyDeviceToHost));

@@ -38,6 +38,7 @@ struct TreeParams {
     uint32_t F;
     uint32_t f32;            // texel dtype is fp32
     uint32_t texel_bytes;
+    uint32_t vertex;         // OO_DIRMAP_VERTEX: maps are (R+1)^2 vertices, unpadded (Rp = R+1, atlas not pre-offset)
     uint32_t depth_eff;      // deepest used depth: positions are quantised to 2^depth_eff cells per axis
     float scale_eff;         // 2^depth_eff
     // top station: dense table at depth T = min(4, depth_eff) giving the local node index at that depth
@@ -57,6 +58,7 @@ struct QueryParams {
     const float* extra;
     uint32_t n_extra;
     const uint32_t* perm;
+    const float* disparity;  // [n] or nullptr (OO_LOOKUP_SHIFTED)
 };
 
 // Decoder image: the padded, shared-memory-ready copy of the weights (built by oo_upload_mlp).
@@ -70,8 +72,10 @@ struct MlpParams {
     uint32_t feat_dim;       // L*F
     // the same weights in the UMMA K-major canonical layout for the tcgen05 kernel: per layer [K/8][N][8] halves
     // (layer 0: K = k1, N = 64; hidden: K = N = 64; output: K = 64, N = 16 with rows >= out_dim zero)
+    // (width-W decoders: N = W for the hidden layers, K = W after the first)
     const uint16_t* image_tc;
     uint32_t image_tc_bytes;
+    uint32_t width;          // 64 or 128; `image` (the mma.sync copy) exists only for 64
 };
 
 struct EncodeOut {
@@ -98,6 +102,14 @@ bool tc_shape_supported(uint32_t L, uint32_t F, bool f32);
 int launch_fused_tm(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
                      cudaStream_t stream);
 bool tm_shape_supported(uint32_t L, uint32_t F, bool f32);
+// full query (oo_full_*.cu)
+struct FullModeH { uint32_t tri8, lookup, attrs_paper; };
+int launch_encode_full(const TreeParams& T, const QueryParams& Q, const FullModeH& mode, float* features, int32_t* slot,
+                       int16_t* cell, int n_sms, cudaStream_t stream);
+int launch_fused_full_w64(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const FullModeH& mode, float* rgb,
+                          int n_sms, cudaStream_t stream);
+int launch_fused_full_w128(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const FullModeH& mode, float* rgb,
+                           int n_sms, cudaStream_t stream);
 int launch_morton_sort(const float* x, uint64_t n, uint32_t* keys_a, uint32_t* keys_b, uint32_t* idx_a, uint32_t* perm_out,
                        uint32_t* hist, cudaStream_t stream);
 size_t morton_sort_hist_ints(uint64_t n);

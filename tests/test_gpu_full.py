@@ -1,0 +1,230 @@
+"""GPU parity of the paper's FULL query against oracle/oo_oracle_full.py, through the C ABI
+(oo_set_mode, oo_encode_full, oo_query): neighbour slots and directional index decisions bit-exact, features within
+1e-3, RGB within the north-star bounds (tests/parity.py).  Every piece is switched on alone and in combination, on
+fp32 / fp16 maps, texel / vertex maps, decoders of width 64 and 128."""
+import numpy as np
+import pytest
+
+import gen
+from oracle import oo_oracle as O
+from oracle import oo_oracle_full as FO
+from parity import check_features, check_rgb
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def P():
+    import paper_2606_08469_b200 as P
+    return P
+
+
+def _cu(a):
+    return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def _expected_cells(tree, q, mode, disparity):
+    """(ci, cj, upper) / (i0, j0, 0) per (query, level, neighbour) from the oracle's own index functions."""
+    N = q.n
+    J = 8 if mode.spatial == "trilinear8" else 1
+    out = np.zeros((N, len(tree.level_depth), J, 3), np.int64)
+    for l, (d, R) in enumerate(zip(tree.level_depth, tree.level_res)):
+        n_c = 1 << d
+        if J == 8:
+            k, _ = FO.neighbours(q.x, d)
+        else:
+            k = O.quantise(q.x, d)[:, None, :]
+        for j in range(J):
+            centre = ((k[:, j] + 0.5) / n_c).astype(np.float32)
+            w32 = FO.lookup_direction(mode, q.x, q.nrm, q.wo, centre, disparity)
+            if mode.dirmap == "vertex":
+                ci, cj, up = FO.vertex_cell_f32(w32, R)
+                out[:, l, j] = np.stack([ci, cj, up], -1)
+            else:
+                i0, j0 = O.texel_base_f32(w32, R)
+                out[:, l, j, 0], out[:, l, j, 1] = i0, j0
+    return out
+
+
+def _check(P, tree, atlas, dtype, mlp, q, mode, disparity=None, check_cells=True):
+    ref_f, ref_s = FO.encode_full(tree, atlas, q.x, q.nrm, q.wo, mode, disparity, return_debug=True)
+    ref_rgb = FO.query_full(tree, atlas, mlp.weights, q.x, q.nrm, q.wo, q.extra, mlp.out_act, mode, disparity)
+    ctx = P.OctaOctree(0)
+    ctx.oo_upload_tree(tree, atlas, dtype, dirmap=mode.dirmap)
+    ctx.oo_upload_mlp(mlp.weights, mlp.out_act)
+    ctx.oo_set_mode(mode.spatial, mode.lookup, mode.attrs)
+    x, n, wo, ex, dd = _cu(q.x), _cu(q.nrm), _cu(q.wo), _cu(q.extra), _cu(disparity)
+    f, s, c = ctx.oo_encode_full(x, n, wo, dd, want_debug=True)
+    rgb = ctx.oo_query(x, n, wo, ex, disparity=dd)
+    torch.cuda.synchronize()
+    assert np.array_equal(s.cpu().numpy().astype(np.int64), ref_s), "neighbour slots differ"
+    if check_cells:
+        want = _expected_cells(tree, q, mode, disparity)
+        got = c.cpu().numpy().astype(np.int64)
+        live = (ref_s >= 0)[..., None] | (mode.lookup != "shifted")          # a shifted direction is only formed for real cells
+        assert np.array_equal(np.where(live, got, 0), np.where(live, want, 0)), "directional index decisions differ"
+    check_features(f.cpu().numpy(), ref_f)
+    err = check_rgb(rgb.cpu().numpy(), ref_rgb)
+    info = ctx.oo_get_info()
+    full = mode != FO.Mode() or mlp.width != 64
+    assert info["path_last_query"] == (P.PATH_FULL if full else P.PATH_FUSED_TC_TMEM)
+    assert info["path_last_encode"] == P.PATH_FULL
+    ctx.close()
+    return err
+
+
+MODES = [
+    FO.Mode(),
+    FO.Mode(spatial="trilinear8"),
+    FO.Mode(lookup="mirror"),
+    FO.Mode(lookup="shifted"),
+    FO.Mode(attrs="paper"),
+    FO.Mode(dirmap="vertex"),
+    FO.Mode(spatial="trilinear8", dirmap="vertex"),
+    FO.Mode(spatial="trilinear8", lookup="shifted"),
+    FO.Mode(dirmap="vertex", lookup="shifted", attrs="paper"),
+    FO.Mode(spatial="trilinear8", dirmap="vertex", lookup="shifted", attrs="paper"),
+]
+_ids = lambda m: "%s-%s-%s-%s" % (m.spatial, m.dirmap, m.lookup, m.attrs)
+
+
+def _edge_queries(q):
+    """Overwrite the first queries with the degenerate positions: cube corners and faces, outside the cube (A16),
+    cell centres and cell boundaries."""
+    x = q.x.copy()
+    special = np.array([[0, 0, 0], [1, 1, 1], [0, 1, 0.5], [-0.25, 0.5, 1.5], [0.125, 0.375, 0.625], [0.25, 0.5, 0.75],
+                        [1.0 - 2.0 ** -24, 0.5, 0.5], [0.5, 0.5, 0.5], [2.0 ** -30, 0.3, 0.9]], np.float32)
+    x[: len(special)] = special
+    return gen.Queries(x, q.nrm, q.wo, q.extra)
+
+
+@pytest.mark.parametrize("mode", MODES, ids=_ids)
+def test_uniform_tree_fp32(P, mode):
+    """config-0 shapes (uniform 73-node tree, F = 4 fp32, decoder 2 x 64), N = 4096 + degenerate positions."""
+    w = gen.config0()
+    q = _edge_queries(w.queries)
+    n_extra = 4 if mode.attrs == "paper" else 0
+    q.extra = gen.albedo_roughness(q.n, 0) if n_extra else None
+    atlas = (gen.make_vertex_atlas(w.tree, 4, "f32", 0) if mode.dirmap == "vertex" else w.atlas).levels
+    mlp = gen.make_mlp(8 + (9 if mode.attrs == "paper" else 6) + n_extra, 2, 0)
+    _check(P, w.tree, atlas, "f32", mlp, q, mode, gen.disparity(q.n, 0))
+
+
+@pytest.mark.parametrize("mode", MODES, ids=_ids)
+def test_sparse_tree_fp16(P, mode):
+    """config-1 recipe at depth 6 (adaptive tree around the three-sphere scene, used depths {2,4,6}: dense tables AND
+    hop tables with a gap of 2, empty neighbours), F = 8 fp16, decoder 3 x 64, a 160x120 frame (ragged last tile)."""
+    w = gen.scene_workload(1, width=160, height=119, max_depth=6)
+    q = _edge_queries(w.queries)
+    n_extra = 4 if mode.attrs == "paper" else 0
+    q.extra = gen.albedo_roughness(q.n, 0) if n_extra else None
+    atlas = (gen.make_vertex_atlas(w.tree, 8, "f16", 0) if mode.dirmap == "vertex" else w.atlas).levels
+    mlp = gen.make_mlp(24 + (9 if mode.attrs == "paper" else 6) + n_extra, 3, 0)
+    _check(P, w.tree, atlas, "f16", mlp, q, mode, gen.disparity(q.n, 0))
+
+
+@pytest.mark.parametrize("mode", [MODES[1], MODES[6], MODES[9]], ids=_ids)
+def test_f16_wide_texels(P, mode):
+    """F = 16 fp16 (32-byte texels, config-3 shape) on the depth-6 tree."""
+    w = gen.scene_workload(3, width=96, height=64, max_depth=6)
+    q = w.queries
+    n_extra = 4 if mode.attrs == "paper" else 0
+    q.extra = gen.albedo_roughness(q.n, 0) if n_extra else None
+    atlas = (gen.make_vertex_atlas(w.tree, 16, "f16", 0) if mode.dirmap == "vertex" else w.atlas).levels
+    mlp = gen.make_mlp(48 + (9 if mode.attrs == "paper" else 6) + n_extra, 4, 0)
+    _check(P, w.tree, atlas, "f16", mlp, q, mode, gen.disparity(q.n, 0))
+
+
+@pytest.mark.parametrize("mode", [FO.Mode(), MODES[1], MODES[9]], ids=_ids)
+def test_width_128_decoder(P, mode):
+    """Decoder 4 x 128 on the tcgen05 path with N = 128 tiles and the two-part teams."""
+    w = gen.scene_workload(1, width=160, height=119, max_depth=6)
+    q = w.queries
+    n_extra = 4 if mode.attrs == "paper" else 0
+    q.extra = gen.albedo_roughness(q.n, 0) if n_extra else None
+    atlas = (gen.make_vertex_atlas(w.tree, 8, "f16", 0) if mode.dirmap == "vertex" else w.atlas).levels
+    mlp = gen.make_mlp(24 + (9 if mode.attrs == "paper" else 6) + n_extra, 4, 0, width=128)
+    _check(P, w.tree, atlas, "f16", mlp, q, mode, gen.disparity(q.n, 0))
+
+
+def test_paper_shapes_reduced(P):
+    """The paper's own configuration (K consecutive levels from depth 2, C = 4 fp32 vertex maps whose resolution halves per
+    level, Eq. 12 attributes, decoder 4 x 128, all of f1-f4 on) with 6 levels (depths 2..7): consecutive depths give
+    dense tables for 2..4 and gap-1 hop tables below."""
+    w = gen.paper_workload(width=128, height=96, depths=[2, 3, 4, 5, 6, 7], res=[64, 32, 16, 8, 4, 2])
+    mode = FO.Mode(spatial="trilinear8", dirmap="vertex", lookup="shifted", attrs="paper")
+    _check(P, w.tree, w.atlas.levels, "f32", w.mlp, w.queries, mode, w.meta["disparity"])
+
+
+def test_incoherent_queries_and_perm(P):
+    """Random-order surface samples (config-4 'incoherent') through the full query; a permutation changes the processing
+    order only."""
+    w = gen.paper_workload(depths=[2, 3, 4, 5, 6], res=[32, 16, 8, 4, 2], incoherent_n=5000)
+    mode = FO.Mode(spatial="trilinear8", dirmap="vertex", lookup="shifted", attrs="paper")
+    q, d = w.queries, w.meta["disparity"]
+    _check(P, w.tree, w.atlas.levels, "f32", w.mlp, q, mode, d)
+    ctx = P.OctaOctree(0)
+    ctx.oo_upload_tree(w.tree, w.atlas.levels, "f32", dirmap="vertex")
+    ctx.oo_upload_mlp(w.mlp.weights, w.mlp.out_act)
+    ctx.oo_set_mode(mode.spatial, mode.lookup, mode.attrs)
+    x, n, wo, ex, dd = _cu(q.x), _cu(q.nrm), _cu(q.wo), _cu(q.extra), _cu(d)
+    a = ctx.oo_query(x, n, wo, ex, disparity=dd)
+    perm = _cu(gen.shuffle_perm(q.n, 3).astype(np.int32))
+    b = ctx.oo_query(x, n, wo, ex, perm=perm, disparity=dd)
+    torch.cuda.synchronize()
+    assert torch.equal(a, b)
+    ctx.close()
+
+
+def test_all_neighbours_empty_gives_the_attribute_only_answer(P):
+    """A tree whose used level has cells only in one corner: queries far away blend no cell at all (Eq. 10 with an empty
+    sum => zero features), so rgb = MLP([0 | attributes])."""
+    tree = gen.build_tree(None, 3, uniform=True)
+    # keep only the octant-0 subtree below the root
+    keep = np.zeros(tree.n_nodes, bool)
+    keep[0] = True
+    for i in range(tree.n_nodes):
+        if keep[i]:
+            for o in range(8):
+                c = tree.child[i, o]
+                if c >= 0 and (i != 0 or o == 0):
+                    keep[c] = True
+    new_id = np.cumsum(keep) - 1
+    child = np.where(tree.child >= 0, np.where(keep[np.maximum(tree.child, 0)], new_id[np.maximum(tree.child, 0)], -1), -1)[keep]
+    depth = tree.depth[keep]
+    coords = tree.coords[keep]
+    depth_first = np.array([np.searchsorted(depth, d) for d in range(5)], np.int64)
+    t2 = gen.Tree(3, child.astype(np.int32), depth, coords, depth_first).set_levels([2, 3], [4, 4])
+    atlas = gen.make_vertex_atlas(t2, 4, "f32", 0).levels
+    q = gen.random_queries(2000, 0)
+    q.extra = gen.albedo_roughness(q.n, 0)
+    mode = FO.Mode(spatial="trilinear8", dirmap="vertex", lookup="shifted", attrs="paper")
+    mlp = gen.make_mlp(8 + 13, 2, 0)
+    d = gen.disparity(q.n, 0)
+    ref_f = FO.encode_full(t2, atlas, q.x, q.nrm, q.wo, mode, d)
+    far = (q.x > 0.7).all(1)
+    assert far.any() and np.all(ref_f[far] == 0.0)
+    _check(P, t2, atlas, "f32", mlp, q, mode, d)
+
+
+def test_full_query_argument_errors(P):
+    w = gen.config0(n=64)
+    ctx = P.OctaOctree(0).upload_workload(w)
+    q = w.queries
+    x, n, wo = _cu(q.x), _cu(q.nrm), _cu(q.wo)
+    ctx.oo_set_mode("trilinear8", "shifted", "n_wo")
+    with pytest.raises(P.OOError) as e:
+        ctx.oo_query(x, n, wo)                      # no disparity
+    assert e.value.status == 1
+    ctx.oo_set_mode("nearest", "wo", "paper")
+    with pytest.raises(P.OOError) as e:
+        ctx.oo_query(x, n, wo)                      # in_dim 14 != 8 + 9
+    assert e.value.status == 2
+    ctx.oo_set_mode()
+    assert ctx.oo_query(x, n, wo).shape == (64, 3)
+    empty = torch.empty((0, 3), device="cuda")
+    ctx.oo_set_mode("trilinear8")
+    assert ctx.oo_query(empty, empty, empty).shape == (0, 3)
+    ctx.close()
