@@ -343,6 +343,97 @@ def run_sweep(args):
     return 0
 
 
+def run_full(args):
+    """--sweep 8: the paper's FULL query at the paper's own shapes: 8 consecutive levels
+    (depths 2..9), C = 4 fp32 vertex maps of resolution 2^8+1 .. 2^1+1, 8-neighbour trilinear blend, disparity-shifted
+    mirror direction, Eq. 12 attributes, decoder 4 x 128, one 1024x1024 frame of primary hits; then each piece switched
+    off in turn.  One JSON line with a table (not the headline line)."""
+    import numpy as np
+    import torch
+    import gen
+    import paper_2606_08469_b200 as P
+    from oracle import oo_oracle_full as FO
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    hbm, tf, which = peaks()
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+    cu = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    w = gen.paper_workload(seed=0)
+    q, disp = w.queries, w.meta["disparity"]
+    L, F = len(w.tree.level_depth), w.atlas.F
+    ctx = P.OctaOctree(0)
+    ctx.oo_upload_tree(w.tree, w.atlas.levels, w.atlas.dtype, dirmap="vertex")
+    x, nrm, wo, ex, dd = cu(q.x), cu(q.nrm), cu(q.wo), cu(q.extra), cu(disp)
+    rgb = torch.empty((q.n, 3), dtype=torch.float32, device=dev)
+    feat_rows = []
+
+    def timed(fn, reps, do_flush=True):
+        for _ in range(3):
+            flush.zero_()
+            fn()
+        evs = []
+        for _ in range(reps):
+            if do_flush:
+                flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+            evs.append((e0, e1))
+        torch.cuda.synchronize(dev)
+        t = sorted(a.elapsed_time(b) for a, b in evs)
+        return t[len(t) // 2]
+
+    variants = [("full: trilinear8 + vertex + shifted + Eq.12 attrs, 4x128", "trilinear8", "shifted", "paper", 128),
+                ("no shift (mirror direction for every cell)", "trilinear8", "mirror", "paper", 128),
+                ("nearest cell (P:266 ablation)", "nearest", "shifted", "paper", 128),
+                ("nearest cell, mirror direction", "nearest", "mirror", "paper", 128),
+                ("full gather, decoder 4x64", "trilinear8", "shifted", "paper", 64)]
+    rows = []
+    for name, spatial, lookup, attrs, width in variants:
+        mlp = gen.make_mlp(L * F + 13, 4, 0, width=width)
+        ctx.oo_upload_mlp(mlp.weights, mlp.out_act)
+        ctx.oo_set_mode(spatial, lookup, attrs)
+        # live neighbours (non-empty cells inside the grid) decide the bytes the method must read
+        sub = slice(0, q.n, 16)
+        _, s, _ = ctx.oo_encode_full(x[sub].contiguous(), nrm[sub].contiguous(), wo[sub].contiguous(), dd[sub].contiguous(), want_debug=True)
+        live = float((s >= 0).float().sum(dim=(1, 2)).mean())
+        J = 8 if spatial == "trilinear8" else 1
+        bq = live * 3 * F * 4 + 36 + 4 + 16 + 12
+        dims = [L * F + 13] + [width] * 4 + [3]
+        flops = 2 * sum(a * b for a, b in zip(dims[:-1], dims[1:]))
+        t = timed(lambda: ctx.oo_query(x, nrm, wo, ex, rgb=rgb, disparity=dd), args.steps)
+        tw = timed(lambda: ctx.oo_query(x, nrm, wo, ex, rgb=rgb, disparity=dd), min(args.steps, 20), do_flush=False)
+        te = timed(lambda: ctx.oo_encode_full(x, nrm, wo, dd), min(args.steps, 20))
+        rows.append({"variant": name, "ms": t, "ms_warm_l2": tw, "Mqueries_per_s": q.n / t / 1e3, "encode_only_ms": te,
+                     "live_neighbour_lookups_per_query": live, "of": L * J, "algorithmic_bytes_per_query": bq,
+                     "flop_per_query": flops, "byte_time_ms": bq * q.n / (hbm * 1e9) * 1e3, "flop_time_ms": flops * q.n / (tf * 1e12) * 1e3,
+                     "roofline_frac": max(bq * q.n / (hbm * 1e9), flops * q.n / (tf * 1e12)) / (t * 1e-3)})
+    out = {"sweep": "full query at the paper's shapes (PAPER.md implementation details; SURVEY.md 8(f) f1-f4)",
+           "workload": "1024x1024 primary hits of the three-sphere scene; octree depth 9 (%d nodes), used depths %s, vertex maps R_l+1 = %s, C=%d fp32 (%.0f MB), "
+                       "Eq. 12 attributes (13 scalars), synthetic disparity U(0.25,4)" %
+                       (w.tree.n_nodes, w.tree.level_depth, [r + 1 for r in w.tree.level_res], F, w.atlas.nbytes / 1e6),
+           "rows": rows, "unit": UNIT, "l2": "flushed between launches (256 MB memset)", "timing": "median of CUDA-event times",
+           "peak_gbs": hbm, "peak_tflops": tf, "peak_source": which, "data": "synthetic",
+           "paper_context": "Table 1: 10-20 ms per frame on an RTX 3090 including Mitsuba G-buffer extraction and the disparity network (not comparable)"}
+    if not args.no_cpu_baseline:
+        n_s = 16384
+        idx = np.arange(0, q.n, q.n // n_s)[:n_s]
+        qs = q.take(idx)
+        mode = FO.Mode("trilinear8", "vertex", "shifted", "paper")
+        mlp = gen.make_mlp(L * F + 13, 4, 0, width=128)
+        t0 = time.perf_counter()
+        FO.query_full(w.tree, w.atlas.levels, mlp.weights, qs.x, qs.nrm, qs.wo, qs.extra, "exp", mode, disp[idx])
+        dt = time.perf_counter() - t0
+        out["cpu_baseline"] = {"value": n_s / dt / 1e6, "unit": UNIT, "cores": 1, "kind": "oracle (numpy float64, oo_oracle_full.py)",
+                               "sample": "%d queries (every %dth pixel)" % (n_s, q.n // n_s)}
+    print(json.dumps(out))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -353,13 +444,15 @@ def main():
     ap.add_argument("--path", default="auto", choices=["auto", "mma", "tc", "tm", "unfused", "generic"])
     ap.add_argument("--ref-sample", type=int, default=131072, help="queries in the CPU-oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--sweep", type=int, default=0, choices=[0, 2, 4], help="side measurements of configs[2] / configs[4] (a table, not the headline line)")
+    ap.add_argument("--sweep", type=int, default=0, choices=[0, 2, 4, 8], help="side measurements of configs[2] / configs[4] / (8) the paper's full query at its own shapes (a table, not the headline line)")
     ap.add_argument("--sweep-max-log2", type=int, default=24)
     ap.add_argument("--quick", action="store_true", help="timed region only (no warm-L2 / e2e / CPU legs): the command ncu wraps")
     args = ap.parse_args()
     # the reference arm is a CPU program: keep each step bounded whatever K the driver passes
     args.steps_ref = max(1, min(args.steps, 5))
     args.warmup_ref = max(0, min(args.warmup, 1))
+    if args.sweep == 8:
+        return run_full(args)
     if args.sweep:
         return run_sweep(args)
     return run_reference(args) if args.impl == "reference" else run_ours(args)

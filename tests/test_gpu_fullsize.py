@@ -59,3 +59,32 @@ def test_config3_full_tree_sampled_queries():
     qi = gen.incoherent_queries(w.scene, 1 << 16, 0)
     ref = co.query(qi.x, qi.nrm, qi.wo)
     check_rgb(ctx.oo_query(_dev(qi.x), _dev(qi.nrm), _dev(qi.wo)).cpu().numpy(), ref)
+
+
+def test_paper_shapes_full_frame_sampled_queries():
+    """The paper's own configuration at full size (bench.py --sweep 8: depths 2..9, ~2 M nodes, ~1 GB of fp32 vertex maps,
+    all of f1-f4 on, decoder 4 x 128, 1024x1024 frame): the whole frame on the GPU, the numpy oracle on a sample of
+    queries spread over the frame."""
+    import paper_2606_08469_b200 as P
+    from oracle import oo_oracle_full as FO
+    w = gen.paper_workload()
+    q, d = w.queries, w.meta["disparity"]
+    assert q.n == 1024 * 1024 and w.tree.level_depth == list(range(2, 10)) and w.atlas.nbytes > 9e8
+    ctx = P.OctaOctree(0)
+    ctx.oo_upload_tree(w.tree, w.atlas.levels, "f32", dirmap="vertex")
+    ctx.oo_upload_mlp(w.mlp.weights, w.mlp.out_act)
+    ctx.oo_set_mode("trilinear8", "shifted", "paper")
+    x, n, wo, ex, dd = _dev(q.x), _dev(q.nrm), _dev(q.wo), _dev(q.extra), _dev(d)
+    got = ctx.oo_query(x, n, wo, ex, disparity=dd)
+    feat, slots, _ = ctx.oo_encode_full(x, n, wo, dd, want_debug=True)
+    torch.cuda.synchronize()
+    assert ctx.oo_get_info()["path_last_query"] == P.PATH_FULL
+    idx = np.arange(0, q.n, 127)                                   # ~8 k queries across the whole frame
+    qs = q.take(idx)
+    mode = FO.Mode("trilinear8", "vertex", "shifted", "paper")
+    ref_f, ref_s = FO.encode_full(w.tree, w.atlas.levels, qs.x, qs.nrm, qs.wo, mode, d[idx], return_debug=True)
+    ref = FO.query_full(w.tree, w.atlas.levels, w.mlp.weights, qs.x, qs.nrm, qs.wo, qs.extra, "exp", mode, d[idx])
+    assert np.array_equal(slots.cpu().numpy()[idx].astype(np.int64), ref_s)
+    check_features(feat.cpu().numpy()[idx], ref_f)
+    mx, mean = check_rgb(got.cpu().numpy()[idx], ref)
+    print("paper shapes full frame: rgb max-abs %.3g mean-abs %.3g on %d sampled queries" % (mx, mean, len(idx)))
