@@ -318,13 +318,17 @@ def run_sweep(args):
         n_max = 1 << args.sweep_max_log2
         side = 1 << ((args.sweep_max_log2 + 1) // 2)
         cam = gen.make_camera(side, n_max // side, 0)
-        dists = {"coherent": gen.raycast(w.scene, cam), "incoherent": gen.incoherent_queries(w.scene, n_max, 0)}
+        dists = {}
+        if args.sweep_dist in ("both", "coherent"):
+            dists["coherent"] = gen.raycast(w.scene, cam)
+        if args.sweep_dist in ("both", "incoherent"):
+            dists["incoherent"] = gen.incoherent_queries(w.scene, n_max, 0)
         ctx.oo_reserve(n_max)
         feat = torch.empty((n_max, L * F), dtype=torch.float16, device=dev)
         rgb = torch.empty((n_max, 3), dtype=torch.float32, device=dev)
         for dname, q in dists.items():
             X, Nn, W = cu(q.x), cu(q.nrm), cu(q.wo)
-            for lg in range(16, args.sweep_max_log2 + 1):
+            for lg in range(args.sweep_min_log2, args.sweep_max_log2 + 1):
                 n = 1 << lg
                 x, nrm, wo = X[:n], Nn[:n], W[:n]
                 reps = max(5, min(args.steps, (1 << 26) // n))
@@ -393,6 +397,8 @@ def run_full(args):
                 ("nearest cell, mirror direction", "nearest", "mirror", "paper", 128),
                 ("full gather, decoder 4x64", "trilinear8", "shifted", "paper", 64)]
     rows = []
+    if args.quick:
+        variants = variants[:1]
     for name, spatial, lookup, attrs, width in variants:
         mlp = gen.make_mlp(L * F + 13, 4, 0, width=width)
         ctx.oo_upload_mlp(mlp.weights, mlp.out_act)
@@ -406,8 +412,8 @@ def run_full(args):
         dims = [L * F + 13] + [width] * 4 + [3]
         flops = 2 * sum(a * b for a, b in zip(dims[:-1], dims[1:]))
         t = timed(lambda: ctx.oo_query(x, nrm, wo, ex, rgb=rgb, disparity=dd), args.steps)
-        tw = timed(lambda: ctx.oo_query(x, nrm, wo, ex, rgb=rgb, disparity=dd), min(args.steps, 20), do_flush=False)
-        te = timed(lambda: ctx.oo_encode_full(x, nrm, wo, dd), min(args.steps, 20))
+        tw = t if args.quick else timed(lambda: ctx.oo_query(x, nrm, wo, ex, rgb=rgb, disparity=dd), min(args.steps, 20), do_flush=False)
+        te = None if args.quick else timed(lambda: ctx.oo_encode_full(x, nrm, wo, dd), min(args.steps, 20))
         rows.append({"variant": name, "ms": t, "ms_warm_l2": tw, "Mqueries_per_s": q.n / t / 1e3, "encode_only_ms": te,
                      "live_neighbour_lookups_per_query": live, "of": L * J, "algorithmic_bytes_per_query": bq,
                      "flop_per_query": flops, "byte_time_ms": bq * q.n / (hbm * 1e9) * 1e3, "flop_time_ms": flops * q.n / (tf * 1e12) * 1e3,
@@ -419,7 +425,7 @@ def run_full(args):
            "rows": rows, "unit": UNIT, "l2": "flushed between launches (256 MB memset)", "timing": "median of CUDA-event times",
            "peak_gbs": hbm, "peak_tflops": tf, "peak_source": which, "data": "synthetic",
            "paper_context": "Table 1: 10-20 ms per frame on an RTX 3090 including Mitsuba G-buffer extraction and the disparity network (not comparable)"}
-    if not args.no_cpu_baseline:
+    if not args.no_cpu_baseline and not args.quick:
         n_s = 16384
         idx = np.arange(0, q.n, q.n // n_s)[:n_s]
         qs = q.take(idx)
@@ -446,6 +452,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--sweep", type=int, default=0, choices=[0, 2, 4, 8], help="side measurements of configs[2] / configs[4] / (8) the paper's full query at its own shapes (a table, not the headline line)")
     ap.add_argument("--sweep-max-log2", type=int, default=24)
+    ap.add_argument("--sweep-min-log2", type=int, default=16)
+    ap.add_argument("--sweep-dist", default="both", choices=["both", "coherent", "incoherent"])
     ap.add_argument("--quick", action="store_true", help="timed region only (no warm-L2 / e2e / CPU legs): the command ncu wraps")
     args = ap.parse_args()
     # the reference arm is a CPU program: keep each step bounded whatever K the driver passes

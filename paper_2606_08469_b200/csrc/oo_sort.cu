@@ -1,16 +1,23 @@
 // oo_sort.cu — row a1: Morton pre-sort of the queries (BASELINE.json north_star; not in the paper).
 //
 // key = 30-bit Morton code of clamp(floor(x*1024), 0, 1023): bit b of q_x -> key bit 3b, q_y -> 3b+1, q_z -> 3b+2 (the
-// octant convention of the tree, so sorted order walks the octree depth-first).  Stable LSD radix sort, 4 passes of 8
-// bits, hand written: per pass a histogram kernel, a single-block exclusive scan, and a stable scatter in which every
-// warp owns a contiguous chunk and ranks its items 32 at a time with __match_any_sync against running per-warp digit
-// counters in shared memory.  Ties keep the original order, so the permutation is unique.
+// octant convention of the tree, so sorted order walks the octree depth-first).  Stable LSD radix sort, 3 passes of 10
+// bits, hand written: per pass a per-tile histogram kernel (4096 keys per block; the first one also makes the keys), an
+// exclusive scan with one block per digit (digit totals come from the histogram kernel's atomics), and a stable scatter in which every warp keeps 512 consecutive keys in registers and ranks
+// them 32 at a time with __match_any_sync against warp-private digit counters in shared memory.  Ties keep the original
+// order, so the permutation is unique.  9 launches.
 #include "oo_device.cuh"
 
 namespace oo {
 
 constexpr int kSortThreads = 256;                 // 8 warps per block
-constexpr int kChunk = 2048;                      // items per warp
+constexpr int kItems = 16;                        // keys per thread
+constexpr int kWarpChunk = 32 * kItems;           // 512 consecutive keys per warp
+constexpr int kTile = kSortThreads * kItems;      // 4096 keys per block
+constexpr int kBits = 10;                         // digit width: 30-bit keys = 3 passes
+constexpr int kDigits = 1 << kBits;
+constexpr int kPasses = 3;
+constexpr int kDPT = kDigits / kSortThreads;      // digits per thread in the per-digit loops
 
 __device__ __forceinline__ uint32_t spread3(uint32_t v) {   // 10 bits -> every third bit
     v = (v | (v << 16)) & 0x030000FFu;
@@ -20,118 +27,174 @@ __device__ __forceinline__ uint32_t spread3(uint32_t v) {   // 10 bits -> every 
     return v;
 }
 
-__global__ void morton_key_kernel(const float* __restrict__ x, uint64_t n, uint32_t* __restrict__ keys) {
-    const uint64_t t = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x;
-    if (t >= n) return;
-    const int qx = quantise(__ldg(x + 3 * t), 1024.0f, 1023), qy = quantise(__ldg(x + 3 * t + 1), 1024.0f, 1023),
-              qz = quantise(__ldg(x + 3 * t + 2), 1024.0f, 1023);
-    keys[t] = spread3((uint32_t)qx) | (spread3((uint32_t)qy) << 1) | (spread3((uint32_t)qz) << 2);
+__device__ __forceinline__ uint32_t morton_of(const float* __restrict__ x, uint64_t i) {
+    const int qx = quantise(__ldg(x + 3 * i), 1024.0f, 1023), qy = quantise(__ldg(x + 3 * i + 1), 1024.0f, 1023),
+              qz = quantise(__ldg(x + 3 * i + 2), 1024.0f, 1023);
+    return spread3((uint32_t)qx) | (spread3((uint32_t)qy) << 1) | (spread3((uint32_t)qz) << 2);
 }
 
-// hist[digit * n_chunks + chunk] = number of keys of that digit in the chunk
-__global__ void __launch_bounds__(kSortThreads) radix_hist_kernel(const uint32_t* __restrict__ keys, uint64_t n,
-                                                                  uint32_t shift, uint32_t n_chunks, uint32_t* __restrict__ hist) {
-    __shared__ uint32_t cnt[kSortThreads / 32][256];
-    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t chunk = blockIdx.x * (kSortThreads / 32) + warp;
-    for (int d = lane; d < 256; d += 32) cnt[warp][d] = 0;
-    __syncwarp();
-    if (chunk < n_chunks) {
-        const uint64_t base = (uint64_t)chunk * kChunk;
-        for (int it = 0; it < kChunk / 32; ++it) {
-            const uint64_t i = base + it * 32 + lane;
-            if (i < n) atomicAdd(&cnt[warp][(keys[i] >> shift) & 255u], 1u);
+// hist[digit * n_tiles + tile] = number of keys of that digit in the tile; tot[digit] += the same (digit totals of
+// the pass).  FIRST: the keys are made here (from x) and written out, so there is no separate key kernel.
+template <bool FIRST>
+__global__ void __launch_bounds__(kSortThreads) radix_hist_kernel(const float* __restrict__ x, uint32_t* __restrict__ keys,
+                                                                  uint64_t n, uint32_t shift, uint32_t n_tiles,
+                                                                  uint32_t* __restrict__ hist, uint32_t* __restrict__ tot) {
+    __shared__ uint32_t cnt[kDigits];
+#pragma unroll
+    for (int k = 0; k < kDPT; ++k) cnt[threadIdx.x + k * kSortThreads] = 0;
+    __syncthreads();
+    const uint64_t base = (uint64_t)blockIdx.x * kTile;
+#pragma unroll 4
+    for (int it = 0; it < kItems; ++it) {
+        const uint64_t i = base + (uint64_t)it * kSortThreads + threadIdx.x;
+        if (i < n) {
+            uint32_t key;
+            if constexpr (FIRST) {
+                key = morton_of(x, i);
+                keys[i] = key;
+            } else {
+                key = keys[i];
+            }
+            atomicAdd(&cnt[(key >> shift) & (kDigits - 1)], 1u);
         }
-        __syncwarp();
-        for (int d = lane; d < 256; d += 32) hist[(size_t)d * n_chunks + chunk] = cnt[warp][d];
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kDPT; ++k) {
+        const uint32_t d = threadIdx.x + k * kSortThreads, c = cnt[d];
+        hist[(size_t)d * n_tiles + blockIdx.x] = c;
+        if (c) atomicAdd(&tot[d], c);
     }
 }
 
-// in-place exclusive scan of `len` counters by one block
-__global__ void __launch_bounds__(1024) scan_kernel(uint32_t* __restrict__ data, uint32_t len) {
-    __shared__ uint32_t part[1024];
-    const uint32_t per = (len + 1023) / 1024;
-    const uint32_t lo = min(threadIdx.x * per, len), hi = min(lo + per, len);
+// Exclusive scan of hist in (digit, tile) order, in place: block d scans row d and adds the total of all smaller digits.
+__global__ void __launch_bounds__(kSortThreads) scan_kernel(uint32_t* __restrict__ hist, const uint32_t* __restrict__ tot,
+                                                            uint32_t n_tiles) {
+    __shared__ uint32_t red[kSortThreads / 32];
+    __shared__ uint32_t part[kSortThreads];
+    const uint32_t d = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     uint32_t s = 0;
-    for (uint32_t i = lo; i < hi; ++i) s += data[i];
-    part[threadIdx.x] = s;
+    for (uint32_t k = threadIdx.x; k < d; k += kSortThreads) s += tot[k];
+#pragma unroll
+    for (int o = 16; o; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if (lane == 0) red[warp] = s;
+    uint32_t* row = hist + (size_t)d * n_tiles;
+    const uint32_t per = (n_tiles + kSortThreads - 1) / kSortThreads;
+    const uint32_t lo = min(threadIdx.x * per, n_tiles), hi = min(lo + per, n_tiles);
+    uint32_t mine = 0;
+    for (uint32_t i = lo; i < hi; ++i) mine += row[i];
+    part[threadIdx.x] = mine;
     __syncthreads();
-    for (uint32_t off = 1; off < 1024; off <<= 1) {
-        uint32_t v = threadIdx.x >= off ? part[threadIdx.x - off] : 0;
+    uint32_t base = 0;
+#pragma unroll
+    for (int w = 0; w < kSortThreads / 32; ++w) base += red[w];
+    for (uint32_t off = 1; off < kSortThreads; off <<= 1) {
+        const uint32_t v = threadIdx.x >= off ? part[threadIdx.x - off] : 0;
         __syncthreads();
         part[threadIdx.x] += v;
         __syncthreads();
     }
-    uint32_t run = part[threadIdx.x] - s;
+    uint32_t run = base + part[threadIdx.x] - mine;
     for (uint32_t i = lo; i < hi; ++i) {
-        const uint32_t v = data[i];
-        data[i] = run;
+        const uint32_t v = row[i];
+        row[i] = run;
         run += v;
     }
 }
 
-// stable scatter: offsets[digit * n_chunks + chunk] = first output position of that (digit, chunk)
+// Stable scatter of one tile: offsets[digit * n_tiles + tile] = first output position of that (digit, tile).  Warp w owns
+// the 512 consecutive keys [tile*4096 + 512 w, +512) and keeps them in registers: it ranks them 32 at a time with
+// __match_any_sync against its private digit counters (rank among equal digits in index order), the block then turns the
+// counters into per-warp start positions, and every key goes to start + rank.
 __global__ void __launch_bounds__(kSortThreads) radix_scatter_kernel(const uint32_t* __restrict__ keys_in,
                                                                      const uint32_t* __restrict__ idx_in, uint64_t n,
-                                                                     uint32_t shift, uint32_t n_chunks,
+                                                                     uint32_t shift, uint32_t n_tiles,
                                                                      const uint32_t* __restrict__ offsets,
                                                                      uint32_t* __restrict__ keys_out, uint32_t* __restrict__ idx_out) {
-    __shared__ uint32_t pos[kSortThreads / 32][256];
+    __shared__ uint32_t pos[kSortThreads / 32][kDigits];
     const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const uint32_t chunk = blockIdx.x * (kSortThreads / 32) + warp;
-    if (chunk >= n_chunks) return;
-    for (int d = lane; d < 256; d += 32) pos[warp][d] = offsets[(size_t)d * n_chunks + chunk];
-    __syncwarp();
-    const uint64_t base = (uint64_t)chunk * kChunk;
+    for (int w = 0; w < kSortThreads / 32; ++w)
+#pragma unroll
+        for (int k = 0; k < kDPT; ++k) pos[w][threadIdx.x + k * kSortThreads] = 0;
+    __syncthreads();
+    const uint64_t base = (uint64_t)blockIdx.x * kTile + (uint64_t)warp * kWarpChunk;
     const uint32_t lt = (1u << lane) - 1u;
-    for (int it = 0; it < kChunk / 32; ++it) {
+    uint32_t key[kItems], rank[kItems];
+#pragma unroll
+    for (int it = 0; it < kItems; ++it) {
+        const uint64_t i = base + it * 32 + lane;
+        key[it] = i < n ? keys_in[i] : 0xFFFFFFFFu;
+    }
+#pragma unroll
+    for (int it = 0; it < kItems; ++it) {
         const uint64_t i = base + it * 32 + lane;
         const bool live = i < n;
         const uint32_t active = __ballot_sync(0xffffffffu, live);
         if (live) {
-            const uint32_t key = keys_in[i];
-            const uint32_t id = idx_in ? idx_in[i] : (uint32_t)i;
-            const uint32_t d = (key >> shift) & 255u;
+            const uint32_t d = (key[it] >> shift) & (kDigits - 1);
             const uint32_t peers = __match_any_sync(active, d);
-            const uint32_t rank = __popc(peers & lt);
-            const uint32_t dst = pos[warp][d] + rank;
-            keys_out[dst] = key;
-            idx_out[dst] = id;
+            const uint32_t r = __popc(peers & lt);
+            rank[it] = pos[warp][d] + r;
             __syncwarp(active);
-            if (rank == 0) pos[warp][d] += __popc(peers);
+            if (r == 0) pos[warp][d] += __popc(peers);
         }
         __syncwarp();
     }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kDPT; ++k) {   // per digit: tile offset, then the warps in order
+        const uint32_t d = threadIdx.x + k * kSortThreads;
+        uint32_t run = offsets[(size_t)d * n_tiles + blockIdx.x];
+#pragma unroll
+        for (int w = 0; w < kSortThreads / 32; ++w) {
+            const uint32_t c = pos[w][d];
+            pos[w][d] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int it = 0; it < kItems; ++it) {
+        const uint64_t i = base + it * 32 + lane;
+        if (i < n) {
+            const uint32_t dst = pos[warp][(key[it] >> shift) & (kDigits - 1)] + rank[it];
+            keys_out[dst] = key[it];
+            idx_out[dst] = idx_in ? idx_in[i] : (uint32_t)i;
+        }
+    }
 }
 
+// scratch ints: the (digit, tile) table + one row of digit totals per pass
 size_t morton_sort_hist_ints(uint64_t n) {
-    const uint64_t chunks = (n + kChunk - 1) / kChunk;
-    return (size_t)(chunks ? chunks : 1) * 256;
+    const uint64_t tiles = (n + kTile - 1) / kTile;
+    return (size_t)(tiles ? tiles : 1) * kDigits + (size_t)kPasses * kDigits;
 }
 
 int launch_morton_sort(const float* x, uint64_t n, uint32_t* keys_a, uint32_t* keys_b, uint32_t* idx_a, uint32_t* perm_out,
                        uint32_t* hist, cudaStream_t stream) {
     if (n == 0) return 0;
     int launches = 0;
-    morton_key_kernel<<<(unsigned)((n + 255) / 256), 256, 0, stream>>>(x, n, keys_a);
-    ++launches;
-    const uint32_t n_chunks = (uint32_t)((n + kChunk - 1) / kChunk);
-    const unsigned blocks = (n_chunks + kSortThreads / 32 - 1) / (kSortThreads / 32);
+    const uint32_t n_tiles = (uint32_t)((n + kTile - 1) / kTile);
+    uint32_t* tot = hist + (size_t)n_tiles * kDigits;
+    cudaMemsetAsync(tot, 0, sizeof(uint32_t) * kPasses * kDigits, stream);
     uint32_t* kin = keys_a;
     uint32_t* kout = keys_b;
     const uint32_t* iin = nullptr;
-    uint32_t* iout = idx_a;
-    for (int pass = 0; pass < 4; ++pass) {
-        const uint32_t shift = 8 * pass;
-        radix_hist_kernel<<<blocks, kSortThreads, 0, stream>>>(kin, n, shift, n_chunks, hist);
-        scan_kernel<<<1, 1024, 0, stream>>>(hist, n_chunks * 256);
-        radix_scatter_kernel<<<blocks, kSortThreads, 0, stream>>>(kin, iin, n, shift, n_chunks, hist, kout, iout);
+    // three passes: the index arrays alternate so that the last scatter writes perm_out
+    uint32_t* iout = perm_out;
+    for (int pass = 0; pass < kPasses; ++pass) {
+        const uint32_t shift = kBits * pass;
+        uint32_t* t = tot + pass * kDigits;
+        if (pass == 0) radix_hist_kernel<true><<<n_tiles, kSortThreads, 0, stream>>>(x, kin, n, shift, n_tiles, hist, t);
+        else radix_hist_kernel<false><<<n_tiles, kSortThreads, 0, stream>>>(nullptr, kin, n, shift, n_tiles, hist, t);
+        scan_kernel<<<kDigits, kSortThreads, 0, stream>>>(hist, t, n_tiles);
+        radix_scatter_kernel<<<n_tiles, kSortThreads, 0, stream>>>(kin, iin, n, shift, n_tiles, hist, kout, iout);
         launches += 3;
-        uint32_t* t = kin; kin = kout; kout = t;
+        uint32_t* tk = kin; kin = kout; kout = tk;
         iin = iout;
         iout = (iout == idx_a) ? perm_out : idx_a;
     }
-    return launches;   // 4 passes: the last scatter wrote perm_out
+    return launches;   // odd number of passes starting at perm_out: the last scatter wrote perm_out
 }
 
 }  // namespace oo
