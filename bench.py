@@ -347,6 +347,68 @@ def run_sweep(args):
     return 0
 
 
+def run_raycast(args):
+    """--sweep 5: primary visibility on the device: oo_raycast alone, and camera -> RGB
+    (oo_raycast + oo_query, no host copy of the queries), for config 1's and config 3's frames."""
+    import numpy as np
+    import torch
+    import gen
+    import paper_2606_08469_b200 as P
+    from oracle import oo_raycast as RC
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
+    flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.current_stream(dev)
+
+    def timed(fn, reps):
+        for _ in range(3):
+            flush.zero_()
+            fn()
+        evs = []
+        for _ in range(reps):
+            flush.zero_()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            fn()
+            e1.record(stream)
+            evs.append((e0, e1))
+        torch.cuda.synchronize(dev)
+        t = sorted(a.elapsed_time(b) for a, b in evs)
+        return t[len(t) // 2]
+
+    rows = []
+    for cfg in (1, 3):
+        w, desc = workload_for(cfg)
+        cam, sc = w.camera, w.scene
+        ctx = P.OctaOctree(0).upload_workload(w)
+        ctx.oo_upload_scene(sc.spheres, sc.lo, sc.hi)
+        n = cam.width * cam.height
+        out = tuple(torch.empty((n, 3), dtype=torch.float32, device=dev) for _ in range(3))
+        rgb = torch.empty((n, 3), dtype=torch.float32, device=dev)
+        cast = lambda: ctx.oo_raycast(cam.eye, cam.look, cam.up, cam.vfov_deg, cam.width, cam.height, out=out)
+        t_c = timed(cast, args.steps)
+        t_q = timed(lambda: ctx.oo_query(out[0], out[1], out[2], rgb=rgb), args.steps)
+        t_b = timed(lambda: (cast(), ctx.oo_query(out[0], out[1], out[2], rgb=rgb)), args.steps)
+        n_surf = len(sc.spheres) + 5
+        row = {"config": cfg, "frame": "%dx%d" % (cam.width, cam.height), "surfaces": n_surf, "raycast_ms": t_c, "query_ms": t_q,
+               "raycast_plus_query_ms": t_b, "Mrays_per_s": n / t_c / 1e3, "camera_to_rgb_Mqueries_per_s": n / t_b / 1e3,
+               "ray_surface_tests_per_s": n * n_surf / (t_c * 1e-3), "bytes_written_per_ray": 36}
+        if not args.no_cpu_baseline and not args.quick:
+            rws = np.arange(0, cam.height, 32)
+            t0 = time.perf_counter()
+            RC.raycast(sc.spheres, sc.lo, sc.hi, cam.eye, cam.look, cam.up, cam.vfov_deg, cam.width, cam.height, rows=rws)
+            dt = time.perf_counter() - t0
+            row["cpu_oracle_Mrays_per_s"] = len(rws) * cam.width / dt / 1e6
+        rows.append(row)
+        ctx.close()
+    print(json.dumps({"sweep": "primary visibility on the device (f5): oo_raycast, fp64 arithmetic, one thread per pixel", "rows": rows,
+                      "l2": "flushed between launches (256 MB memset)", "timing": "median of CUDA-event times", "data": "synthetic",
+                      "cpu_oracle": "oracle/oo_raycast.py (numpy float64, 1 core) on every 32nd scanline"}))
+    return 0
+
+
 def run_full(args):
     """--sweep 8: the paper's FULL query at the paper's own shapes: 8 consecutive levels
     (depths 2..9), C = 4 fp32 vertex maps of resolution 2^8+1 .. 2^1+1, 8-neighbour trilinear blend, disparity-shifted
@@ -450,7 +512,7 @@ def main():
     ap.add_argument("--path", default="auto", choices=["auto", "mma", "tc", "tm", "unfused", "generic"])
     ap.add_argument("--ref-sample", type=int, default=131072, help="queries in the CPU-oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--sweep", type=int, default=0, choices=[0, 2, 4, 8], help="side measurements of configs[2] / configs[4] / (8) the paper's full query at its own shapes (a table, not the headline line)")
+    ap.add_argument("--sweep", type=int, default=0, choices=[0, 2, 4, 5, 8], help="side measurements of configs[2] / configs[4] / (8) the paper's full query at its own shapes (a table, not the headline line)")
     ap.add_argument("--sweep-max-log2", type=int, default=24)
     ap.add_argument("--sweep-min-log2", type=int, default=16)
     ap.add_argument("--sweep-dist", default="both", choices=["both", "coherent", "incoherent"])
@@ -461,6 +523,8 @@ def main():
     args.warmup_ref = max(0, min(args.warmup, 1))
     if args.sweep == 8:
         return run_full(args)
+    if args.sweep == 5:
+        return run_raycast(args)
     if args.sweep:
         return run_sweep(args)
     return run_reference(args) if args.impl == "reference" else run_ours(args)

@@ -150,6 +150,25 @@ typedef struct {
     const float* disparity;      /* [n] d^ of Eq. 7-9, required by OO_LOOKUP_SHIFTED, ignored otherwise (may be NULL) */
 } oo_queries;
 
+/* ---- Primary visibility of an analytic scene ("standard primary visibility"). ----
+ * The scene BASELINE.json's configs describe: spheres plus a 5-plane box (x=lo, x=hi, y=lo, y=hi, z=lo, each a rectangle
+ * spanning [lo,hi] on the other two axes, open towards +z).  The paper traces its G-buffers with Mitsuba 3;
+ * this is the stand-in that lets a frame be produced on the device. */
+typedef struct {
+    uint32_t n_spheres;          /* 0..2048 */
+    const double* spheres;       /* HOST [n_spheres][4] = centre x, y, z, radius */
+    double lo, hi;               /* the box planes */
+} oo_scene_desc;
+
+/* Pinhole camera: f = normalize(look - eye), r = normalize(f x up), u = r x f; pixel (i, j) of a width x height frame is
+ * sampled at its centre, d = normalize(f + px r + py u) with px = (2(i+1/2)/width - 1) tan(vfov/2) width/height and
+ * py = (1 - 2(j+1/2)/height) tan(vfov/2); scanline order (query index = j*width + i). */
+typedef struct {
+    double eye[3], look[3], up[3];
+    double vfov_deg;             /* vertical field of view, degrees */
+    uint32_t width, height;
+} oo_camera_desc;
+
 typedef struct {
     uint64_t launches;           /* kernels launched by this context so far (all kinds) */
     uint64_t query_launches;     /* kernels launched by oo_query / oo_encode / oo_sort_queries / oo_query_host */
@@ -214,6 +233,17 @@ OO_API oo_status oo_query(oo_ctx* ctx, const oo_queries* q, float* d_rgb, void* 
  * copies RGB back to h_rgb (HOST [n][out_dim]) and synchronises the stream.  q->perm must be NULL.  Pinned host
  * memory makes the copies asynchronous; pageable memory works.  Needs oo_reserve(n). */
 OO_API oo_status oo_query_host(oo_ctx* ctx, const oo_queries* q, float* h_rgb, void* cuda_stream);
+
+/* Copy the scene into library-owned device memory.  Synchronises the stream. */
+OO_API oo_status oo_upload_scene(oo_ctx* ctx, const oo_scene_desc* scene, void* cuda_stream);
+/* Trace one primary ray per pixel against the uploaded scene and write the queries of the frame: d_x (hit point), d_nrm
+ * (sphere: outward normal (x - c)/R; plane: the unit axis vector pointing into the box), d_wo = -d, each DEVICE
+ * [width*height][3] fp32, and optionally d_surf DEVICE [width*height] (sphere index, n_spheres + plane index, -1 = miss;
+ * a miss writes zeros).  The nearest hit with t > 1e-9 wins; among equal t the earlier surface (spheres in order, then
+ * the planes).  Arithmetic: double precision, every operation rounded on its own, outputs rounded once to fp32
+ * (DESIGN.md "Ray cast").  The buffers can be passed to oo_query / oo_encode as they are. */
+OO_API oo_status oo_raycast(oo_ctx* ctx, const oo_camera_desc* cam, float* d_x, float* d_nrm, float* d_wo, int32_t* d_surf,
+                     void* cuda_stream);
 
 /* Debug read-back of the library's re-laid-out atlas: copies the padded map of (level, slot) to HOST
  * h_out [(R+2)][(R+2)][F] in the tree's dtype.  Synchronous. */

@@ -19,7 +19,7 @@ _STATUS = {0: "OO_OK", 1: "OO_ERR_INVALID_ARG", 2: "OO_ERR_NOT_READY", 3: "OO_ER
 
 EXPORTED_SYMBOLS = ["oo_create", "oo_destroy", "oo_last_error", "oo_upload_tree", "oo_upload_mlp", "oo_reserve", "oo_set_path",
                     "oo_get_info", "oo_sort_queries", "oo_encode", "oo_query", "oo_query_host", "oo_read_padded_map", "oo_set_mode",
-                    "oo_encode_full"]
+                    "oo_encode_full", "oo_upload_scene", "oo_raycast"]
 
 
 class OOError(RuntimeError):
@@ -43,6 +43,15 @@ class _MlpDesc(C.Structure):
 class _Queries(C.Structure):
     _fields_ = [("n", C.c_uint64), ("x", C.c_void_p), ("nrm", C.c_void_p), ("wo", C.c_void_p), ("extra", C.c_void_p),
                 ("n_extra", C.c_uint32), ("perm", C.c_void_p), ("disparity", C.c_void_p)]
+
+
+class _SceneDesc(C.Structure):
+    _fields_ = [("n_spheres", C.c_uint32), ("spheres", C.c_void_p), ("lo", C.c_double), ("hi", C.c_double)]
+
+
+class _CameraDesc(C.Structure):
+    _fields_ = [("eye", C.c_double * 3), ("look", C.c_double * 3), ("up", C.c_double * 3), ("vfov_deg", C.c_double),
+                ("width", C.c_uint32), ("height", C.c_uint32)]
 
 
 class _Mode(C.Structure):
@@ -87,6 +96,8 @@ def load_library():
     L.oo_query_host.argtypes = [vp, C.POINTER(_Queries), vp, vp]
     L.oo_read_padded_map.argtypes = [vp, u32, u32, vp]
     L.oo_set_mode.argtypes = [vp, C.POINTER(_Mode)]
+    L.oo_upload_scene.argtypes = [vp, C.POINTER(_SceneDesc), vp]
+    L.oo_raycast.argtypes = [vp, C.POINTER(_CameraDesc), vp, vp, vp, vp, vp]
     L.oo_encode_full.argtypes = [vp, C.POINTER(_Queries), vp, vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
         if name not in ("oo_destroy", "oo_last_error"):
@@ -261,6 +272,27 @@ class OctaOctree:
         q = _Queries(n, ptr(x), ptr(nrm), ptr(wo), ptr(extra), ne, None, ptr(disparity))
         self._check(self._L.oo_query_host(self._ctx, C.byref(q), C.c_void_p(ptr(rgb)), self._stream()))
         return rgb
+
+    def oo_upload_scene(self, spheres, lo: float, hi: float):
+        """spheres: [n][4] (centre, radius), float64."""
+        import numpy as np
+        sp = np.ascontiguousarray(spheres, np.float64).reshape(-1, 4)
+        d = _SceneDesc(sp.shape[0], _np_ptr(sp) if sp.shape[0] else None, float(lo), float(hi))
+        self._check(self._L.oo_upload_scene(self._ctx, C.byref(d), self._stream()))
+
+    def oo_raycast(self, eye, look, up, vfov_deg: float, width: int, height: int, want_surf: bool = False, out=None):
+        """Primary hits of a frame as query tensors (x, nrm, wo[, surf]) on the device, scanline order."""
+        torch = self._torch
+        n = int(width) * int(height)
+        if out is None:
+            out = tuple(torch.empty((n, 3), dtype=torch.float32, device=self.device) for _ in range(3))
+        x, nrm, wo = out
+        surf = torch.empty(n, dtype=torch.int32, device=self.device) if want_surf else None
+        cam = _CameraDesc((C.c_double * 3)(*[float(v) for v in eye]), (C.c_double * 3)(*[float(v) for v in look]),
+                          (C.c_double * 3)(*[float(v) for v in up]), float(vfov_deg), int(width), int(height))
+        self._check(self._L.oo_raycast(self._ctx, C.byref(cam), C.c_void_p(x.data_ptr()), C.c_void_p(nrm.data_ptr()),
+                                       C.c_void_p(wo.data_ptr()), C.c_void_p(surf.data_ptr()) if want_surf else None, self._stream()))
+        return (x, nrm, wo, surf) if want_surf else (x, nrm, wo)
 
     def oo_read_padded_map(self, level: int, slot: int, R: int):
         import numpy as np

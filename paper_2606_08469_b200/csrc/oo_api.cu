@@ -41,6 +41,12 @@ struct oo_ctx {
     void* d_image = nullptr;
     void* d_image_tc = nullptr;
 
+    // scene (f5)
+    bool have_scene = false;
+    void* d_spheres = nullptr;
+    uint32_t n_spheres = 0;
+    double scene_lo = 0.0, scene_hi = 1.0;
+
     // scratch
     uint64_t reserved = 0;
     void* d_feat = nullptr;    uint64_t feat_bytes = 0;
@@ -181,6 +187,7 @@ extern "C" OO_API void oo_destroy(oo_ctx* c) {
         free_tree(c);
         free_dev(c->d_image);
         free_dev(c->d_image_tc);
+        free_dev(c->d_spheres);
         free_scratch(c);
     }
     delete c;
@@ -709,6 +716,53 @@ extern "C" OO_API oo_status oo_query_host(oo_ctx* c, const oo_queries* q, float*
     OO_CUDA(c, cudaMemcpyAsync(h_rgb, c->d_rgb, q->n * 4 * c->M.out_dim, cudaMemcpyDeviceToHost, stream));
     OO_CUDA(c, cudaStreamSynchronize(stream));
     return OO_OK;
+}
+
+extern "C" OO_API oo_status oo_upload_scene(oo_ctx* c, const oo_scene_desc* sc, void* cuda_stream) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (!sc) return fail(c, OO_ERR_INVALID_ARG, "scene is NULL");
+    if (sc->n_spheres > 2048) return fail(c, OO_ERR_UNSUPPORTED, "%u spheres: at most 2048 (they are kept in shared memory)", sc->n_spheres);
+    if (sc->n_spheres && !sc->spheres) return fail(c, OO_ERR_INVALID_ARG, "scene.spheres is NULL");
+    if (!(sc->lo < sc->hi)) return fail(c, OO_ERR_INVALID_ARG, "scene box: need lo < hi");
+    for (uint32_t s = 0; s < sc->n_spheres; ++s)
+        if (!(sc->spheres[4 * s + 3] > 0.0)) return fail(c, OO_ERR_INVALID_ARG, "sphere %u: radius must be positive", s);
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    DeviceGuard g(c->device);
+    free_dev(c->d_spheres);
+    c->have_scene = false;
+    OO_CUDA(c, cudaMalloc(&c->d_spheres, std::max<size_t>(sc->n_spheres, 1) * 4 * sizeof(double)));
+    if (sc->n_spheres) OO_CUDA(c, cudaMemcpyAsync(c->d_spheres, sc->spheres, (size_t)sc->n_spheres * 4 * sizeof(double), cudaMemcpyHostToDevice, stream));
+    OO_CUDA(c, cudaStreamSynchronize(stream));
+    c->n_spheres = sc->n_spheres; c->scene_lo = sc->lo; c->scene_hi = sc->hi;
+    c->have_scene = true;
+    return OO_OK;
+}
+
+extern "C" OO_API oo_status oo_raycast(oo_ctx* c, const oo_camera_desc* cam, float* d_x, float* d_nrm, float* d_wo, int32_t* d_surf,
+                                void* cuda_stream) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (!c->have_scene) return fail(c, OO_ERR_NOT_READY, "no scene uploaded");
+    if (!cam) return fail(c, OO_ERR_INVALID_ARG, "camera is NULL");
+    const uint64_t n = (uint64_t)cam->width * cam->height;
+    if (n >= (1ull << 32)) return fail(c, OO_ERR_UNSUPPORTED, "more than 2^32-1 pixels per frame");
+    if (n && (!d_x || !d_nrm || !d_wo)) return fail(c, OO_ERR_INVALID_ARG, "output buffer is NULL");
+    if (!(cam->vfov_deg > 0.0 && cam->vfov_deg < 180.0)) return fail(c, OO_ERR_INVALID_ARG, "vfov_deg must lie in (0, 180)");
+    double fl = 0.0, cr = 0.0;
+    {
+        const double f[3] = {cam->look[0] - cam->eye[0], cam->look[1] - cam->eye[1], cam->look[2] - cam->eye[2]};
+        fl = f[0] * f[0] + f[1] * f[1] + f[2] * f[2];
+        const double r[3] = {f[1] * cam->up[2] - f[2] * cam->up[1], f[2] * cam->up[0] - f[0] * cam->up[2], f[0] * cam->up[1] - f[1] * cam->up[0]};
+        cr = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
+    }
+    if (!(fl > 0.0) || !(cr > 0.0)) return fail(c, OO_ERR_INVALID_ARG, "degenerate camera: look == eye, or up parallel to the view direction");
+    if (oo_status st = check_async(c)) return st;
+    if (n == 0) return OO_OK;
+    DeviceGuard g(c->device);
+    const int k = launch_raycast((const double*)c->d_spheres, c->n_spheres, c->scene_lo, c->scene_hi, cam->eye, cam->look, cam->up,
+                                 cam->vfov_deg, cam->width, cam->height, d_x, d_nrm, d_wo, d_surf, (cudaStream_t)cuda_stream);
+    if (k < 0) return fail(c, OO_ERR_UNSUPPORTED, "ray-cast kernel unavailable for this scene size");
+    count(c, k);
+    return check_async(c);
 }
 
 extern "C" OO_API oo_status oo_read_padded_map(oo_ctx* c, uint32_t level, uint32_t slot, void* h_out) {

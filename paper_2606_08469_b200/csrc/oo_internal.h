@@ -110,6 +110,9 @@ int launch_fused_full_w64(const TreeParams& T, const MlpParams& M, const QueryPa
                           int n_sms, cudaStream_t stream);
 int launch_fused_full_w128(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const FullModeH& mode, float* rgb,
                            int n_sms, cudaStream_t stream);
+int launch_raycast(const double* d_spheres, uint32_t n_spheres, double lo, double hi, const double eye[3], const double look[3],
+                   const double up[3], double vfov_deg, uint32_t width, uint32_t height, float* x, float* nrm, float* wo,
+                   int32_t* surf, cudaStream_t stream);
 int launch_morton_sort(const float* x, uint64_t n, uint32_t* keys_a, uint32_t* keys_b, uint32_t* idx_a, uint32_t* perm_out,
                        uint32_t* hist, cudaStream_t stream);
 size_t morton_sort_hist_ints(uint64_t n);
