@@ -229,9 +229,13 @@ OO_API oo_status oo_encode_full(oo_ctx* ctx, const oo_queries* q, float* d_featu
  * launch as well). */
 OO_API oo_status oo_query(oo_ctx* ctx, const oo_queries* q, float* d_rgb, void* cuda_stream);
 
-/* The whole path from HOST buffers: copies the queries to the device (cudaMemcpyAsync on the stream), runs oo_query,
- * copies RGB back to h_rgb (HOST [n][out_dim]) and synchronises the stream.  q->perm must be NULL.  Pinned host
- * memory makes the copies asynchronous; pageable memory works.  Needs oo_reserve(n). */
+/* The whole path from HOST buffers, as a chunked three-stage pipeline: the queries are split into up to 4 chunks
+ * (environment variable OO_HOST_CHUNKS = 1..16 overrides the count;
+ * whole 128-query tiles, at least 65,536 queries each); chunk i+1 is copied to the device on a library-owned copy-in
+ * stream while oo_query runs chunk i on the caller's stream and chunk i-1's RGB returns to h_rgb (HOST [n][out_dim]) on
+ * a library-owned copy-out stream.  Work starts after everything already enqueued on the caller's stream; the call
+ * returns after all three streams have finished (it synchronises).  q->perm must be NULL.  Pinned host memory lets the
+ * copies overlap; pageable memory works but serialises.  Needs oo_reserve(n).  Launches one fused kernel per chunk. */
 OO_API oo_status oo_query_host(oo_ctx* ctx, const oo_queries* q, float* h_rgb, void* cuda_stream);
 
 /* Copy the scene into library-owned device memory.  Synchronises the stream. */

@@ -5,6 +5,7 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -52,6 +53,12 @@ struct oo_ctx {
     void* d_feat = nullptr;    uint64_t feat_bytes = 0;
     uint32_t *d_keys_a = nullptr, *d_keys_b = nullptr, *d_idx_a = nullptr, *d_hist = nullptr;
     float *d_qx = nullptr, *d_qn = nullptr, *d_qw = nullptr, *d_qe = nullptr, *d_rgb = nullptr, *d_qd = nullptr;
+
+    // oo_query_host pipeline: copy-in and copy-out streams beside the caller's stream, one event pair per chunk
+    static constexpr int kMaxChunks = 16;
+    bool have_pipe = false;
+    cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_out = nullptr, ev_in[kMaxChunks] = {}, ev_k[kMaxChunks] = {};
 };
 
 namespace {
@@ -113,6 +120,21 @@ void free_scratch(oo_ctx* c) {
                    (void**)&c->d_qn,     (void**)&c->d_qw,     (void**)&c->d_qe,    (void**)&c->d_rgb, (void**)&c->d_qd};
     for (void** p : ps) free_dev(*p);
     c->reserved = 0;
+}
+
+void free_pipe(oo_ctx* c) {
+    if (c->s_h2d) cudaStreamDestroy(c->s_h2d);
+    if (c->s_d2h) cudaStreamDestroy(c->s_d2h);
+    if (c->ev_start) cudaEventDestroy(c->ev_start);
+    if (c->ev_out) cudaEventDestroy(c->ev_out);
+    for (int i = 0; i < oo_ctx::kMaxChunks; ++i) {
+        if (c->ev_in[i]) cudaEventDestroy(c->ev_in[i]);
+        if (c->ev_k[i]) cudaEventDestroy(c->ev_k[i]);
+        c->ev_in[i] = c->ev_k[i] = nullptr;
+    }
+    c->s_h2d = c->s_d2h = nullptr;
+    c->ev_start = c->ev_out = nullptr;
+    c->have_pipe = false;
 }
 
 bool is_pow2(uint32_t v) { return v && !(v & (v - 1)); }
@@ -189,6 +211,7 @@ extern "C" OO_API void oo_destroy(oo_ctx* c) {
         free_dev(c->d_image_tc);
         free_dev(c->d_spheres);
         free_scratch(c);
+        free_pipe(c);
     }
     delete c;
 }
@@ -704,16 +727,55 @@ extern "C" OO_API oo_status oo_query_host(oo_ctx* c, const oo_queries* q, float*
     if (!c->have_mlp) return fail(c, OO_ERR_NOT_READY, "no MLP uploaded");
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     DeviceGuard g(c->device);
-    OO_CUDA(c, cudaMemcpyAsync(c->d_qx, q->x, q->n * 12, cudaMemcpyHostToDevice, stream));
-    OO_CUDA(c, cudaMemcpyAsync(c->d_qn, q->nrm, q->n * 12, cudaMemcpyHostToDevice, stream));
-    OO_CUDA(c, cudaMemcpyAsync(c->d_qw, q->wo, q->n * 12, cudaMemcpyHostToDevice, stream));
-    if (q->n_extra) OO_CUDA(c, cudaMemcpyAsync(c->d_qe, q->extra, q->n * 4 * q->n_extra, cudaMemcpyHostToDevice, stream));
-    if (q->disparity) OO_CUDA(c, cudaMemcpyAsync(c->d_qd, q->disparity, q->n * 4, cudaMemcpyHostToDevice, stream));
-    oo_queries dq = *q;
-    dq.x = c->d_qx; dq.nrm = c->d_qn; dq.wo = c->d_qw; dq.extra = q->n_extra ? c->d_qe : nullptr;
-    dq.disparity = q->disparity ? c->d_qd : nullptr;
-    if (oo_status st = query_device(c, &dq, c->d_rgb, stream)) return st;
-    OO_CUDA(c, cudaMemcpyAsync(h_rgb, c->d_rgb, q->n * 4 * c->M.out_dim, cudaMemcpyDeviceToHost, stream));
+    if (!c->have_pipe) {
+        OO_CUDA(c, cudaStreamCreateWithFlags(&c->s_h2d, cudaStreamNonBlocking));
+        OO_CUDA(c, cudaStreamCreateWithFlags(&c->s_d2h, cudaStreamNonBlocking));
+        OO_CUDA(c, cudaEventCreateWithFlags(&c->ev_start, cudaEventDisableTiming));
+        OO_CUDA(c, cudaEventCreateWithFlags(&c->ev_out, cudaEventDisableTiming));
+        for (int i = 0; i < oo_ctx::kMaxChunks; ++i) {
+            OO_CUDA(c, cudaEventCreateWithFlags(&c->ev_in[i], cudaEventDisableTiming));
+            OO_CUDA(c, cudaEventCreateWithFlags(&c->ev_k[i], cudaEventDisableTiming));
+        }
+        c->have_pipe = true;
+    }
+    // Chunked three-stage pipeline: copy-in of chunk i+1 (s_h2d) overlaps the kernel of chunk i (caller's stream) and the
+    // copy-out of chunk i-1 (s_d2h); PCIe is full duplex, so a frame costs about its copy-in time instead of the sum of the three.
+    // Chunks are whole multiples of 128-query tiles and at least 64 Ki queries, so every chunk still fills the persistent grid.
+    // Measured on B200 (config 1, pinned buffers): 1 chunk 1.07-1.10 ms, 2: 0.99, 4: 0.98, 8: 1.01-1.03, 16: 1.15 ms; copy-in slows
+    // ~12 % while copy-out shares the link, so the floor is ~0.85 ms of copy-in + the last chunk's kernel and copy-out.
+    const uint64_t n = q->n;
+    static const int want = [] { const char* e = getenv("OO_HOST_CHUNKS"); const int v = e ? atoi(e) : 0; return v > 0 ? std::min(v, oo_ctx::kMaxChunks) : 4; }();
+    uint64_t chunk = (n + want - 1) / want;
+    chunk = std::max<uint64_t>((chunk + 127) & ~127ull, 65536);
+    const int n_chunks = (int)((n + chunk - 1) / chunk);
+    const uint32_t od = c->M.out_dim;
+    OO_CUDA(c, cudaEventRecord(c->ev_start, stream));
+    OO_CUDA(c, cudaStreamWaitEvent(c->s_h2d, c->ev_start, 0));
+    OO_CUDA(c, cudaStreamWaitEvent(c->s_d2h, c->ev_start, 0));
+    for (int i = 0; i < n_chunks; ++i) {
+        const uint64_t o = (uint64_t)i * chunk, m = std::min(chunk, n - o);
+        OO_CUDA(c, cudaMemcpyAsync(c->d_qx + o * 3, q->x + o * 3, m * 12, cudaMemcpyHostToDevice, c->s_h2d));
+        OO_CUDA(c, cudaMemcpyAsync(c->d_qn + o * 3, q->nrm + o * 3, m * 12, cudaMemcpyHostToDevice, c->s_h2d));
+        OO_CUDA(c, cudaMemcpyAsync(c->d_qw + o * 3, q->wo + o * 3, m * 12, cudaMemcpyHostToDevice, c->s_h2d));
+        if (q->n_extra) OO_CUDA(c, cudaMemcpyAsync(c->d_qe + o * q->n_extra, q->extra + o * q->n_extra, m * 4 * q->n_extra, cudaMemcpyHostToDevice, c->s_h2d));
+        if (q->disparity) OO_CUDA(c, cudaMemcpyAsync(c->d_qd + o, q->disparity + o, m * 4, cudaMemcpyHostToDevice, c->s_h2d));
+        OO_CUDA(c, cudaEventRecord(c->ev_in[i], c->s_h2d));
+        OO_CUDA(c, cudaStreamWaitEvent(stream, c->ev_in[i], 0));
+        oo_queries dq = *q;
+        dq.n = m;
+        dq.x = c->d_qx + o * 3; dq.nrm = c->d_qn + o * 3; dq.wo = c->d_qw + o * 3;
+        dq.extra = q->n_extra ? c->d_qe + o * q->n_extra : nullptr;
+        dq.disparity = q->disparity ? c->d_qd + o : nullptr;
+        if (oo_status st = query_device(c, &dq, c->d_rgb + o * od, stream)) {
+            cudaStreamSynchronize(c->s_h2d); cudaStreamSynchronize(c->s_d2h); cudaStreamSynchronize(stream);
+            return st;
+        }
+        OO_CUDA(c, cudaEventRecord(c->ev_k[i], stream));
+        OO_CUDA(c, cudaStreamWaitEvent(c->s_d2h, c->ev_k[i], 0));
+        OO_CUDA(c, cudaMemcpyAsync(h_rgb + o * od, c->d_rgb + o * od, m * 4 * od, cudaMemcpyDeviceToHost, c->s_d2h));
+    }
+    OO_CUDA(c, cudaEventRecord(c->ev_out, c->s_d2h));
+    OO_CUDA(c, cudaStreamWaitEvent(stream, c->ev_out, 0));
     OO_CUDA(c, cudaStreamSynchronize(stream));
     return OO_OK;
 }

@@ -233,6 +233,29 @@ def test_query_host_equals_query(P):
     assert np.array_equal(host2, dev)
 
 
+def test_query_host_pipeline_many_chunks(P):
+    """oo_query_host splits the frame into chunks that overlap copy-in, kernel and copy-out: several chunks with a ragged
+    last one must give the same bytes as one device-side oo_query, with and without extras, called twice in a row."""
+    w = gen.scene_workload(2, width=640, height=333)          # 213,120 queries -> 4 chunks of 65,536 (last: 16,512)
+    q = w.queries
+    ctx = P.OctaOctree(0).upload_workload(w)
+    ctx.oo_reserve(q.n)
+    x, n, wo, ex = _dev(q)
+    dev = ctx.oo_query(x, n, wo, ex).cpu().numpy()
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    hx, hn, hw, he = pin(q.x), pin(q.nrm), pin(q.wo), pin(q.extra)
+    l0 = ctx.oo_get_info()["query_launches"]
+    for _ in range(2):
+        out = torch.full((q.n, 3), float("nan")).pin_memory()
+        host = ctx.oo_query_host(hx, hn, hw, he, rgb=out)
+        assert np.array_equal(host.numpy(), dev)
+    assert ctx.oo_get_info()["query_launches"] - l0 == 2 * 4          # 213,120 = 3 x 65,536 + 16,512
+    s = torch.cuda.Stream()
+    with torch.cuda.stream(s):
+        host = ctx.oo_query_host(hx, hn, hw, he)            # the binding passes torch's current stream
+    assert np.array_equal(host.numpy(), dev)
+
+
 def test_error_codes(P):
     w = gen.config0()
     ctx = P.OctaOctree(0)
