@@ -29,6 +29,8 @@ STREAM_WEIGHTS = 200    # + layer
 STREAM_POS, STREAM_NRM, STREAM_DIR, STREAM_ROUGH = 3, 4, 5, 6
 STREAM_SCENE, STREAM_CAMERA, STREAM_INCOH, STREAM_SHUFFLE = 7, 8, 9, 10
 STREAM_DISPARITY, STREAM_ALBEDO = 11, 12
+STREAM_HASHGRID = 300   # + level
+STREAM_DISP_WEIGHTS = 400   # + layer
 
 
 def build_lib(force: bool = False) -> str:
@@ -314,6 +316,44 @@ def make_mlp(in_dim: int, n_hidden: int, seed: int, width: int = 64, out_dim: in
         w = normal(seed, STREAM_WEIGHTS + k, fan_in * fan_out) * np.sqrt(2.0 / fan_in)
         ws.append(f64_to_f16(w).reshape(fan_out, fan_in))
     return MLP(in_dim, width, n_hidden, out_dim, ws, out_act)
+
+
+@dataclass
+class DisparityNet:
+    """The disparity predictor g_psi of PAPER.md Eq. 7 as data: a multi-resolution hash grid over position plus a small MLP
+    (DESIGN.md §14 lists the hyper-parameters the paper leaves open)."""
+    res: List[int]                 # N_g: intervals per axis of level g, coarse -> fine
+    hash_log2: int                 # hashed levels have 2^hash_log2 entries; a level with (N_g+1)^3 <= that is dense
+    tables: List[np.ndarray]       # fp16 [T_g][Fh]
+    weights: List[np.ndarray]      # fp16 [64][G*Fh+3], [64][64], [1][64]
+
+    @property
+    def n_features(self) -> int:
+        return int(self.tables[0].shape[1])
+
+
+def hashgrid_resolutions(n_levels: int, n_min: int, n_max: int) -> List[int]:
+    """Geometric progression N_g = floor(N_min * b^g), b = (N_max/N_min)^(1/(G-1)) (the schedule of the paper's ref. [25])."""
+    if n_levels == 1:
+        return [int(n_min)]
+    b = np.exp((np.log(n_max) - np.log(n_min)) / (n_levels - 1))
+    return [int(np.floor(n_min * b ** g + 1e-9)) for g in range(n_levels)]
+
+
+def make_disparity_net(seed: int, n_levels: int = 8, n_min: int = 16, n_max: int = 512, hash_log2: int = 17, n_features: int = 2,
+                       n_hidden: int = 2, std: float = 0.5, res=None) -> DisparityNet:
+    """Seeded stand-in for a trained g_psi: table entries ~ N(0, std) in fp16, weights He-normal fp16, no biases."""
+    res = hashgrid_resolutions(n_levels, n_min, n_max) if res is None else [int(r) for r in res]
+    tables = []
+    for g, N in enumerate(res):
+        T = (N + 1) ** 3 if (N + 1) ** 3 <= (1 << hash_log2) else (1 << hash_log2)
+        tables.append(normal_f16(seed, STREAM_HASHGRID + g, T * n_features, std).reshape(T, n_features))
+    dims = [len(res) * n_features + 3] + [64] * n_hidden + [1]
+    ws = []
+    for k in range(n_hidden + 1):
+        w = normal(seed, STREAM_DISP_WEIGHTS + k, dims[k] * dims[k + 1]) * np.sqrt(2.0 / dims[k])
+        ws.append(f64_to_f16(w).reshape(dims[k + 1], dims[k]))
+    return DisparityNet(res, hash_log2, tables, ws)
 
 
 def random_queries(n: int, seed: int, n_extra: int = 0) -> Queries:
