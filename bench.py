@@ -488,6 +488,26 @@ def run_full(args):
                      "live_neighbour_lookups_per_query": live, "of": L * J, "algorithmic_bytes_per_query": bq,
                      "flop_per_query": flops, "byte_time_ms": bq * q.n / (hbm * 1e9) * 1e3, "flop_time_ms": flops * q.n / (tf * 1e12) * 1e3,
                      "roofline_frac": max(bq * q.n / (hbm * 1e9), flops * q.n / (tf * 1e12)) / (t * 1e-3)})
+    # Eq. 7 on the device: the disparity predictor alone, then the full query predicting d^ itself (two launches, no d^ input)
+    net = gen.make_disparity_net(0)
+    ctx.oo_upload_disparity(net.res, net.hash_log2, net.tables, net.weights)
+    ctx.oo_reserve(q.n)
+    mlp = gen.make_mlp(L * F + 13, 4, 0, width=128)
+    ctx.oo_upload_mlp(mlp.weights, mlp.out_act)
+    ctx.oo_set_mode("trilinear8", "shifted", "paper")
+    dbuf = torch.empty(q.n, dtype=torch.float32, device=dev)
+    G = len(net.res)
+    t_p = timed(lambda: ctx.oo_predict_disparity(x, nrm, wo, disparity=dbuf), args.steps)
+    t_pq = timed(lambda: ctx.oo_query(x, nrm, wo, ex, rgb=rgb), args.steps)
+    bq_p = G * 8 * 4 + 36 + 4
+    fl_p = 2 * ((2 * G + 3) * 64 + 64 * 64 + 64)
+    disparity_rows = [
+        {"variant": "disparity predictor g_psi alone (Eq. 7): %d-level hash grid %s, 2^%d-entry tables (%.1f MB), MLP %d->2x64->1 exp" %
+                    (G, net.res, net.hash_log2, sum(t.nbytes for t in net.tables) / 1e6, 2 * G + 3),
+         "ms": t_p, "Mqueries_per_s": q.n / t_p / 1e3, "algorithmic_bytes_per_query": bq_p, "flop_per_query": fl_p,
+         "byte_time_ms": bq_p * q.n / (hbm * 1e9) * 1e3, "roofline_frac": bq_p * q.n / (hbm * 1e9) / (t_p * 1e-3)},
+        {"variant": "full query predicting d^ itself (g_psi launch + fused full-query launch)", "ms": t_pq, "Mqueries_per_s": q.n / t_pq / 1e3}]
+    rows += disparity_rows
     out = {"sweep": "full query at the paper's shapes (PAPER.md implementation details; SURVEY.md 8(f) f1-f4)",
            "workload": "1024x1024 primary hits of the three-sphere scene; octree depth 9 (%d nodes), used depths %s, vertex maps R_l+1 = %s, C=%d fp32 (%.0f MB), "
                        "Eq. 12 attributes (13 scalars), synthetic disparity U(0.25,4)" %

@@ -238,6 +238,35 @@ OO_API oo_status oo_query(oo_ctx* ctx, const oo_queries* q, float* d_rgb, void* 
  * copies overlap; pageable memory works but serialises.  Needs oo_reserve(n).  Launches one fused kernel per chunk. */
 OO_API oo_status oo_query_host(oo_ctx* ctx, const oo_queries* q, float* h_rgb, void* cuda_stream);
 
+/* ---- The disparity predictor g_psi of Eq. 7 (the rest of SURVEY.md §8(f) row f3) ----
+ * d^(x, w_r) = g_psi(x, w_r): "a compact multi-resolution hash-grid network in the style of Instant-NGP" with "2 hidden
+ * layers of 64 neurons".  The paper gives no further hyper-parameter; the readings:
+ *   - G levels over position; level g has res[g] = N_g intervals per axis, i.e. (N_g+1)^3 grid vertices over [0,1]^3, and
+ *     a table of T_g entries of two fp16 features; T_g = (N_g+1)^3 when that is <= 2^hash_log2 (dense: vertex (i,j,k) owns
+ *     entry i + (N_g+1)(j + (N_g+1)k)), else T_g = 2^hash_log2 and vertex (i,j,k) reads entry
+ *     (i ^ j*2654435761 ^ k*805459861) mod 2^hash_log2, products modulo 2^32 (collisions are not resolved);
+ *   - x is clamped to [0,1]^3; p = x*N_g in fp32, cell c0 = min(floor(p), N_g-1), t = p - c0; the level's feature is the
+ *     trilinear interpolation of the cell's eight vertices;
+ *   - network input [e_0 .. e_{G-1} | w_r] (2G + 3 scalars, w_r = 2(n.wo)n - wo raw), hidden layers 64 wide, ReLU, no
+ *     biases, one output z, d^ = exp(z). */
+#define OO_MAX_GRID_LEVELS 16
+typedef struct {
+    uint32_t n_levels;           /* G in 1..OO_MAX_GRID_LEVELS */
+    uint32_t n_features;         /* features per entry: 2 */
+    const uint32_t* res;         /* HOST [G]: N_g, coarse to fine, each in 1..2^20 */
+    uint32_t hash_log2;          /* 4..28 */
+    const void* const* tables;   /* HOST [G] of HOST fp16 [T_g][2] */
+    uint32_t n_hidden;           /* 1..OO_MAX_HIDDEN (the paper: 2) */
+    const void* const* weights;  /* HOST [n_hidden+1] of HOST fp16 matrices: [64][2G+3], (n_hidden-1) x [64][64], [1][64] */
+} oo_disparity_desc;
+/* Copy the tables and weights into library-owned device memory.  Synchronises the stream.  From then on oo_query /
+ * oo_encode_full / oo_query_host with OO_LOOKUP_SHIFTED and queries.disparity == NULL predict d^ themselves (one extra
+ * launch into scratch: needs oo_reserve(n)). */
+OO_API oo_status oo_upload_disparity(oo_ctx* ctx, const oo_disparity_desc* d, void* cuda_stream);
+/* d_disparity: DEVICE [n] fp32 = d^ per query (q->x, q->nrm, q->wo; perm and extras ignored).  d_features: optional
+ * DEVICE [n][2G] fp32, the hash-grid features e(x) before they are rounded to fp16 for the network (NULL to skip). */
+OO_API oo_status oo_predict_disparity(oo_ctx* ctx, const oo_queries* q, float* d_disparity, float* d_features, void* cuda_stream);
+
 /* Copy the scene into library-owned device memory.  Synchronises the stream. */
 OO_API oo_status oo_upload_scene(oo_ctx* ctx, const oo_scene_desc* scene, void* cuda_stream);
 /* Trace one primary ray per pixel against the uploaded scene and write the queries of the frame: d_x (hit point), d_nrm

@@ -19,7 +19,7 @@ _STATUS = {0: "OO_OK", 1: "OO_ERR_INVALID_ARG", 2: "OO_ERR_NOT_READY", 3: "OO_ER
 
 EXPORTED_SYMBOLS = ["oo_create", "oo_destroy", "oo_last_error", "oo_upload_tree", "oo_upload_mlp", "oo_reserve", "oo_set_path",
                     "oo_get_info", "oo_sort_queries", "oo_encode", "oo_query", "oo_query_host", "oo_read_padded_map", "oo_set_mode",
-                    "oo_encode_full", "oo_upload_scene", "oo_raycast"]
+                    "oo_encode_full", "oo_upload_scene", "oo_raycast", "oo_upload_disparity", "oo_predict_disparity"]
 
 
 class OOError(RuntimeError):
@@ -43,6 +43,11 @@ class _MlpDesc(C.Structure):
 class _Queries(C.Structure):
     _fields_ = [("n", C.c_uint64), ("x", C.c_void_p), ("nrm", C.c_void_p), ("wo", C.c_void_p), ("extra", C.c_void_p),
                 ("n_extra", C.c_uint32), ("perm", C.c_void_p), ("disparity", C.c_void_p)]
+
+
+class _DisparityDesc(C.Structure):
+    _fields_ = [("n_levels", C.c_uint32), ("n_features", C.c_uint32), ("res", C.c_void_p), ("hash_log2", C.c_uint32),
+                ("tables", C.c_void_p), ("n_hidden", C.c_uint32), ("weights", C.c_void_p)]
 
 
 class _SceneDesc(C.Structure):
@@ -99,6 +104,8 @@ def load_library():
     L.oo_upload_scene.argtypes = [vp, C.POINTER(_SceneDesc), vp]
     L.oo_raycast.argtypes = [vp, C.POINTER(_CameraDesc), vp, vp, vp, vp, vp]
     L.oo_encode_full.argtypes = [vp, C.POINTER(_Queries), vp, vp, vp, vp]
+    L.oo_upload_disparity.argtypes = [vp, C.POINTER(_DisparityDesc), vp]
+    L.oo_predict_disparity.argtypes = [vp, C.POINTER(_Queries), vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
         if name not in ("oo_destroy", "oo_last_error"):
             getattr(L, name).restype = C.c_int
@@ -180,6 +187,29 @@ class OctaOctree:
                      {"none": OO_ACT_NONE, "exp": OO_ACT_EXP}[out_act])
         self._check(self._L.oo_upload_mlp(self._ctx, C.byref(d), self._stream()))
         self.out_dim = int(ws[-1].shape[0])
+
+    def oo_upload_disparity(self, res: Sequence[int], hash_log2: int, tables: Sequence, weights: Sequence):
+        """The disparity predictor g_psi (Eq. 7): per-level resolutions, fp16 tables [T_g][2], fp16 weights."""
+        import numpy as np
+        r = np.ascontiguousarray(res, np.uint32)
+        ts = [np.ascontiguousarray(t, np.float16) for t in tables]
+        ws = [np.ascontiguousarray(w, np.float16) for w in weights]
+        tp = (C.c_void_p * len(ts))(*[t.ctypes.data for t in ts])
+        wp = (C.c_void_p * len(ws))(*[w.ctypes.data for w in ws])
+        d = _DisparityDesc(len(ts), int(ts[0].shape[1]), _np_ptr(r), int(hash_log2), C.cast(tp, C.c_void_p), len(ws) - 1, C.cast(wp, C.c_void_p))
+        self._check(self._L.oo_upload_disparity(self._ctx, C.byref(d), self._stream()))
+        self.n_grid_levels = len(ts)
+
+    def oo_predict_disparity(self, x, nrm, wo, want_features: bool = False, disparity=None):
+        """d^ [n] fp32 on the device (and, with want_features, the hash-grid features [n][2G] fp32)."""
+        torch = self._torch
+        q, n = self._queries(x, nrm, wo, None, None, None)
+        if disparity is None:
+            disparity = torch.empty(n, dtype=torch.float32, device=self.device)
+        feats = torch.empty((n, 2 * self.n_grid_levels), dtype=torch.float32, device=self.device) if want_features else None
+        self._check(self._L.oo_predict_disparity(self._ctx, C.byref(q), C.c_void_p(disparity.data_ptr()),
+                                                 C.c_void_p(feats.data_ptr()) if want_features else None, self._stream()))
+        return (disparity, feats) if want_features else disparity
 
     def oo_reserve(self, n: int):
         self._check(self._L.oo_reserve(self._ctx, int(n)))

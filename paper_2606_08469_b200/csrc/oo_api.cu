@@ -42,6 +42,13 @@ struct oo_ctx {
     void* d_image = nullptr;
     void* d_image_tc = nullptr;
 
+    // disparity predictor g_psi (f3)
+    bool have_disp = false;
+    GridParams G{};
+    MlpParams MD{};
+    void* d_grid = nullptr;
+    void* d_disp_image = nullptr;
+
     // scene (f5)
     bool have_scene = false;
     void* d_spheres = nullptr;
@@ -210,6 +217,8 @@ extern "C" OO_API void oo_destroy(oo_ctx* c) {
         free_dev(c->d_image);
         free_dev(c->d_image_tc);
         free_dev(c->d_spheres);
+        free_dev(c->d_grid);
+        free_dev(c->d_disp_image);
         free_scratch(c);
         free_pipe(c);
     }
@@ -468,6 +477,28 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
     return OO_OK;
 }
 
+// The decoder weights in the UMMA K-major canonical layout (SWIZZLE_NONE): per layer chunk-major [K/8][N][8] halves; layer 0
+// zero-padded to K1 = in_dim rounded up to 16, the output layer to N = 16 rows.
+static std::vector<uint16_t> make_tc_image(uint32_t in_dim, uint32_t W, uint32_t n_hidden, uint32_t out_dim, const void* const* weights) {
+    const uint32_t k1 = (in_dim + 15) & ~15u;
+    std::vector<uint16_t> tc((size_t)k1 * W + (size_t)(n_hidden - 1) * W * W + (size_t)W * 16, 0);
+    auto put = [&](size_t base, uint32_t N, uint32_t n, uint32_t k, uint16_t v) { tc[base + ((size_t)(k / 8) * N + n) * 8 + (k % 8)] = v; };
+    const uint16_t* w0 = (const uint16_t*)weights[0];
+    for (uint32_t o = 0; o < W; ++o)
+        for (uint32_t i = 0; i < in_dim; ++i) put(0, W, o, i, w0[(size_t)o * in_dim + i]);
+    size_t base = (size_t)k1 * W;
+    for (uint32_t k = 1; k < n_hidden; ++k) {
+        const uint16_t* w = (const uint16_t*)weights[k];
+        for (uint32_t o = 0; o < W; ++o)
+            for (uint32_t i = 0; i < W; ++i) put(base, W, o, i, w[(size_t)o * W + i]);
+        base += (size_t)W * W;
+    }
+    const uint16_t* wl = (const uint16_t*)weights[n_hidden];
+    for (uint32_t o = 0; o < out_dim; ++o)
+        for (uint32_t i = 0; i < W; ++i) put(base, 16, o, i, wl[(size_t)o * W + i]);
+    return tc;
+}
+
 // ---------------------------------------------------------------------------------------------------------------------
 // oo_upload_mlp
 // ---------------------------------------------------------------------------------------------------------------------
@@ -502,23 +533,8 @@ extern "C" OO_API oo_status oo_upload_mlp(oo_ctx* c, const oo_mlp_desc* m, void*
     const uint16_t* wl = (const uint16_t*)m->weights[m->n_hidden];
     for (uint32_t o = 0; W == 64 && o < m->out_dim; ++o)
         for (uint32_t i = 0; i < 64; ++i) img[off + (size_t)o * s1 + i] = wl[(size_t)o * 64 + i];
-    // tensor-core image: chunk-major [K/8][N][8] per layer
-    const size_t tc_halves = (size_t)k1 * W + (size_t)(m->n_hidden - 1) * W * W + (size_t)W * 16;
-    std::vector<uint16_t> tc(tc_halves, 0);
-    {
-        auto put = [&](size_t base, uint32_t N, uint32_t n, uint32_t k, uint16_t v) { tc[base + ((size_t)(k / 8) * N + n) * 8 + (k % 8)] = v; };
-        for (uint32_t o = 0; o < W; ++o)
-            for (uint32_t i = 0; i < m->in_dim; ++i) put(0, W, o, i, w0[(size_t)o * m->in_dim + i]);
-        size_t base = (size_t)k1 * W;
-        for (uint32_t k = 1; k < m->n_hidden; ++k) {
-            const uint16_t* w = (const uint16_t*)m->weights[k];
-            for (uint32_t o = 0; o < W; ++o)
-                for (uint32_t i = 0; i < W; ++i) put(base, W, o, i, w[(size_t)o * W + i]);
-            base += (size_t)W * W;
-        }
-        for (uint32_t o = 0; o < m->out_dim; ++o)
-            for (uint32_t i = 0; i < W; ++i) put(base, 16, o, i, wl[(size_t)o * W + i]);
-    }
+    const std::vector<uint16_t> tc = make_tc_image(m->in_dim, W, m->n_hidden, m->out_dim, m->weights);
+    const size_t tc_halves = tc.size();
     free_dev(c->d_image);
     free_dev(c->d_image_tc);
     c->have_mlp = false;
@@ -537,6 +553,63 @@ extern "C" OO_API oo_status oo_upload_mlp(oo_ctx* c, const oo_mlp_desc* m, void*
     M.width = W;
     c->M = M;
     c->have_mlp = true;
+    return OO_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// oo_upload_disparity
+// ---------------------------------------------------------------------------------------------------------------------
+extern "C" OO_API oo_status oo_upload_disparity(oo_ctx* c, const oo_disparity_desc* d, void* cuda_stream) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (!d || !d->res || !d->tables || !d->weights) return fail(c, OO_ERR_INVALID_ARG, "disparity descriptor or one of its arrays is NULL");
+    if (d->n_levels < 1 || d->n_levels > OO_MAX_GRID_LEVELS) return fail(c, OO_ERR_INVALID_ARG, "n_levels %u outside 1..%d", d->n_levels, OO_MAX_GRID_LEVELS);
+    if (d->n_features != 2) return fail(c, OO_ERR_UNSUPPORTED, "n_features %u: only 2 (one 32-bit entry) is implemented", d->n_features);
+    if (d->hash_log2 < 4 || d->hash_log2 > 28) return fail(c, OO_ERR_INVALID_ARG, "hash_log2 %u outside 4..28", d->hash_log2);
+    if (d->n_hidden < 1 || d->n_hidden > OO_MAX_HIDDEN) return fail(c, OO_ERR_INVALID_ARG, "n_hidden %u outside 1..%d", d->n_hidden, OO_MAX_HIDDEN);
+    const uint64_t t_max = 1ull << d->hash_log2;
+    std::vector<uint64_t> entries(d->n_levels), offset(d->n_levels);
+    uint64_t total = 0;
+    for (uint32_t g = 0; g < d->n_levels; ++g) {
+        const uint64_t N = d->res[g];
+        if (N < 1 || N > (1u << 20)) return fail(c, OO_ERR_INVALID_ARG, "res[%u] = %llu outside 1..2^20", g, (unsigned long long)N);
+        if (!d->tables[g]) return fail(c, OO_ERR_INVALID_ARG, "tables[%u] is NULL", g);
+        const uint64_t dense = (N + 1) * (N + 1) * (N + 1);
+        entries[g] = dense <= t_max ? dense : t_max;
+        offset[g] = total;
+        total += entries[g];
+    }
+    for (uint32_t k = 0; k <= d->n_hidden; ++k)
+        if (!d->weights[k]) return fail(c, OO_ERR_INVALID_ARG, "weights[%u] is NULL", k);
+    const uint32_t in_dim = 2 * d->n_levels + 3;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+    DeviceGuard g(c->device);
+    const std::vector<uint16_t> tc = make_tc_image(in_dim, 64, d->n_hidden, 1, d->weights);
+    free_dev(c->d_grid);
+    free_dev(c->d_disp_image);
+    c->have_disp = false;
+    OO_CUDA(c, cudaMalloc(&c->d_grid, total * 4));
+    OO_CUDA(c, cudaMalloc(&c->d_disp_image, tc.size() * 2));
+    GridParams G{};
+    G.n_levels = d->n_levels;
+    for (uint32_t l = 0; l < d->n_levels; ++l) {
+        OO_CUDA(c, cudaMemcpyAsync((uint32_t*)c->d_grid + offset[l], d->tables[l], entries[l] * 4, cudaMemcpyHostToDevice, stream));
+        GridLevel& lv = G.lv[l];
+        lv.table = (const uint32_t*)c->d_grid + offset[l];
+        lv.scale = (float)d->res[l];
+        lv.n_max = d->res[l] - 1;
+        lv.stride = d->res[l] + 1;
+        lv.mask = entries[l] == t_max && (uint64_t)(d->res[l] + 1) * (d->res[l] + 1) * (d->res[l] + 1) > t_max ? (uint32_t)(t_max - 1) : 0u;
+    }
+    OO_CUDA(c, cudaMemcpyAsync(c->d_disp_image, tc.data(), tc.size() * 2, cudaMemcpyHostToDevice, stream));
+    OO_CUDA(c, cudaStreamSynchronize(stream));
+    MlpParams M{};
+    M.in_dim = in_dim; M.k1 = (in_dim + 15) & ~15u; M.n_hidden = d->n_hidden; M.out_dim = 1; M.out_act = (uint32_t)OO_ACT_EXP;
+    M.image_tc = (const uint16_t*)c->d_disp_image;
+    M.image_tc_bytes = (uint32_t)(tc.size() * 2);
+    M.width = 64;
+    c->G = G;
+    c->MD = M;
+    c->have_disp = true;
     return OO_OK;
 }
 
@@ -624,8 +697,38 @@ static bool needs_full(const oo_ctx* c) {
 static oo_status check_full(oo_ctx* c, const oo_queries* q) {
     if (!c->plan_ok) return fail(c, OO_ERR_UNSUPPORTED, "the full query needs the hop-table descent (used depths at most 3 apart below depth 4)");
     if (c->mode.lookup != OO_LOOKUP_WO && q->n && !q->nrm) return fail(c, OO_ERR_INVALID_ARG, "queries.nrm is NULL (mirror direction)");
-    if (c->mode.lookup == OO_LOOKUP_SHIFTED && q->n && !q->disparity) return fail(c, OO_ERR_INVALID_ARG, "queries.disparity is NULL (OO_LOOKUP_SHIFTED)");
+    if (c->mode.lookup == OO_LOOKUP_SHIFTED && q->n && !q->disparity) {
+        if (!c->have_disp) return fail(c, OO_ERR_INVALID_ARG, "queries.disparity is NULL (OO_LOOKUP_SHIFTED) and no disparity predictor is uploaded");
+        if (q->n > c->reserved) return fail(c, OO_ERR_NOT_READY, "predicting the disparity needs scratch: call oo_reserve(%llu) first", (unsigned long long)q->n);
+    }
     return OO_OK;
+}
+
+// Eq. 7: d^ = g_psi(x, w_r) for every query, into d_out (DEVICE [n]); optionally the hash-grid features.
+static oo_status predict_disparity(oo_ctx* c, const oo_queries* q, float* d_out, float* d_features, cudaStream_t stream) {
+    if (!c->have_disp) return fail(c, OO_ERR_NOT_READY, "no disparity predictor uploaded");
+    if (oo_status st = check_queries(c, q, true)) return st;
+    if (q->n && !d_out) return fail(c, OO_ERR_INVALID_ARG, "disparity output is NULL");
+    if (oo_status st = check_async(c)) return st;
+    if (q->n == 0) return OO_OK;
+    const int n = launch_disparity(c->G, c->MD, make_qp(q), d_out, d_features, c->n_sms, stream);
+    if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "no disparity kernel for this predictor");
+    count(c, n);
+    return check_async(c);
+}
+
+// OO_LOOKUP_SHIFTED without a caller-supplied d^: run the predictor into the context's scratch and point the queries at it.
+static oo_status fill_disparity(oo_ctx* c, oo_queries* q, cudaStream_t stream) {
+    if (c->mode.lookup != OO_LOOKUP_SHIFTED || q->disparity || q->n == 0) return OO_OK;
+    if (oo_status st = predict_disparity(c, q, c->d_qd, nullptr, stream)) return st;
+    q->disparity = c->d_qd;
+    return OO_OK;
+}
+
+extern "C" OO_API oo_status oo_predict_disparity(oo_ctx* c, const oo_queries* q, float* d_disparity, float* d_features, void* cuda_stream) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    DeviceGuard g(c->device);
+    return predict_disparity(c, q, d_disparity, d_features, (cudaStream_t)cuda_stream);
 }
 
 extern "C" OO_API oo_status oo_encode_full(oo_ctx* c, const oo_queries* q, float* d_features, int32_t* d_slot, int16_t* d_cell,
@@ -637,6 +740,9 @@ extern "C" OO_API oo_status oo_encode_full(oo_ctx* c, const oo_queries* q, float
     if (oo_status st = check_async(c)) return st;
     if (q->n == 0) return OO_OK;
     DeviceGuard g(c->device);
+    oo_queries qd = *q;
+    if (oo_status st = fill_disparity(c, &qd, (cudaStream_t)cuda_stream)) return st;
+    q = &qd;
     const int n = launch_encode_full(c->T, make_qp(q), c->mode, d_features, d_slot, d_cell, c->n_sms, (cudaStream_t)cuda_stream);
     if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "no full-query encode kernel for F=%u %s", c->T.F, c->T.f32 ? "fp32" : "fp16");
     count(c, n);
@@ -659,7 +765,9 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
         if (oo_status st = check_async(c)) return st;
         if (q->n == 0) return OO_OK;
         c->M.feat_dim = feat;
-        const QueryParams Q = make_qp(q);
+        oo_queries qd = *q;
+        if (oo_status st = fill_disparity(c, &qd, stream)) return st;
+        const QueryParams Q = make_qp(&qd);
         const int n = c->M.width == 64 ? launch_fused_full_w64(c->T, c->M, Q, c->mode, d_rgb, c->n_sms, stream)
                                        : launch_fused_full_w128(c->T, c->M, Q, c->mode, d_rgb, c->n_sms, stream);
         if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "no full-query kernel for F=%u %s, in_dim %u, out_dim %u", c->T.F, c->T.f32 ? "fp32" : "fp16", c->M.in_dim, c->M.out_dim);

@@ -78,6 +78,19 @@ struct MlpParams {
     uint32_t width;          // 64 or 128; `image` (the mma.sync copy) exists only for 64
 };
 
+// Disparity predictor g_psi (Eq. 7): multi-resolution hash grid over position.  All tables live in one device buffer.
+struct GridLevel {
+    const uint32_t* table;   // [T_g] entries of two fp16 features (one 32-bit word)
+    float scale;             // N_g as fp32
+    uint32_t n_max;          // N_g - 1: the last cell
+    uint32_t stride;         // N_g + 1 vertices per axis (dense levels)
+    uint32_t mask;           // T_max - 1 (hashed levels); 0 = dense
+};
+struct GridParams {
+    GridLevel lv[OO_MAX_GRID_LEVELS];
+    uint32_t n_levels;
+};
+
 struct EncodeOut {
     void* features;          // [n][L*F] tree dtype, or nullptr
     int32_t* slot;           // [n][L] or nullptr
@@ -110,6 +123,9 @@ int launch_fused_full_w64(const TreeParams& T, const MlpParams& M, const QueryPa
                           int n_sms, cudaStream_t stream);
 int launch_fused_full_w128(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const FullModeH& mode, float* rgb,
                            int n_sms, cudaStream_t stream);
+// g_psi: d^ [n] (and optionally the hash-grid features [n][2G] fp32); M is the predictor's own decoder image (out_dim 1)
+int launch_disparity(const GridParams& G, const MlpParams& M, const QueryParams& Q, float* disparity, float* features, int n_sms,
+                     cudaStream_t stream);
 int launch_raycast(const double* d_spheres, uint32_t n_spheres, double lo, double hi, const double eye[3], const double look[3],
                    const double up[3], double vfov_deg, uint32_t width, uint32_t height, float* x, float* nrm, float* wo,
                    int32_t* surf, cudaStream_t stream);
