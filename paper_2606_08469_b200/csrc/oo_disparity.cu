@@ -103,7 +103,7 @@ __global__ void __launch_bounds__(kNWG * 128, 1) disparity_kernel(const __grid_c
     constexpr uint32_t idesc_h = instr_desc(128, 64), idesc_o = instr_desc(128, 16);
     const uint32_t n_lv = G.n_levels;
 
-    for (uint32_t tile = blockIdx.x * kNWG + wg; tile < n_tiles; tile += gridDim.x * kNWG) {
+    for (uint32_t tile = wg * gridDim.x + blockIdx.x; tile < n_tiles; tile += gridDim.x * kNWG) {
         const uint64_t t = (uint64_t)tile * kRows + row;
         const bool valid = t < Q.n;
         const uint64_t qi = valid ? t : Q.n - 1;

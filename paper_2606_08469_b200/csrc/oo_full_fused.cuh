@@ -87,7 +87,7 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
-    uint32_t tile = blockIdx.x * NTEAM + team;
+    uint32_t tile = team * gridDim.x + blockIdx.x;        // the partial last round spreads one tile per SM (see oo_fused_tm.cu)
     if (tile < n_tiles && part == 0) prefetch(tile);
     for (; tile < n_tiles; tile += tile_stride) {
         const bool valid = (uint64_t)tile * 128 + row < Q.n;

@@ -93,7 +93,10 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
 
-    uint32_t tile = blockIdx.x * NWG + wg;
+    // Warpgroup wg of block b takes tiles wg*grid + b, + grid*NWG, ...: the n_tiles mod (grid*NWG) tiles of the last, partial
+    // round then land one per SM (a lone warpgroup finishes its tile about twice as fast as five sharing an SM) instead of five
+    // per SM on a few SMs.  Measured on B200: config 1 61.1 -> 60.1 us, config 3 333.3 -> 329.4 us.
+    uint32_t tile = wg * gridDim.x + blockIdx.x;
     if (tile < n_tiles) prefetch(tile);
     for (; tile < n_tiles; tile += tile_stride) {
         float x[3], w[3];
