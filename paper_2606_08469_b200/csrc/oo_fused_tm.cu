@@ -179,24 +179,23 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             phase ^= 1;
             fence_after_sync();
             // epilogue: my row of D -> ReLU -> fp16 -> my row of the next layer's A (over columns of D already read)
-            uint32_t r[32], p[16];
+            // both halves of D are requested before the single wait::ld, so the second TMEM read hides behind the first
+            uint32_t r0[32], r1[32], p[16];
             if (!odd) {
-                tmem_ld32(tmem_lane, r);
+                tmem_ld32(tmem_lane, r0);
+                tmem_ld32(tmem_lane + 32, r1);
                 tmem_wait_ld();
-                relu_pack32(r, p);
+                relu_pack32(r0, p);
                 tmem_st16(tmem_lane, p);
-                tmem_ld32(tmem_lane + 32, r);
-                tmem_wait_ld();
-                relu_pack32(r, p);
+                relu_pack32(r1, p);
                 tmem_st16(tmem_lane + 16, p);
             } else {
-                tmem_ld32(tmem_lane + 64, r);
+                tmem_ld32(tmem_lane + 64, r0);
+                tmem_ld32(tmem_lane + 32, r1);
                 tmem_wait_ld();
-                relu_pack32(r, p);
+                relu_pack32(r0, p);
                 tmem_st16(tmem_lane + 80, p);
-                tmem_ld32(tmem_lane + 32, r);
-                tmem_wait_ld();
-                relu_pack32(r, p);
+                relu_pack32(r1, p);
                 tmem_st16(tmem_lane + 64, p);
             }
         }
