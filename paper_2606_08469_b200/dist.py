@@ -35,3 +35,29 @@ def reduce_max_sum(values_max, values_sum, device):
         dist.all_reduce(a, op=dist.ReduceOp.MAX)
         dist.all_reduce(b, op=dist.ReduceOp.SUM)
     return a.tolist(), b.tolist()
+
+
+def all_gather_rows(local, n_total: int):
+    """The one optional collective of the path: every rank computed RGB for its shard_range slice of the
+    n_total queries; returns the whole [n_total, C] frame on every rank (NCCL on GPUs: 12 B x N over NVLink; gloo on CPU).
+    `local` is this rank's [hi - lo, C] tensor.  With one rank it is returned as is."""
+    import torch
+    import torch.distributed as dist
+    if not dist.is_initialized() or dist.get_world_size() == 1:
+        assert local.shape[0] == n_total
+        return local
+    world, rank = dist.get_world_size(), dist.get_rank()
+    lo, hi = shard_range(n_total, rank, world)
+    assert local.shape[0] == hi - lo, "local rows %d != this rank's shard %d" % (local.shape[0], hi - lo)
+    # shards differ by at most one row: gather equal-sized padded blocks, then drop the padding
+    m = -(-n_total // world)
+    tail = tuple(local.shape[1:])
+    mine = torch.zeros((m,) + tail, dtype=local.dtype, device=local.device)
+    mine[: hi - lo] = local
+    blocks = torch.empty((world, m) + tail, dtype=local.dtype, device=local.device)
+    dist.all_gather([blocks[r] for r in range(world)], mine)      # equal-sized views of one buffer (works on nccl and gloo)
+    out = torch.empty((n_total,) + tail, dtype=local.dtype, device=local.device)
+    for r in range(world):
+        a, b = shard_range(n_total, r, world)
+        out[a:b] = blocks[r, : b - a]
+    return out

@@ -30,6 +30,11 @@ def test_gloo_world_size_2_reduce(tmp_path):
         lo, hi = D.shard_range(1000001, rank, world)
         (mx,), (tot,) = D.reduce_max_sum([1.0 + rank], [hi - lo], torch.device("cpu"))
         assert mx == 2.0 and tot == 1000001, (mx, tot)
+        # the optional RGB all-gather: ragged shards (7 rows over 2 ranks = 4 + 3) come back in query order on every rank
+        full = torch.arange(21, dtype=torch.float32).reshape(7, 3)
+        a, b = D.shard_range(7, rank, world)
+        got = D.all_gather_rows(full[a:b].clone(), 7)
+        assert torch.equal(got, full), got
         if rank == 0:
             print("OK", mx, tot)
     """ % ROOT))
