@@ -600,6 +600,13 @@ extern "C" OO_API oo_status oo_upload_disparity(oo_ctx* c, const oo_disparity_de
         lv.stride = d->res[l] + 1;
         lv.mask = entries[l] == t_max && (uint64_t)(d->res[l] + 1) * (d->res[l] + 1) * (d->res[l] + 1) > t_max ? (uint32_t)(t_max - 1) : 0u;
     }
+    {
+        uint32_t nd = 0;
+        while (nd < G.n_levels && !G.lv[nd].mask) ++nd;
+        G.n_dense = nd;
+        for (uint32_t l = nd; l < G.n_levels; ++l)
+            if (!G.lv[l].mask) G.n_dense = G.n_levels + 1;
+    }
     OO_CUDA(c, cudaMemcpyAsync(c->d_disp_image, tc.data(), tc.size() * 2, cudaMemcpyHostToDevice, stream));
     OO_CUDA(c, cudaStreamSynchronize(stream));
     MlpParams M{};

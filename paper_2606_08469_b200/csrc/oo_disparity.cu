@@ -11,6 +11,7 @@
 // Gather: per level 8 independent 4-byte loads (one entry = two fp16 features); the tables of the default predictor
 // total 3 MB and stay in L2, so the phase is bound by load issue and latency, not by HBM.
 #include <cstdio>
+#include <type_traits>
 
 #include "oo_device.cuh"
 #include "oo_full.cuh"
@@ -31,6 +32,7 @@ __device__ __forceinline__ void relu_pack32(const uint32_t (&r)[32], uint32_t (&
 
 // One level of the hash grid at position x (already clamped to [0,1]^3).  The cell decision is taken in fp32 exactly as
 // DESIGN.md §14 states it: p = fl(x * N), c0 = min(floor(p), N - 1), t = p - c0 (exact).
+template <bool HASHED>
 __device__ __forceinline__ void grid_level(const GridLevel& lv, const float (&x)[3], float& f0, float& f1) {
     uint32_t c[3];
     float t[3];
@@ -44,7 +46,7 @@ __device__ __forceinline__ void grid_level(const GridLevel& lv, const float (&x)
     uint32_t ix[2], iy[2], iz[2], idx[8];
     ix[0] = c[0];
     ix[1] = c[0] + 1;
-    if (lv.mask) {                 // hashed level: xor of the per-axis products (mod 2^32), reduced to the table
+    if constexpr (HASHED) {        // hashed level: xor of the per-axis products (mod 2^32), reduced to the table
         iy[0] = c[1] * kPrimeY;
         iy[1] = iy[0] + kPrimeY;
         iz[0] = c[2] * kPrimeZ;
@@ -116,14 +118,35 @@ __global__ void __launch_bounds__(kNWG * 128, 1) disparity_kernel(const __grid_c
         mirror_dir(n, wo, wr);
         // ------------------------------------------------------------------ hash-grid features -> A0 (even layer: columns 64..)
         const uint32_t a0 = tmem_lane + 64;
-#pragma unroll 2
-        for (uint32_t g = 0; g < n_lv; ++g) {
-            float f0, f1;
-            grid_level(G.lv[g], x, f0, f1);
-            tmem_st1(a0 + g, pack_half2(f0, f1));
-            if (features && valid) {
-                features[qi * (2 * n_lv) + 2 * g] = f0;
-                features[qi * (2 * n_lv) + 2 * g + 1] = f1;
+        // Levels in batches of 4, 2, 1 within the dense prefix and within the hashed rest: all loads of a batch are issued
+        // before its first TMEM store (whose asm statement orders memory operations and would otherwise serialise the
+        // levels), and a batch has no branch on the level kind.
+        auto batch = [&](auto hashed, auto nb, uint32_t g0) {
+            constexpr uint32_t NB = decltype(nb)::value;
+            float f0[NB], f1[NB];
+#pragma unroll
+            for (uint32_t b = 0; b < NB; ++b) grid_level<decltype(hashed)::value>(G.lv[g0 + b], x, f0[b], f1[b]);
+#pragma unroll
+            for (uint32_t b = 0; b < NB; ++b) {
+                tmem_st1(a0 + g0 + b, pack_half2(f0[b], f1[b]));
+                if (features && valid) {
+                    features[qi * (2 * n_lv) + 2 * (g0 + b)] = f0[b];
+                    features[qi * (2 * n_lv) + 2 * (g0 + b) + 1] = f1[b];
+                }
+            }
+        };
+        auto span = [&](auto hashed, uint32_t g, uint32_t end) {
+            for (; g + 4 <= end; g += 4) batch(hashed, std::integral_constant<uint32_t, 4>{}, g);
+            if (g + 2 <= end) { batch(hashed, std::integral_constant<uint32_t, 2>{}, g); g += 2; }
+            if (g < end) batch(hashed, std::integral_constant<uint32_t, 1>{}, g);
+        };
+        if (G.n_dense <= n_lv) {                      // dense levels first, hashed after (any increasing resolution schedule)
+            span(std::false_type{}, 0u, G.n_dense);
+            span(std::true_type{}, G.n_dense, n_lv);
+        } else {                                      // arbitrary order: one level at a time
+            for (uint32_t g = 0; g < n_lv; ++g) {
+                if (G.lv[g].mask) batch(std::true_type{}, std::integral_constant<uint32_t, 1>{}, g);
+                else batch(std::false_type{}, std::integral_constant<uint32_t, 1>{}, g);
             }
         }
         tmem_st1(a0 + n_lv, pack_half2(wr[0], wr[1]));

@@ -89,6 +89,7 @@ struct GridLevel {
 struct GridParams {
     GridLevel lv[OO_MAX_GRID_LEVELS];
     uint32_t n_levels;
+    uint32_t n_dense;        // dense levels come first and number n_dense; n_levels + 1 if dense and hashed levels interleave
 };
 
 struct EncodeOut {

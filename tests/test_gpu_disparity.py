@@ -72,8 +72,10 @@ def test_default_predictor_random_queries(P):
 
 @pytest.mark.parametrize("kw", [dict(n_levels=1, n_min=8, n_max=8), dict(n_levels=16, n_min=4, n_max=1024, hash_log2=14),
                                 dict(n_levels=4, n_min=2, n_max=16, hash_log2=20), dict(n_levels=4, n_min=64, n_max=512, hash_log2=10),
-                                dict(n_levels=8, n_hidden=1), dict(n_levels=6, n_hidden=3), dict(n_levels=13, n_min=16, n_max=300)],
-                         ids=["one-level", "sixteen-levels", "all-dense", "all-hashed-tiny-table", "one-hidden", "three-hidden", "k1-is-32"])
+                                dict(n_levels=8, n_hidden=1), dict(n_levels=6, n_hidden=3), dict(n_levels=13, n_min=16, n_max=300),
+                                dict(res=[64, 4, 128, 8, 5], hash_log2=12), dict(n_levels=7, n_min=4, n_max=256, hash_log2=12)],
+                         ids=["one-level", "sixteen-levels", "all-dense", "all-hashed-tiny-table", "one-hidden", "three-hidden", "k1-is-32",
+                              "dense-and-hashed-interleaved", "ragged-batches"])
 def test_predictor_shapes(P, kw):
     net = gen.make_disparity_net(2, **kw)
     q = _edge_positions(gen.random_queries(3000, 3))
