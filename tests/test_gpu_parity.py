@@ -57,6 +57,26 @@ def _run_all(P, w, ref_feat, ref_slot, ref_tex, ref_rgb, expect_fast=True):
         assert P.PATH_FUSED_MMA in results and P.PATH_FUSED_TC in results and P.PATH_FUSED_TC_TMEM in results
         # same arithmetic in the same order: the fused and unfused specialised paths agree bit for bit
         assert np.array_equal(results[P.PATH_FUSED_MMA], results[P.PATH_UNFUSED])
+    if ctx.oo_get_info()["hop_plan_ok"] and P.PATH_UNFUSED in results:
+        # OO_LAYOUT_QUAD (pre-expanded four-tap records): same texel values, same arithmetic, same order -> every fast
+        # path reproduces its own padded-layout result bit for bit (and therefore the oracle within the same bars)
+        ctx.oo_set_path(P.PATH_UNFUSED)
+        f_pad = ctx.oo_encode(x, wo)
+        ctx.oo_set_layout("quad")
+        info = ctx.oo_get_info()
+        assert info["layout"] == 1 and info["quad_atlas_bytes"] > info["atlas_bytes"]
+        for path, ref in results.items():
+            if path == P.PATH_GENERIC:
+                continue
+            ctx.oo_set_path(path)
+            assert np.array_equal(ctx.oo_query(x, n, wo, ex).cpu().numpy(), ref), "path %d differs under OO_LAYOUT_QUAD" % path
+        ctx.oo_set_path(P.PATH_UNFUSED)
+        f_quad = ctx.oo_encode(x, wo)
+        assert torch.equal(f_pad, f_quad)
+        check_features(f_quad.float().cpu().numpy(), ref_feat)
+        ctx.oo_set_layout("padded")
+        info = ctx.oo_get_info()
+        assert info["layout"] == 0 and info["quad_atlas_bytes"] == 0
     ctx.oo_set_path(P.PATH_AUTO)
     rgb = ctx.oo_query(x, n, wo, ex).cpu().numpy()
     info = ctx.oo_get_info()
@@ -217,6 +237,56 @@ def test_morton_sort_and_permuted_query(P):
     ctx.oo_reserve(70001)
     perm = ctx.oo_sort_queries(xs).cpu().numpy().astype(np.int64)
     assert np.array_equal(perm, O.morton_order(xs.cpu().numpy()))
+
+
+def test_presort_bin_is_bit_identical(P):
+    """a1': OO_PRESORT_BIN moves the queries into Morton bins inside oo_query; every RGB lands at its query's own index and
+    equals the unsorted call bit for bit (and therefore the oracle within the same bars).  Incoherent surface samples in
+    random order, a ragged size spanning several 4096-key radix tiles, with and without the extra scalar; below the
+    threshold and with a caller-supplied perm the call proceeds unsorted."""
+    for cfg, n in ((2, 40961), (3, 50000)):
+        w = gen.scene_workload(cfg, width=32, height=32, max_depth=8 if cfg == 3 else None, incoherent_n=n, extra_rough=(cfg == 2))
+        q = w.queries
+        ctx = P.OctaOctree(0).upload_workload(w)
+        x, nr, wo, ex = _dev(q)
+        ref = ctx.oo_query(x, nr, wo, ex)
+        assert ctx.oo_get_info()["presorted_last_query"] == 0
+        ctx.oo_set_presort("bin")
+        with pytest.raises(P.OOError) as e:          # the binned copy lives in reserved scratch
+            ctx.oo_query(x, nr, wo, ex)
+        assert e.value.status == 2
+        ctx.oo_reserve(n)
+        for layout in ("padded", "quad"):
+            ctx.oo_set_layout(layout)
+            guard = torch.full((n + 64, 3), -7.0, dtype=torch.float32, device="cuda")
+            ctx.oo_query(x, nr, wo, ex, rgb=guard[:n])
+            assert ctx.oo_get_info()["presorted_last_query"] == 1
+            assert torch.equal(guard[:n], ref) and bool((guard[n:] == -7.0).all())
+        # through the host pipeline (chunks of the frame are binned one by one)
+        h = ctx.oo_query_host(q.x, q.nrm, q.wo, q.extra)
+        assert np.array_equal(np.asarray(h), ref.cpu().numpy())
+        # small batches and caller-ordered batches are not binned
+        m = 4096
+        small = ctx.oo_query(x[:m], nr[:m], wo[:m], None if ex is None else ex[:m])
+        assert ctx.oo_get_info()["presorted_last_query"] == 0 and torch.equal(small, ref[:m])
+        shuf = torch.from_numpy(gen.shuffle_perm(n, 1).astype(np.int32)).cuda()
+        got = ctx.oo_query(x, nr, wo, ex, perm=shuf)
+        assert ctx.oo_get_info()["presorted_last_query"] == 0 and torch.equal(got, ref)
+        # every kernel path runs on the binned copy and reproduces its own unsorted result
+        for path in (P.PATH_GENERIC, P.PATH_UNFUSED, P.PATH_FUSED_MMA, P.PATH_FUSED_TC):
+            ctx.oo_set_path(path)
+            got = ctx.oo_query(x, nr, wo, ex)
+            assert ctx.oo_get_info()["presorted_last_query"] == 1
+            ctx.oo_set_presort("none")
+            assert torch.equal(got, ctx.oo_query(x, nr, wo, ex))
+            ctx.oo_set_presort("bin")
+        ctx.oo_set_path(P.PATH_AUTO)
+        ctx.oo_set_presort("none")
+        ctx.oo_query(x, nr, wo, ex)
+        assert ctx.oo_get_info()["presorted_last_query"] == 0
+        co = OC.from_workload(w)
+        check_rgb(ref.cpu().numpy(), co.query(q.x, q.nrm, q.wo, q.extra))
+        ctx.close()
 
 
 def test_query_host_equals_query(P):
