@@ -161,8 +161,6 @@ def run_ours(args):
     ctx = P.OctaOctree(local_rank).upload_workload(w)
     path = {"auto": P.PATH_AUTO, "mma": P.PATH_FUSED_MMA, "tc": P.PATH_FUSED_TC, "tm": P.PATH_FUSED_TC_TMEM, "unfused": P.PATH_UNFUSED, "generic": P.PATH_GENERIC}[args.path]
     ctx.oo_set_path(path)
-    if args.layout == "quad":
-        ctx.oo_set_layout("quad")
     ctx.oo_set_presort(args.presort)
     ctx.oo_reserve(q.n)
     cu = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
@@ -245,7 +243,7 @@ def run_ours(args):
         "ms_per_step": mx_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16",
         "data": "synthetic",
         "config": dict(desc, l2="flushed between steps (256 MB memset)", path={0: "auto", 1: "generic", 2: "unfused", 3: "fused_mma", 4: "fused_tcgen05", 5: "fused_tcgen05_tmem_a"}[info["path_last_query"]],
-                       ms_per_frame_warm_l2=mx_warm, frames_per_rank=1, layout=args.layout if args.layout == "quad" else "padded", presort=args.presort, parallelism="replicated cache, one frame per GPU, no collective"),
+                       ms_per_frame_warm_l2=mx_warm, frames_per_rank=1, presort=args.presort, parallelism="replicated cache, one frame per GPU, no collective"),
         "clocks": clocks,
         "e2e": {"value": tot_q / (mx_e2e * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": int((36 + 4 * (0 if q.extra is None else q.extra.shape[1])) * q.n),
                 "d2h_bytes_per_step": int(12 * q.n), "ms_per_step": mx_e2e, "api": "oo_query_host (pinned host buffers)", "checksum": checksum},
@@ -338,35 +336,34 @@ def run_sweep(args):
         feat = torch.empty((n_max, L * F), dtype=torch.float16, device=dev)
         rgb = torch.empty((n_max, 3), dtype=torch.float32, device=dev)
         perm = torch.empty(n_max, dtype=torch.int32, device=dev)
-        layouts = ["padded", "quad"] if args.layout == "both" else [args.layout]
-        for layout in layouts:
-            ctx.oo_set_layout(layout)
-            for dname, q in dists.items():
-                X, Nn, W = cu(q.x), cu(q.nrm), cu(q.wo)
-                for lg in range(args.sweep_min_log2, args.sweep_max_log2 + 1):
-                    n = 1 << lg
-                    x, nrm, wo = X[:n], Nn[:n], W[:n]
-                    reps = max(5, min(args.steps, (1 << 26) // n))
-                    t_f = timed(lambda: ctx.oo_query(x, nrm, wo, rgb=rgb[:n]), reps)
-                    t_e = timed(lambda: ctx.oo_encode(x, wo, features=feat[:n]), reps)
-                    row = {"layout": layout, "distribution": dname, "n": n, "fused_ms": t_f, "fused_Mqueries_per_s": n / t_f / 1e3,
-                           "fused_roofline_frac": bq_fused * n / (t_f * 1e-3) / 1e9 / hbm,
-                           "encode_ms": t_e, "encode_Mqueries_per_s": n / t_e / 1e3,
-                           "encode_roofline_frac": bq_enc * n / (t_e * 1e-3) / 1e9 / hbm}
-                    if dname == "incoherent":
-                        # a1: Morton pre-sort inside the timed region, RGB still in the caller's order
-                        t_s = timed(lambda: (ctx.oo_sort_queries(x, perm_out=perm[:n]),
-                                             ctx.oo_query(x, nrm, wo, perm=perm[:n], rgb=rgb[:n])), reps)
-                        row.update({"sort_plus_fused_ms": t_s, "sort_plus_fused_roofline_frac": bq_fused * n / (t_s * 1e-3) / 1e9 / hbm})
-                    # a1': OO_PRESORT_BIN, one radix pass inside oo_query that moves the queries (3 + 1 launches, all timed)
-                    ctx.oo_set_presort("bin")
-                    t_b = timed(lambda: ctx.oo_query(x, nrm, wo, rgb=rgb[:n]), reps)
-                    binned = ctx.oo_get_info()["presorted_last_query"]
-                    ctx.oo_set_presort("none")
-                    row.update({"bin_fused_ms": t_b, "bin_fused_roofline_frac": bq_fused * n / (t_b * 1e-3) / 1e9 / hbm, "binned": binned})
-                    rows.append(row)
+        for dname, q in dists.items():
+            X, Nn, W = cu(q.x), cu(q.nrm), cu(q.wo)
+            for lg in range(args.sweep_min_log2, args.sweep_max_log2 + 1):
+                n = 1 << lg
+                x, nrm, wo = X[:n], Nn[:n], W[:n]
+                reps = max(5, min(args.steps, (1 << 26) // n))
+                t_f = timed(lambda: ctx.oo_query(x, nrm, wo, rgb=rgb[:n]), reps)
+                t_e = timed(lambda: ctx.oo_encode(x, wo, features=feat[:n]), reps)
+                row = {"distribution": dname, "n": n, "fused_ms": t_f, "fused_Mqueries_per_s": n / t_f / 1e3,
+                       "fused_roofline_frac": bq_fused * n / (t_f * 1e-3) / 1e9 / hbm,
+                       "encode_ms": t_e, "encode_Mqueries_per_s": n / t_e / 1e3,
+                       "encode_roofline_frac": bq_enc * n / (t_e * 1e-3) / 1e9 / hbm}
+                if dname == "incoherent":
+                    # a1: Morton pre-sort inside the timed region, RGB still in the caller's order
+                    t_s = timed(lambda: (ctx.oo_sort_queries(x, perm_out=perm[:n]),
+                                         ctx.oo_query(x, nrm, wo, perm=perm[:n], rgb=rgb[:n])), reps)
+                    row.update({"sort_plus_fused_ms": t_s, "sort_plus_fused_roofline_frac": bq_fused * n / (t_s * 1e-3) / 1e9 / hbm})
+                # a1': OO_PRESORT_BIN, one counting pass inside oo_query / oo_encode that moves the queries (all launches timed;
+                # min_queries=1 so that the table shows from which batch size on it pays)
+                ctx.oo_set_presort("bin", min_queries=1)
+                t_b = timed(lambda: ctx.oo_query(x, nrm, wo, rgb=rgb[:n]), reps)
+                t_be = timed(lambda: ctx.oo_encode(x, wo, features=feat[:n]), reps)
+                ctx.oo_set_presort("none")
+                row.update({"bin_fused_ms": t_b, "bin_fused_roofline_frac": bq_fused * n / (t_b * 1e-3) / 1e9 / hbm,
+                            "bin_encode_ms": t_be, "bin_encode_roofline_frac": bq_enc * n / (t_be * 1e-3) / 1e9 / hbm})
+                rows.append(row)
         out = {"sweep": "BASELINE.json configs[4]: batch size x query distribution on the config-3 tree and MLP",
-               "tree_nodes": w.tree.n_nodes, "atlas_bytes": w.atlas.nbytes, "device_bytes": ctx.oo_get_info(), "bytes_per_query": {"fused": bq_fused, "encode": bq_enc},
+               "tree_nodes": w.tree.n_nodes, "atlas_bytes": w.atlas.nbytes, "bytes_per_query": {"fused": bq_fused, "encode": bq_enc},
                "rows": rows}
     out.update({"unit": UNIT, "l2": "flushed between launches (256 MB memset)", "timing": "median of CUDA-event times",
                 "peak_gbs": hbm, "peak_source": which, "data": "synthetic"})
@@ -564,8 +561,6 @@ def main():
     ap.add_argument("--sweep-max-log2", type=int, default=24)
     ap.add_argument("--sweep-min-log2", type=int, default=16)
     ap.add_argument("--sweep-dist", default="both", choices=["both", "coherent", "incoherent"])
-    ap.add_argument("--layout", default="padded", choices=["padded", "quad", "both"],
-                    help="atlas layout for the fast kernels (oo_set_layout); 'both' only with --sweep 4")
     ap.add_argument("--presort", default="none", choices=["none", "bin"], help="oo_set_presort for the headline run")
     ap.add_argument("--quick", action="store_true", help="timed region only (no warm-L2 / e2e / CPU legs): the command ncu wraps")
     args = ap.parse_args()

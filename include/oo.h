@@ -101,26 +101,17 @@ typedef enum {
                                 not selectable with oo_set_path */
 } oo_path;
 
-/* How the library lays the texel atlases out for the fast kernels' four-tap gather (a6; BASELINE.json north_star:
- * "level-major fp16 feature atlas read with coalesced 16-byte vector gathers ... border-texel wrap").
- * OO_LAYOUT_PADDED (default): [slot][R+2][R+2][F], the wrapped one-texel border baked in; the four taps of a base texel
- *   are two pairs of neighbours in two rows.  Neighbouring queries share texels: the layout for coherent (screen-order) frames.
- * OO_LAYOUT_QUAD: in addition, [slot][R+1][R+1][4][F]: every base texel (i0, j0) in [-1, R-1]^2 owns one aligned record
- *   holding its four taps, so a query reads ONE 64- or 128-byte line per level (exactly the algorithmic bytes from DRAM)
- *   instead of two row segments that straddle memory atoms.  About 4 (R+1)^2/(R+2)^2 times the padded atlas in device
- *   memory, on top of it.  The layout for incoherent queries out of an HBM-resident cache (configs[4]).
- * Results are bit-identical between the two: same texel values, same arithmetic, same order. */
-typedef enum { OO_LAYOUT_PADDED = 0, OO_LAYOUT_QUAD = 1 } oo_layout;
-
 /* Row a1 inside oo_query (BASELINE.json north_star: "an optional Morton pre-sort of queries for gather locality").
  * OO_PRESORT_NONE (default): queries are processed in the caller's order (or in queries.perm's).
  * OO_PRESORT_BIN: oo_query first bins the queries by the top 10 bits of their 30-bit Morton key (the octree cell at depth 3
- *   plus one bit: ONE stable radix pass, 3 launches) MOVING x, n, wo and the extras into library scratch, runs the chosen
+ *   plus one bit: ONE counting pass, 3 launches) MOVING x, n, wo and the extras into library scratch, runs the chosen
  *   kernel path over the binned copy, and a last kernel brings the RGB back to the caller's order.  Results are
  *   bit-identical to OO_PRESORT_NONE (queries are independent); what changes is which atlas pages the thread blocks touch
  *   at a time.  For incoherent queries out of an HBM-resident cache (configs[4]); screen-order frames are coherent already.
- *   Takes effect on the hot path (not the full query) when queries.perm is NULL and n >= 32768; otherwise the call
- *   proceeds in the given order (oo_info.presorted_last_query says which).  Needs oo_reserve(n). */
+ *   Takes effect on the hot path (not the full query) when queries.perm is NULL and n >= min_queries of oo_set_presort (default 262144:
+ *   below that the extra launches cost more than they save); otherwise the call proceeds in the given order (oo_info.presorted_last_query says
+ *   which).  oo_encode on OO_PATH_UNFUSED does the same with x and wo and stores every feature row at its query's index
+ *   (oo_info.presorted_last_encode).  Needs oo_reserve(n). */
 typedef enum { OO_PRESORT_NONE = 0, OO_PRESORT_BIN = 1 } oo_presort;
 
 /* The octree and its feature atlases ("every non-empty cell stores a learnable octahedral feature map").
@@ -200,9 +191,8 @@ typedef struct {
     uint32_t path_last_encode;   /* oo_path actually used by the last oo_encode */
     uint32_t hop_plan_ok;        /* 1 if the uploaded tree admits the hop-table descent (else only OO_PATH_GENERIC) */
     uint32_t n_sms;
-    uint64_t quad_atlas_bytes;   /* device bytes of the OO_LAYOUT_QUAD records (0 under OO_LAYOUT_PADDED) */
-    uint32_t layout;             /* oo_layout in force */
     uint32_t presorted_last_query; /* 1 if the last oo_query ran on binned queries (OO_PRESORT_BIN took effect) */
+    uint32_t presorted_last_encode; /* the same for the last oo_encode */
 } oo_info;
 
 /* Create a context on a CUDA device.  Fails with OO_ERR_CUDA if the device is absent or is not compute capability
@@ -225,16 +215,10 @@ OO_API oo_status oo_reserve(oo_ctx* ctx, uint64_t max_queries);
 OO_API oo_status oo_set_path(oo_ctx* ctx, oo_path path);
 OO_API oo_status oo_get_info(const oo_ctx* ctx, oo_info* out);
 
-/* Choose the atlas layout the fast paths (OO_PATH_UNFUSED and the fused paths) gather from; see oo_layout.  Call after
- * oo_upload_tree (a new upload resets the layout to OO_LAYOUT_PADDED).  OO_LAYOUT_QUAD allocates the records and fills them
- * from the library's padded atlas with one kernel per level on `cuda_stream`; queries must be issued on that stream or
- * after it has been synchronised.  OO_LAYOUT_PADDED frees them (synchronises the device first).  OO_PATH_GENERIC and the
- * full-query kernels always read the padded atlas.  Errors: OO_ERR_NOT_READY (no tree), OO_ERR_UNSUPPORTED (vertex maps),
- * OO_ERR_OOM (the records do not fit; the layout is left unchanged), OO_ERR_INVALID_ARG. */
-OO_API oo_status oo_set_layout(oo_ctx* ctx, oo_layout layout, void* cuda_stream);
-
-/* Switch the in-query pre-sort on or off; see oo_presort.  OO_ERR_INVALID_ARG for an unknown value. */
-OO_API oo_status oo_set_presort(oo_ctx* ctx, oo_presort presort);
+/* Switch the in-query pre-sort on or off; see oo_presort.  Batches of fewer than min_queries queries proceed unsorted;
+ * 0 selects the library default (262144, about where binning starts to pay on a B200).  OO_ERR_INVALID_ARG for an unknown
+ * presort value. */
+OO_API oo_status oo_set_presort(oo_ctx* ctx, oo_presort presort, uint64_t min_queries);
 /* Select the variant of the query (default all-zero = the hot path).  Takes effect from the next oo_encode_full /
  * oo_query.  OO_LOOKUP_SHIFTED needs oo_queries.disparity; OO_ATTRS_PAPER changes the expected MLP in_dim. */
 OO_API oo_status oo_set_mode(oo_ctx* ctx, const oo_mode* mode);

@@ -13,14 +13,13 @@ SPATIAL = {"nearest": 0, "trilinear8": 1}
 DIRMAP = {"texel": 0, "vertex": 1}
 LOOKUP = {"wo": 0, "mirror": 1, "shifted": 2}
 ATTRS = {"n_wo": 0, "paper": 1}
-LAYOUT = {"padded": 0, "quad": 1}
 OO_F16, OO_F32 = 0, 1
 OO_ACT_NONE, OO_ACT_EXP = 0, 1
 _STATUS = {0: "OO_OK", 1: "OO_ERR_INVALID_ARG", 2: "OO_ERR_NOT_READY", 3: "OO_ERR_UNSUPPORTED", 4: "OO_ERR_CUDA", 5: "OO_ERR_OOM"}
 
 EXPORTED_SYMBOLS = ["oo_create", "oo_destroy", "oo_last_error", "oo_upload_tree", "oo_upload_mlp", "oo_reserve", "oo_set_path",
                     "oo_get_info", "oo_sort_queries", "oo_encode", "oo_query", "oo_query_host", "oo_read_padded_map", "oo_set_mode",
-                    "oo_encode_full", "oo_upload_scene", "oo_raycast", "oo_upload_disparity", "oo_predict_disparity", "oo_set_layout", "oo_set_presort"]
+                    "oo_encode_full", "oo_upload_scene", "oo_raycast", "oo_upload_disparity", "oo_predict_disparity", "oo_set_presort"]
 
 
 class OOError(RuntimeError):
@@ -67,8 +66,8 @@ class _Mode(C.Structure):
 class _Info(C.Structure):
     _fields_ = [("launches", C.c_uint64), ("query_launches", C.c_uint64), ("node_table_bytes", C.c_uint64),
                 ("atlas_bytes", C.c_uint64), ("path_last_query", C.c_uint32), ("path_last_encode", C.c_uint32),
-                ("hop_plan_ok", C.c_uint32), ("n_sms", C.c_uint32), ("quad_atlas_bytes", C.c_uint64),
-                ("layout", C.c_uint32), ("presorted_last_query", C.c_uint32)]
+                ("hop_plan_ok", C.c_uint32), ("n_sms", C.c_uint32),
+                ("presorted_last_query", C.c_uint32), ("presorted_last_encode", C.c_uint32)]
 
 
 _lib = None
@@ -97,8 +96,7 @@ def load_library():
     L.oo_reserve.argtypes = [vp, u64]
     L.oo_set_path.argtypes = [vp, C.c_int]
     L.oo_get_info.argtypes = [vp, C.POINTER(_Info)]
-    L.oo_set_layout.argtypes = [vp, C.c_int, vp]
-    L.oo_set_presort.argtypes = [vp, C.c_int]
+    L.oo_set_presort.argtypes = [vp, C.c_int, u64]
     L.oo_sort_queries.argtypes = [vp, C.POINTER(_Queries), vp, vp]
     L.oo_encode.argtypes = [vp, C.POINTER(_Queries), vp, vp, vp, vp]
     L.oo_query.argtypes = [vp, C.POINTER(_Queries), vp, vp]
@@ -221,13 +219,10 @@ class OctaOctree:
     def oo_set_path(self, path: int):
         self._check(self._L.oo_set_path(self._ctx, int(path)))
 
-    def oo_set_layout(self, layout: str = "padded"):
-        """"padded" (default) or "quad" (pre-expanded four-tap records; see oo_layout in include/oo.h)."""
-        self._check(self._L.oo_set_layout(self._ctx, LAYOUT[layout], self._stream()))
-
-    def oo_set_presort(self, presort: str = "none"):
-        """"none" (default) or "bin" (oo_query bins the queries by their top Morton bits first; see oo_presort)."""
-        self._check(self._L.oo_set_presort(self._ctx, {"none": 0, "bin": 1}[presort]))
+    def oo_set_presort(self, presort: str = "none", min_queries: int = 0):
+        """"none" (default) or "bin" (oo_query / oo_encode bin the queries by their top Morton bits first; see oo_presort).
+        Batches below min_queries proceed unsorted (0 = library default)."""
+        self._check(self._L.oo_set_presort(self._ctx, {"none": 0, "bin": 1}[presort], int(min_queries)))
 
     def oo_set_mode(self, spatial: str = "nearest", lookup: str = "wo", attrs: str = "n_wo"):
         m = _Mode(SPATIAL[spatial], LOOKUP[lookup], ATTRS[attrs])

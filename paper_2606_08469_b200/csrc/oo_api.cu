@@ -30,8 +30,6 @@ struct oo_ctx {
     uint32_t tree_max_depth = 0;
     TreeParams T{};
     std::vector<void*> atlas_dev;          // library-owned padded atlases (unshifted base pointers)
-    std::vector<void*> quad_dev;           // OO_LAYOUT_QUAD: pre-expanded four-tap records (empty when the layout is PADDED)
-    oo_layout layout = OO_LAYOUT_PADDED;
     std::vector<uint64_t> level_slots;
     void* d_dense = nullptr;
     std::vector<void*> d_hop;
@@ -64,8 +62,9 @@ struct oo_ctx {
     float *d_qx = nullptr, *d_qn = nullptr, *d_qw = nullptr, *d_qe = nullptr, *d_rgb = nullptr, *d_qd = nullptr;
     // OO_PRESORT_BIN: the binned copy of the queries and their original indices (allocated on first use, `reserved` rows)
     oo_presort presort = OO_PRESORT_NONE;
+    uint64_t bin_min = 1u << 18;           // batches below this proceed unsorted (the extra launches cost more than they save)
     float *d_bx = nullptr, *d_bn = nullptr, *d_bw = nullptr, *d_be = nullptr;
-    uint32_t* d_binv = nullptr;
+    uint32_t *d_binv = nullptr, *d_bidx = nullptr;
     float* d_brgb = nullptr;
     uint64_t bin_rows = 0;
 
@@ -118,11 +117,6 @@ void free_dev(void*& p) {
 void free_tree(oo_ctx* c) {
     for (void*& p : c->atlas_dev) free_dev(p);
     c->atlas_dev.clear();
-    for (void*& p : c->quad_dev) free_dev(p);
-    c->quad_dev.clear();
-    c->layout = OO_LAYOUT_PADDED;
-    c->info.quad_atlas_bytes = 0;
-    c->info.layout = (uint32_t)OO_LAYOUT_PADDED;
     for (void*& p : c->d_hop) free_dev(p);
     c->d_hop.clear();
     free_dev(c->d_dense);
@@ -139,7 +133,7 @@ void free_scratch(oo_ctx* c) {
     void** ps[] = {(void**)&c->d_keys_a, (void**)&c->d_keys_b, (void**)&c->d_idx_a, (void**)&c->d_hist, (void**)&c->d_qx,
                    (void**)&c->d_qn,     (void**)&c->d_qw,     (void**)&c->d_qe,    (void**)&c->d_rgb, (void**)&c->d_qd};
     for (void** p : ps) free_dev(*p);
-    void** bs[] = {(void**)&c->d_bx, (void**)&c->d_bn, (void**)&c->d_bw, (void**)&c->d_be, (void**)&c->d_binv, (void**)&c->d_brgb};
+    void** bs[] = {(void**)&c->d_bx, (void**)&c->d_bn, (void**)&c->d_bw, (void**)&c->d_be, (void**)&c->d_binv, (void**)&c->d_bidx, (void**)&c->d_brgb};
     for (void** p : bs) free_dev(*p);
     c->bin_rows = 0;
     c->reserved = 0;
@@ -249,68 +243,11 @@ extern "C" OO_API oo_status oo_set_path(oo_ctx* c, oo_path path) {
     c->path = path;
     return OO_OK;
 }
-
-// The padded view of level l as the fast kernels' gather view.
-static void padded_view(LevelParams& lv, uint32_t texel_bytes) {
-    lv.fatlas = lv.atlas; lv.f_map_bytes = lv.map_bytes;
-    lv.f_is = texel_bytes; lv.f_js = lv.row_bytes; lv.f_pair = lv.row_bytes;
-}
-
-extern "C" OO_API oo_status oo_set_layout(oo_ctx* c, oo_layout layout, void* cuda_stream) {
-    if (!c) return OO_ERR_INVALID_ARG;
-    if (layout != OO_LAYOUT_PADDED && layout != OO_LAYOUT_QUAD) return fail(c, OO_ERR_INVALID_ARG, "unknown layout %d", (int)layout);
-    if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "oo_set_layout: no tree uploaded (the layout is a property of the uploaded atlas)");
-    if (c->T.vertex && layout == OO_LAYOUT_QUAD) return fail(c, OO_ERR_UNSUPPORTED, "OO_LAYOUT_QUAD applies to texel maps (OO_DIRMAP_TEXEL)");
-    DeviceGuard g(c->device);
-    cudaStream_t stream = (cudaStream_t)cuda_stream;
-    if (oo_status st = check_async(c)) return st;
-    if (layout == c->layout) return OO_OK;
-    const uint32_t L = c->T.n_levels, TB = c->T.texel_bytes;
-    if (layout == OO_LAYOUT_PADDED) {
-        // kernels already queued on any stream may still read the records
-        OO_CUDA(c, cudaDeviceSynchronize());
-        for (void*& p : c->quad_dev) free_dev(p);
-        c->quad_dev.clear();
-        for (uint32_t l = 0; l < L; ++l) padded_view(c->T.lv[l], TB);
-        c->info.quad_atlas_bytes = 0;
-    } else {
-        std::vector<void*> quad(L, nullptr);
-        uint64_t total = 0;
-        int launches = 0;
-        for (uint32_t l = 0; l < L; ++l) {
-            const uint32_t R = c->T.lv[l].R;
-            const uint64_t slots = std::max<uint64_t>(c->level_slots[l], 1);
-            const uint64_t bytes = slots * (uint64_t)(R + 1) * (R + 1) * 4 * TB;
-            const cudaError_t e = cudaMalloc(&quad[l], bytes);
-            if (e != cudaSuccess) {
-                for (void*& p : quad) free_dev(p);
-                cudaGetLastError();
-                return fail(c, OO_ERR_OOM, "oo_set_layout: %llu bytes for the level-%u records: %s", (unsigned long long)bytes, l, cudaGetErrorString(e));
-            }
-            total += bytes;
-            launches += launch_expand_quad(c->atlas_dev[l], quad[l], slots, R, TB, stream);
-        }
-        OO_CUDA(c, cudaGetLastError());
-        c->quad_dev = quad;
-        for (uint32_t l = 0; l < L; ++l) {
-            LevelParams& lv = c->T.lv[l];
-            const uint32_t Rq = lv.R + 1;
-            lv.f_is = 4 * TB; lv.f_js = Rq * 4 * TB; lv.f_pair = 2 * TB;
-            lv.f_map_bytes = Rq * Rq * 4 * TB;
-            lv.fatlas = (const uint8_t*)quad[l] + lv.f_js + lv.f_is;     // (i0, j0) = (-1, -1) is record (0, 0)
-        }
-        c->info.quad_atlas_bytes = total;
-        c->info.launches += (uint64_t)launches;
-    }
-    c->layout = layout;
-    c->info.layout = (uint32_t)layout;
-    return OO_OK;
-}
-
-extern "C" OO_API oo_status oo_set_presort(oo_ctx* c, oo_presort presort) {
+extern "C" OO_API oo_status oo_set_presort(oo_ctx* c, oo_presort presort, uint64_t min_queries) {
     if (!c) return OO_ERR_INVALID_ARG;
     if (presort != OO_PRESORT_NONE && presort != OO_PRESORT_BIN) return fail(c, OO_ERR_INVALID_ARG, "unknown presort %d", (int)presort);
     c->presort = presort;
+    c->bin_min = min_queries ? min_queries : (1u << 18);
     return OO_OK;
 }
 
@@ -431,7 +368,6 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
         lv.R = R; lv.Rp = Rp;
         lv.map_bytes = Rp * Rp * texel_bytes;
         lv.row_bytes = Rp * texel_bytes;
-        padded_view(lv, texel_bytes);
         lv.depth = t->level_depth[l];
         lv.shift = T.depth_eff - lv.depth;
     }
@@ -732,6 +668,25 @@ static oo_status ensure_feat(oo_ctx* c, uint64_t bytes) {
     return OO_OK;
 }
 
+// OO_PRESORT_BIN scratch: the binned copy of the queries, both index maps and the binned RGB (`reserved` rows)
+static oo_status ensure_bin(oo_ctx* c, uint64_t n) {
+    if (n > c->reserved) return fail(c, OO_ERR_NOT_READY, "OO_PRESORT_BIN: call oo_reserve(%llu) first", (unsigned long long)n);
+    if (c->bin_rows >= n) return OO_OK;
+    void** bs[] = {(void**)&c->d_bx, (void**)&c->d_bn, (void**)&c->d_bw, (void**)&c->d_be, (void**)&c->d_binv, (void**)&c->d_bidx, (void**)&c->d_brgb};
+    for (void** b : bs) free_dev(*b);
+    c->bin_rows = 0;
+    const uint64_t rows = c->reserved;
+    OO_CUDA(c, cudaMalloc((void**)&c->d_bx, rows * 12));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_bn, rows * 12));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_bw, rows * 12));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_be, rows * 4 * OO_MAX_EXTRA));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_binv, rows * 4));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_bidx, rows * 4));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_brgb, rows * 4 * 8));
+    c->bin_rows = rows;
+    return OO_OK;
+}
+
 // ---------------------------------------------------------------------------------------------------------------------
 // oo_sort_queries
 // ---------------------------------------------------------------------------------------------------------------------
@@ -769,6 +724,15 @@ extern "C" OO_API oo_status oo_encode(oo_ctx* c, const oo_queries* q, void* d_fe
     if ((int)p < 0) return fail(c, OO_ERR_UNSUPPORTED, "no specialised kernel for L=%u F=%u (or the tree has no hop plan); use OO_PATH_GENERIC/AUTO", c->T.n_levels, c->T.F);
     QueryParams Q = make_qp(q);
     EncodeOut O{d_features, d_slot, d_texel};
+    c->info.presorted_last_encode = 0;
+    if (c->presort == OO_PRESORT_BIN && p == OO_PATH_UNFUSED && !q->perm && q->n >= c->bin_min) {
+        // a1': x and wo move into Morton bins; the encode kernel reads them in order and stores every row at its query's index
+        if (oo_status st = ensure_bin(c, q->n)) return st;
+        Q.nrm = nullptr; Q.extra = nullptr; Q.n_extra = 0;
+        count(c, launch_bin_queries(Q, c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, c->d_bidx, (cudaStream_t)cuda_stream));
+        Q.x = c->d_bx; Q.wo = c->d_bw; Q.out_idx = c->d_bidx;
+        c->info.presorted_last_encode = 1;
+    }
     int n = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Q, O, c->tree_max_depth, (cudaStream_t)cuda_stream)
                                  : launch_encode_fast(c->T, Q, O, c->n_sms, (cudaStream_t)cuda_stream);
     if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "encode kernel missing");
@@ -838,9 +802,6 @@ extern "C" OO_API oo_status oo_encode_full(oo_ctx* c, const oo_queries* q, float
     return check_async(c);
 }
 
-// OO_PRESORT_BIN pays from about this many queries on (below it the three extra launches cost more than they save)
-static constexpr uint64_t kBinMinQueries = 1u << 15;
-
 static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cudaStream_t stream) {
     if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "no tree uploaded");
     if (!c->have_mlp) return fail(c, OO_ERR_NOT_READY, "no MLP uploaded");
@@ -880,24 +841,11 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
     int n = 0;
     float* const d_out = d_rgb;
     c->info.presorted_last_query = 0;
-    if (c->presort == OO_PRESORT_BIN && !q->perm && q->n >= kBinMinQueries) {
+    if (c->presort == OO_PRESORT_BIN && !q->perm && q->n >= c->bin_min) {
         // a1': one radix pass on the top Morton bits moves the queries into the binned scratch; whichever kernel path was
         // chosen then runs over the binned copy into binned RGB, and unbin_kernel restores the caller's order
-        if (q->n > c->reserved) return fail(c, OO_ERR_NOT_READY, "OO_PRESORT_BIN: call oo_reserve(%llu) first", (unsigned long long)q->n);
-        if (c->bin_rows < q->n) {
-            void** bs[] = {(void**)&c->d_bx, (void**)&c->d_bn, (void**)&c->d_bw, (void**)&c->d_be, (void**)&c->d_binv, (void**)&c->d_brgb};
-            for (void** b : bs) free_dev(*b);
-            c->bin_rows = 0;
-            const uint64_t rows = c->reserved;
-            OO_CUDA(c, cudaMalloc((void**)&c->d_bx, rows * 12));
-            OO_CUDA(c, cudaMalloc((void**)&c->d_bn, rows * 12));
-            OO_CUDA(c, cudaMalloc((void**)&c->d_bw, rows * 12));
-            OO_CUDA(c, cudaMalloc((void**)&c->d_be, rows * 4 * OO_MAX_EXTRA));
-            OO_CUDA(c, cudaMalloc((void**)&c->d_binv, rows * 4));
-            OO_CUDA(c, cudaMalloc((void**)&c->d_brgb, rows * 4 * 8));
-            c->bin_rows = rows;
-        }
-        count(c, launch_bin_queries(Q, c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, stream));
+        if (oo_status st = ensure_bin(c, q->n)) return st;
+        count(c, launch_bin_queries(Q, c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, nullptr, stream));
         Q.x = c->d_bx; Q.nrm = c->d_bn; Q.wo = c->d_bw; Q.extra = q->n_extra ? c->d_be : nullptr;
         d_rgb = c->d_brgb;
         c->info.presorted_last_query = 1;

@@ -29,14 +29,7 @@ struct LevelParams {
     uint32_t dense;         // 1: slot = dense table lookup (depth <= 4); 0: hop from the previous station
     uint32_t dense_off;     // offset (ints) of this level's dense table inside the dense block
     uint32_t gap;           // depth - previous station depth (1..3) when !dense
-    // The view the fast kernels gather through (gather_level / gather_levels): tap (i0, j0) starts at
-    //   fatlas + slot*f_map_bytes + j0*f_js + i0*f_is   and its four texels sit at  +0, +TB, +f_pair, +f_pair+TB.
-    // OO_LAYOUT_PADDED: the padded atlas itself (f_is = TB, f_js = f_pair = row_bytes).  OO_LAYOUT_QUAD: a second,
-    // pre-expanded atlas [slot][R+1][R+1][4 taps][F] in which every base texel owns an aligned 4*TB-byte record
-    // (f_is = 4*TB, f_js = (R+1)*4*TB, f_pair = 2*TB): one 64/128-byte line per level and query instead of two rows.
-    uint32_t f_map_bytes;
-    const uint8_t* fatlas;
-    uint32_t f_is, f_js, f_pair, pad_;
+    uint32_t pad_;
 };
 
 struct TreeParams {
@@ -66,6 +59,7 @@ struct QueryParams {
     uint32_t n_extra;
     const uint32_t* perm;
     const float* disparity;  // [n] or nullptr (OO_LOOKUP_SHIFTED)
+    const uint32_t* out_idx; // encode_fast_kernel only (OO_PRESORT_BIN): thread t reads query t and stores its rows at out_idx[t]
 };
 
 // Decoder image: the padded, shared-memory-ready copy of the weights (built by oo_upload_mlp).
@@ -109,7 +103,6 @@ struct EncodeOut {
 // Launchers (oo_kernels.cu / oo_sort.cu).  Each returns the number of kernels it launched, or -1 if the requested
 // specialisation does not exist.  All launches go to `stream`.
 int launch_pad_atlas(const void* src, void* dst, uint64_t slots, uint32_t R, uint32_t texel_bytes, cudaStream_t stream);
-int launch_expand_quad(const void* padded, void* quad, uint64_t slots, uint32_t R, uint32_t texel_bytes, cudaStream_t stream);
 int launch_encode_generic(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, uint32_t tree_max_depth,
                           cudaStream_t stream);
 int launch_encode_fast(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, int n_sms, cudaStream_t stream);
@@ -142,7 +135,7 @@ int launch_morton_sort(const float* x, uint64_t n, uint32_t* keys_a, uint32_t* k
                        uint32_t* hist, cudaStream_t stream);
 size_t morton_sort_hist_ints(uint64_t n);
 int launch_bin_queries(const QueryParams& Q, uint32_t* keys, uint32_t* hist, float* sx, float* sn, float* sw, float* se,
-                       uint32_t* inv, cudaStream_t stream);
+                       uint32_t* inv, uint32_t* idx, cudaStream_t stream);
 int launch_unbin(const float* binned, const uint32_t* inv, uint64_t n, uint32_t out_dim, float* out, int n_sms, cudaStream_t stream);
 
 }  // namespace oo

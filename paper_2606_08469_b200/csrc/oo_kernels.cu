@@ -38,38 +38,6 @@ int launch_pad_atlas(const void* src, void* dst, uint64_t slots, uint32_t R, uin
 }
 
 // =====================================================================================================================
-// OO_LAYOUT_QUAD: expand the padded atlas [slot][R+2][R+2][TB] into [slot][R+1][R+1][4][TB], record (j, i) holding the
-// four taps of base texel (i0, j0) = (i-1, j-1) in the order (i0,j0), (i0+1,j0), (i0,j0+1), (i0+1,j0+1): the bilinear
-// footprint of a6 becomes one aligned 4*TB-byte record.  One thread per 16-byte vector of the destination.
-// =====================================================================================================================
-__global__ void expand_quad_kernel(const uint4* __restrict__ src, uint4* __restrict__ dst, uint64_t slots, uint32_t R,
-                                   uint32_t vec_per_texel) {
-    const uint32_t Rp = R + 2, Rq = R + 1;
-    const uint64_t per_map = (uint64_t)Rq * Rq * 4 * vec_per_texel;
-    const uint64_t total = slots * per_map;
-    for (uint64_t t = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; t < total; t += (uint64_t)gridDim.x * blockDim.x) {
-        const uint64_t slot = t / per_map;
-        uint32_t r = (uint32_t)(t - slot * per_map);
-        const uint32_t v = r % vec_per_texel;
-        r /= vec_per_texel;
-        const uint32_t tap = r & 3u;
-        r >>= 2;
-        const uint32_t i = r % Rq + (tap & 1u), j = r / Rq + (tap >> 1);
-        dst[t] = src[((slot * Rp + j) * Rp + i) * vec_per_texel + v];
-    }
-}
-
-int launch_expand_quad(const void* padded, void* quad, uint64_t slots, uint32_t R, uint32_t texel_bytes, cudaStream_t stream) {
-    if (slots == 0) return 0;
-    const uint32_t vpt = texel_bytes / 16;
-    const uint64_t total = slots * (uint64_t)(R + 1) * (R + 1) * 4 * vpt;
-    const uint64_t blocks = (total + 255) / 256;
-    const unsigned grid = (unsigned)(blocks < 148ull * 32 ? blocks : 148ull * 32);
-    expand_quad_kernel<<<grid, 256, 0, stream>>>((const uint4*)padded, (uint4*)quad, slots, R, vpt);
-    return 1;
-}
-
-// =====================================================================================================================
 // Generic encode: any tree, any (F, dtype) with 16/32/64-byte texels.  Plain child-table descent per level.
 // One thread per query.  Slow by design; it is the fallback and a cross-check of the specialised kernels.
 // =====================================================================================================================
@@ -151,6 +119,7 @@ __global__ void __launch_bounds__(256) encode_fast_kernel(const __grid_constant_
     constexpr int TB = F * (F32 ? 4 : 2);
     for (uint64_t t = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; t < Q.n; t += (uint64_t)gridDim.x * blockDim.x) {
         const uint64_t qi = Q.perm ? Q.perm[t] : t;
+        const uint64_t oi = Q.out_idx ? Q.out_idx[t] : qi;      // where this query's rows go (binned queries: its own index)
         float x[3], w[3];
         load3(Q.x, qi, x);
         load3(Q.wo, qi, w);
@@ -160,15 +129,15 @@ __global__ void __launch_bounds__(256) encode_fast_kernel(const __grid_constant_
         for (int l = 0; l < L; ++l) {
             const LevelParams& lv = T.lv[l];
             const Tap tp = level_tap(e.uv, lv.half_r, lv.off);
-            if (O.slot) O.slot[qi * L + l] = e.slot[l];
+            if (O.slot) O.slot[oi * L + l] = e.slot[l];
             if (O.texel) {
-                O.texel[(qi * L + l) * 2] = (int16_t)tp.i0;
-                O.texel[(qi * L + l) * 2 + 1] = (int16_t)tp.j0;
+                O.texel[(oi * L + l) * 2] = (int16_t)tp.i0;
+                O.texel[(oi * L + l) * 2 + 1] = (int16_t)tp.j0;
             }
             if (O.features) {
                 float h[F];
                 gather_level<F, F32>(lv, e.slot[l], tp, h);
-                uint8_t* dst = (uint8_t*)O.features + (qi * L + l) * TB;
+                uint8_t* dst = (uint8_t*)O.features + (oi * L + l) * TB;
                 if constexpr (F32) {
 #pragma unroll
                     for (int v = 0; v < F / 4; ++v)

@@ -7,6 +7,7 @@
 // them 32 at a time with __match_any_sync against warp-private digit counters in shared memory.  Ties keep the original
 // order, so the permutation is unique.  9 launches.
 #include "oo_device.cuh"
+#include "oo_tc_ptx.cuh"
 
 namespace oo {
 
@@ -198,71 +199,91 @@ int launch_morton_sort(const float* x, uint64_t n, uint32_t* keys_a, uint32_t* k
 }
 
 // =====================================================================================================================
-// OO_PRESORT_BIN (a1'): ONE stable radix pass on the top kBits bits of the Morton key (the cell at depth 3 plus one bit)
-// that moves the QUERIES, not (key, index) pairs.  Same per-tile histogram and scan as above; the scatter below ranks
-// its tile exactly like radix_scatter_kernel, then sorts the tile locally in shared memory so that global writes are runs
-// (all queries of one digit in a tile are consecutive in the output): x, n and wo are staged through a 48 KB buffer, one
-// array at a time, read back in sorted order and written with consecutive threads on consecutive floats.  A direct
-// scatter of 4-byte stores to 1024 open buckets made DRAM read-modify-write partial sectors (measured on B200, 2^22
-// incoherent queries: 313 MB read + 263 MB written, 387 us; this version moves the algorithmic ~320 MB).
+// OO_PRESORT_BIN (a1'): ONE counting pass on the top kBits bits of the Morton key (the cell at depth 3 plus one bit) that
+// moves the QUERIES, not (key, index) pairs.  Same per-tile histogram and scan as above.  The scatter below gives every
+// query of its tile a rank inside its digit with a shared-memory atomic (the order inside a bin is whatever the atomics
+// return: nothing downstream depends on it, every query is evaluated on its own and inv brings its RGB home), turns the
+// ranks into a tile-local sorted order, and copies x, n and wo out of shared memory in that order, consecutive threads on
+// consecutive floats, so that global writes are whole runs (all queries of one digit in a tile are consecutive in the
+// output).  The tile's three arrays (3 x 48 KB) arrive by three bulk asynchronous copies issued before the ranking starts.
+// A direct scatter of 4-byte stores to 1024 open buckets made DRAM read-modify-write partial sectors (measured on B200,
+// 2^22 incoherent queries: 313 MB read + 263 MB written, 387 us); staging one array at a time through registers 140 us.
 // inv[i] = position of query i in the binned arrays (written in query order, coalesced): unbin_kernel uses it to bring the
 // RGB back to the caller's order with coalesced stores.
 // =====================================================================================================================
 struct BinPayload {
-    const float *x, *nrm, *wo, *extra;
+    const float *x, *nrm, *wo, *extra;   // nrm may be nullptr (oo_encode): that array is then skipped
     uint32_t n_extra;
     float *sx, *sn, *sw, *se;
+    uint32_t* idx;                       // optional: idx[binned position] = query index (oo_encode stores rows at it)
 };
-constexpr uint32_t kBinSmemBytes = (kSortThreads / 32) * kDigits * 4 + kTile * 4 + kTile * 2 + kDigits * 4 + kTile * 3 * 4 + 64;
+constexpr int kBinThreads = 512;
+constexpr int kBinItems = kTile / kBinThreads;      // 8 queries per thread
+constexpr int kBinDPT = kDigits / kBinThreads;      // 2 digits per thread in the scan
+constexpr uint32_t kBinSmemBytes = kTile * 9 * 4 + kTile * 4 + kTile * 2 + kDigits * 4 * 2 + (kBinThreads / 32) * 4 + 16;
 
-__global__ void __launch_bounds__(kSortThreads) bin_scatter_kernel(const uint32_t* __restrict__ keys_in, uint64_t n, uint32_t shift,
-                                                                   uint32_t n_tiles, const uint32_t* __restrict__ offsets,
-                                                                   const BinPayload B, uint32_t* __restrict__ inv) {
-    extern __shared__ __align__(16) uint32_t sm[];
-    uint32_t(*pos)[kDigits] = (uint32_t(*)[kDigits])sm;              // [8][1024] per-warp digit counters, then start positions
-    uint32_t* s_src = sm + (kSortThreads / 32) * kDigits;            // [4096] tile-local source index at each sorted position
-    uint32_t* s_delta = s_src + kTile;                               // [1024] global position - tile-local sorted position
-    float* s_pay = (float*)(s_delta + kDigits);                      // [4096*3] one staged array
-    uint16_t* s_dig = (uint16_t*)(s_pay + kTile * 3);                // [4096] digit at each sorted position
-    uint32_t* s_warp = (uint32_t*)(s_dig + kTile);                   // [8] warp totals of the digit scan
-    const uint32_t warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    for (int w = 0; w < kSortThreads / 32; ++w)
-#pragma unroll
-        for (int k = 0; k < kDPT; ++k) pos[w][threadIdx.x + k * kSortThreads] = 0;
-    __syncthreads();
+__device__ __forceinline__ void bulk_g2s(uint32_t saddr, const void* gptr, uint32_t bytes, uint32_t mbar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(saddr), "l"(gptr),
+                 "r"(bytes), "r"(mbar)
+                 : "memory");
+}
+
+__global__ void __launch_bounds__(kBinThreads, 1) bin_scatter_kernel(const uint32_t* __restrict__ keys_in, uint64_t n, uint32_t shift,
+                                                                     uint32_t n_tiles, const uint32_t* __restrict__ offsets,
+                                                                     const BinPayload B, uint32_t* __restrict__ inv) {
+    extern __shared__ __align__(128) uint8_t smem_raw[];
+    float* s_pay = (float*)smem_raw;                                 // [3][4096*3] x, n, wo of the tile as they lie in memory
+    uint32_t* s_dst = (uint32_t*)(s_pay + kTile * 9);                // [4096] global position of each sorted position
+    uint32_t* s_cnt = s_dst + kTile;                                 // [1024] digit counts, then tile-local start positions
+    uint32_t* s_delta = s_cnt + kDigits;                             // [1024] global position - tile-local sorted position
+    uint32_t* s_warp = s_delta + kDigits;                            // [16] warp totals of the digit scan
+    uint64_t* s_bar = (uint64_t*)(s_warp + kBinThreads / 32);
+    uint16_t* s_src = (uint16_t*)(s_bar + 2);                        // [4096] tile-local source row of each sorted position
+    const uint32_t tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const uint64_t tile_base = (uint64_t)blockIdx.x * kTile;
     const uint32_t tile_n = (uint32_t)(n - tile_base < (uint64_t)kTile ? n - tile_base : (uint64_t)kTile);
-    const uint32_t wbase = warp * kWarpChunk;
-    const uint32_t lt = (1u << lane) - 1u;
-    uint32_t dig[kItems], rank[kItems];
+    const uint32_t nf = tile_n * 3;
+    const float* g[3] = {B.x + tile_base * 3, B.nrm ? B.nrm + tile_base * 3 : nullptr, B.wo + tile_base * 3};
+    const uint32_t n_arr = B.nrm ? 3u : 2u;
+    const uint32_t bar = smem_u32(s_bar);
+    // bulk copies need 16-byte aligned addresses and sizes; anything else takes the plain loop
+    const bool bulk = (tile_n & 3u) == 0 && ((((uintptr_t)g[0]) | ((uintptr_t)g[1]) | ((uintptr_t)g[2])) & 15u) == 0;
+    if (tid == 0) {
+        mbar_init(bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
 #pragma unroll
-    for (int it = 0; it < kItems; ++it) {
-        const uint32_t li = wbase + it * 32 + lane;
+    for (int k = 0; k < kBinDPT; ++k) s_cnt[tid + k * kBinThreads] = 0;
+    __syncthreads();
+    if (bulk) {
+        if (tid == 0) {
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(nf * 4u * n_arr) : "memory");
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                if (g[a]) bulk_g2s(smem_u32(s_pay + a * kTile * 3), g[a], nf * 4u, bar);
+        }
+    } else {
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            if (g[a])
+                for (uint32_t f = tid; f < nf; f += kBinThreads) s_pay[a * kTile * 3 + f] = __ldg(g[a] + f);
+    }
+    uint32_t dig[kBinItems], rank[kBinItems];
+#pragma unroll
+    for (int it = 0; it < kBinItems; ++it) {
+        const uint32_t li = it * kBinThreads + tid;
         dig[it] = li < tile_n ? (keys_in[tile_base + li] >> shift) & (kDigits - 1) : 0u;
     }
 #pragma unroll
-    for (int it = 0; it < kItems; ++it) {
-        const bool live = wbase + it * 32 + lane < tile_n;
-        const uint32_t active = __ballot_sync(0xffffffffu, live);
-        if (live) {
-            const uint32_t peers = __match_any_sync(active, dig[it]);
-            const uint32_t r = __popc(peers & lt);
-            rank[it] = pos[warp][dig[it]] + r;
-            __syncwarp(active);
-            if (r == 0) pos[warp][dig[it]] += __popc(peers);
-        }
-        __syncwarp();
-    }
+    for (int it = 0; it < kBinItems; ++it)
+        if (it * kBinThreads + tid < tile_n) rank[it] = atomicAdd(&s_cnt[dig[it]], 1u);
     __syncthreads();
-    {   // exclusive scan of the tile's digit counts in digit order; thread t owns digits 4t .. 4t+3
-        uint32_t cnt[kDPT], mine = 0;
+    {   // exclusive scan of the tile's digit counts in digit order; thread t owns digits 2t, 2t+1
+        uint32_t cnt[kBinDPT], mine = 0;
 #pragma unroll
-        for (int k = 0; k < kDPT; ++k) {
-            uint32_t c = 0;
-#pragma unroll
-            for (int w = 0; w < kSortThreads / 32; ++w) c += pos[w][threadIdx.x * kDPT + k];
-            cnt[k] = c;
-            mine += c;
+        for (int k = 0; k < kBinDPT; ++k) {
+            cnt[k] = s_cnt[tid * kBinDPT + k];
+            mine += cnt[k];
         }
         uint32_t incl = mine;
 #pragma unroll
@@ -275,51 +296,46 @@ __global__ void __launch_bounds__(kSortThreads) bin_scatter_kernel(const uint32_
         uint32_t run = incl - mine;
         for (uint32_t w = 0; w < warp; ++w) run += s_warp[w];
 #pragma unroll
-        for (int k = 0; k < kDPT; ++k) {
-            const uint32_t d = threadIdx.x * kDPT + k;
+        for (int k = 0; k < kBinDPT; ++k) {
+            const uint32_t d = tid * kBinDPT + k;
             s_delta[d] = offsets[(size_t)d * n_tiles + blockIdx.x] - run;
-            uint32_t r = run;
-#pragma unroll
-            for (int w = 0; w < kSortThreads / 32; ++w) {
-                const uint32_t c = pos[w][d];
-                pos[w][d] = r;
-                r += c;
-            }
+            s_cnt[d] = run;
             run += cnt[k];
         }
     }
     __syncthreads();
 #pragma unroll
-    for (int it = 0; it < kItems; ++it) {
-        const uint32_t li = wbase + it * 32 + lane;
+    for (int it = 0; it < kBinItems; ++it) {
+        const uint32_t li = it * kBinThreads + tid;
         if (li < tile_n) {
-            const uint32_t lp = pos[warp][dig[it]] + rank[it];
-            s_src[lp] = li;
-            s_dig[lp] = (uint16_t)dig[it];
-            inv[tile_base + li] = lp + s_delta[dig[it]];
+            const uint32_t lp = s_cnt[dig[it]] + rank[it];
+            const uint32_t dst = lp + s_delta[dig[it]];
+            s_dst[lp] = dst;
+            s_src[lp] = (uint16_t)li;
+            inv[tile_base + li] = dst;
         }
     }
     __syncthreads();
-    const float* src[3] = {B.x, B.nrm, B.wo};
-    float* dst[3] = {B.sx, B.sn, B.sw};
-    const uint32_t nf = tile_n * 3;
-#pragma unroll 1
+    if (bulk) mbar_wait(bar, 0);
+    float* out[3] = {B.sx, B.sn, B.sw};
+#pragma unroll
     for (int a = 0; a < 3; ++a) {
-        const float* g = src[a] + tile_base * 3;
-        for (uint32_t f = threadIdx.x; f < nf; f += kSortThreads) s_pay[f] = __ldg(g + f);
-        __syncthreads();
-        float* o = dst[a];
-        for (uint32_t f = threadIdx.x; f < nf; f += kSortThreads) {
-            const uint32_t lp = f / 3u, k = f - 3u * lp;
-            o[(size_t)(lp + s_delta[s_dig[lp]]) * 3 + k] = s_pay[3u * s_src[lp] + k];
+        if (!g[a]) continue;
+        const float* sp = s_pay + a * kTile * 3;
+        float* o = out[a];
+#pragma unroll 4
+        for (uint32_t f = tid; f < nf; f += kBinThreads) {
+            const uint32_t p = f / 3u, k = f - 3u * p;
+            o[(size_t)s_dst[p] * 3 + k] = sp[3u * s_src[p] + k];
         }
-        __syncthreads();
     }
-    if (B.n_extra) {   // extras: gathered straight from the tile's own rows (L1-resident), written in runs
+    if (B.idx)
+        for (uint32_t p = tid; p < tile_n; p += kBinThreads) B.idx[s_dst[p]] = (uint32_t)tile_base + s_src[p];
+    if (B.n_extra) {   // extras: gathered straight from the tile's own rows, written in runs
         const uint32_t ne = B.n_extra, nfe = tile_n * ne;
-        for (uint32_t f = threadIdx.x; f < nfe; f += kSortThreads) {
-            const uint32_t lp = f / ne, k = f - ne * lp;
-            B.se[(size_t)(lp + s_delta[s_dig[lp]]) * ne + k] = __ldg(B.extra + (tile_base + s_src[lp]) * ne + k);
+        for (uint32_t f = tid; f < nfe; f += kBinThreads) {
+            const uint32_t p = f / ne, k = f - ne * p;
+            B.se[(size_t)s_dst[p] * ne + k] = __ldg(B.extra + (tile_base + s_src[p]) * ne + k);
         }
     }
 }
@@ -336,7 +352,7 @@ __global__ void __launch_bounds__(256) unbin_kernel(const float* __restrict__ bi
 }
 
 int launch_bin_queries(const QueryParams& Q, uint32_t* keys, uint32_t* hist, float* sx, float* sn, float* sw, float* se,
-                       uint32_t* inv, cudaStream_t stream) {
+                       uint32_t* inv, uint32_t* idx, cudaStream_t stream) {
     if (Q.n == 0) return 0;
     static bool attr = false;
     if (!attr) {
@@ -349,8 +365,8 @@ int launch_bin_queries(const QueryParams& Q, uint32_t* keys, uint32_t* hist, flo
     constexpr uint32_t shift = 30 - kBits;
     radix_hist_kernel<true><<<n_tiles, kSortThreads, 0, stream>>>(Q.x, keys, Q.n, shift, n_tiles, hist, tot);
     scan_kernel<<<kDigits, kSortThreads, 0, stream>>>(hist, tot, n_tiles);
-    const BinPayload B{Q.x, Q.nrm, Q.wo, Q.extra, Q.n_extra, sx, sn, sw, se};
-    bin_scatter_kernel<<<n_tiles, kSortThreads, kBinSmemBytes, stream>>>(keys, Q.n, shift, n_tiles, hist, B, inv);
+    const BinPayload B{Q.x, Q.nrm, Q.wo, Q.extra, Q.extra ? Q.n_extra : 0u, sx, sn, sw, se, idx};
+    bin_scatter_kernel<<<n_tiles, kBinThreads, kBinSmemBytes, stream>>>(keys, Q.n, shift, n_tiles, hist, B, inv);
     return 3;
 }
 

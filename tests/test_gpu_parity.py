@@ -57,26 +57,6 @@ def _run_all(P, w, ref_feat, ref_slot, ref_tex, ref_rgb, expect_fast=True):
         assert P.PATH_FUSED_MMA in results and P.PATH_FUSED_TC in results and P.PATH_FUSED_TC_TMEM in results
         # same arithmetic in the same order: the fused and unfused specialised paths agree bit for bit
         assert np.array_equal(results[P.PATH_FUSED_MMA], results[P.PATH_UNFUSED])
-    if ctx.oo_get_info()["hop_plan_ok"] and P.PATH_UNFUSED in results:
-        # OO_LAYOUT_QUAD (pre-expanded four-tap records): same texel values, same arithmetic, same order -> every fast
-        # path reproduces its own padded-layout result bit for bit (and therefore the oracle within the same bars)
-        ctx.oo_set_path(P.PATH_UNFUSED)
-        f_pad = ctx.oo_encode(x, wo)
-        ctx.oo_set_layout("quad")
-        info = ctx.oo_get_info()
-        assert info["layout"] == 1 and info["quad_atlas_bytes"] > info["atlas_bytes"]
-        for path, ref in results.items():
-            if path == P.PATH_GENERIC:
-                continue
-            ctx.oo_set_path(path)
-            assert np.array_equal(ctx.oo_query(x, n, wo, ex).cpu().numpy(), ref), "path %d differs under OO_LAYOUT_QUAD" % path
-        ctx.oo_set_path(P.PATH_UNFUSED)
-        f_quad = ctx.oo_encode(x, wo)
-        assert torch.equal(f_pad, f_quad)
-        check_features(f_quad.float().cpu().numpy(), ref_feat)
-        ctx.oo_set_layout("padded")
-        info = ctx.oo_get_info()
-        assert info["layout"] == 0 and info["quad_atlas_bytes"] == 0
     ctx.oo_set_path(P.PATH_AUTO)
     rgb = ctx.oo_query(x, n, wo, ex).cpu().numpy()
     info = ctx.oo_get_info()
@@ -251,17 +231,15 @@ def test_presort_bin_is_bit_identical(P):
         x, nr, wo, ex = _dev(q)
         ref = ctx.oo_query(x, nr, wo, ex)
         assert ctx.oo_get_info()["presorted_last_query"] == 0
-        ctx.oo_set_presort("bin")
+        ctx.oo_set_presort("bin", min_queries=32768)
         with pytest.raises(P.OOError) as e:          # the binned copy lives in reserved scratch
             ctx.oo_query(x, nr, wo, ex)
         assert e.value.status == 2
         ctx.oo_reserve(n)
-        for layout in ("padded", "quad"):
-            ctx.oo_set_layout(layout)
-            guard = torch.full((n + 64, 3), -7.0, dtype=torch.float32, device="cuda")
-            ctx.oo_query(x, nr, wo, ex, rgb=guard[:n])
-            assert ctx.oo_get_info()["presorted_last_query"] == 1
-            assert torch.equal(guard[:n], ref) and bool((guard[n:] == -7.0).all())
+        guard = torch.full((n + 64, 3), -7.0, dtype=torch.float32, device="cuda")
+        ctx.oo_query(x, nr, wo, ex, rgb=guard[:n])
+        assert ctx.oo_get_info()["presorted_last_query"] == 1
+        assert torch.equal(guard[:n], ref) and bool((guard[n:] == -7.0).all())
         # through the host pipeline (chunks of the frame are binned one by one)
         h = ctx.oo_query_host(q.x, q.nrm, q.wo, q.extra)
         assert np.array_equal(np.asarray(h), ref.cpu().numpy())
@@ -279,7 +257,16 @@ def test_presort_bin_is_bit_identical(P):
             assert ctx.oo_get_info()["presorted_last_query"] == 1
             ctx.oo_set_presort("none")
             assert torch.equal(got, ctx.oo_query(x, nr, wo, ex))
-            ctx.oo_set_presort("bin")
+            ctx.oo_set_presort("bin", min_queries=32768)
+        # oo_encode: x and wo binned, every row (features, slots, base texels) stored at its query's own index
+        ctx.oo_set_path(P.PATH_UNFUSED)
+        f1, s1, t1 = ctx.oo_encode(x, wo, want_debug=True)
+        assert ctx.oo_get_info()["presorted_last_encode"] == 1
+        ctx.oo_set_presort("none")
+        f0, s0, t0 = ctx.oo_encode(x, wo, want_debug=True)
+        assert ctx.oo_get_info()["presorted_last_encode"] == 0
+        assert torch.equal(f0, f1) and torch.equal(s0, s1) and torch.equal(t0, t1)
+        ctx.oo_set_presort("bin", min_queries=32768)
         ctx.oo_set_path(P.PATH_AUTO)
         ctx.oo_set_presort("none")
         ctx.oo_query(x, nr, wo, ex)
