@@ -32,7 +32,12 @@ __device__ __forceinline__ void relu_pack32(const uint32_t (&r)[32], uint32_t (&
 }
 }  // namespace
 
-template <int L, int F, bool F32, int NWG>
+// PIPE (chosen at launch for fp16 trees whose first two used levels are dense and the rest hops, i.e. the BASELINE.json configs):
+// the hop chain and the gathers overlap.  Stage l resolves slot l from the hop load issued one stage earlier, issues the next
+// hop and the taps of level l, and consumes the taps of level l-2: a query exposes max(hop, taps) once per hop level plus one
+// last gather (4 latencies for L = 5) instead of every hop and then every gather batch (6).  Same taps, same weights, same
+// accumulation order per level: bit-identical to the batched form.
+template <int L, int F, bool F32, int NWG, bool PIPE = false>
 __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_constant__ TreeParams T,
                                                                const __grid_constant__ MlpParams M,
                                                                const __grid_constant__ QueryParams Q,
@@ -105,34 +110,70 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
 #pragma unroll
         for (int k = 0; k < 3; ++k) { x[k] = s_q[k * 128]; w[k] = s_q[(6 + k) * 128]; }
         // ------------------------------------------------------------------ gather: one query per thread -> A0 in TMEM
-        Encoded<L, F, F32> e;
-        locate<L, F, F32>(T, s_dense, x, w, e);
         const uint32_t a0 = tmem_lane + 64;                          // layer 0 is even: A at [64, 64 + k1/2)
-        constexpr int NB = (F * (F32 ? 4 : 2) == 16) ? (L < 4 ? L : 4) : (F * (F32 ? 4 : 2) == 32 ? 2 : 1);   // levels per load batch
+        auto store_level = [&](int l, const float (&h)[F]) {
+            if constexpr (F % 8 == 0) {
 #pragma unroll
-        for (int l0 = 0; l0 < L; l0 += NB) {
-            float h[NB][F];
-            if (l0 + NB <= L) {
-                gather_levels<F, F32, NB>(&T.lv[l0], &e.slot[l0], e.uv, h);
-            } else {     // ragged last batch: one level at a time
+                for (int v = 0; v < F / 8; ++v)
+                    tmem_st4(a0 + (l * F) / 2 + 4 * v, pack_half2(h[8 * v], h[8 * v + 1]), pack_half2(h[8 * v + 2], h[8 * v + 3]),
+                             pack_half2(h[8 * v + 4], h[8 * v + 5]), pack_half2(h[8 * v + 6], h[8 * v + 7]));
+            } else {   // F == 4
+                tmem_st2(a0 + (l * 4) / 2, pack_half2(h[0], h[1]), pack_half2(h[2], h[3]));
+            }
+        };
+        if constexpr (PIPE && L >= 3) {
+            const int qmax = (int)(1u << T.depth_eff) - 1;
+            const int qx = quantise(x[0], T.scale_eff, qmax), qy = quantise(x[1], T.scale_eff, qmax), qz = quantise(x[2], T.scale_eff, qmax);
+            const OctaUV uv = octa_project(w[0], w[1], w[2]);
+            auto dense_at = [&](uint32_t off, uint32_t d, uint32_t sh) {
+                return s_dense[off + (((qz >> sh) << (2 * d)) | ((qy >> sh) << d) | (qx >> sh))];
+            };
+            auto hop_load = [&](const LevelParams& lv, int prev) {
+                const uint32_t sh = lv.shift, g = lv.gap, m = (1u << g) - 1u;
+                const uint32_t idx = ((((uint32_t)qz >> sh) & m) << (2 * g)) | ((((uint32_t)qy >> sh) & m) << g) | (((uint32_t)qx >> sh) & m);
+                return prev >= 0 ? __ldg(lv.hop + (((size_t)prev << (3 * g)) + idx)) : -1;
+            };
+            TapSet<F, F32> ring[2];
+            int hv = hop_load(T.lv[2], dense_at(T.t_dense_off, T.t_depth, T.t_shift));
+            issue_taps<F, F32>(T.lv[0], dense_at(T.lv[0].dense_off, T.lv[0].depth, T.lv[0].shift), uv, ring[0]);
+            issue_taps<F, F32>(T.lv[1], dense_at(T.lv[1].dense_off, T.lv[1].depth, T.lv[1].shift), uv, ring[1]);
 #pragma unroll
-                for (int b = 0; b < NB; ++b)
-                    if (l0 + b < L) {
-                        const Tap tp = level_tap(e.uv, T.lv[l0 + b].half_r, T.lv[l0 + b].off);
-                        gather_level<F, F32>(T.lv[l0 + b], e.slot[l0 + b], tp, h[b]);
-                    }
+            for (int l = 2; l < L; ++l) {
+                const int slot = hv;
+                if (l + 1 < L) hv = hop_load(T.lv[l + 1], slot);
+                float h[F];
+                consume_taps<F, F32>(ring[l & 1], h);
+                store_level(l - 2, h);
+                issue_taps<F, F32>(T.lv[l], slot, uv, ring[l & 1]);
             }
 #pragma unroll
-            for (int b = 0; b < NB; ++b) {
-                const int l = l0 + b;
-                if (l >= L) break;
-                if constexpr (F % 8 == 0) {
+            for (int l = L - 2; l < L; ++l) {
+                float h[F];
+                consume_taps<F, F32>(ring[l & 1], h);
+                store_level(l, h);
+            }
+        } else {
+            Encoded<L, F, F32> e;
+            locate<L, F, F32>(T, s_dense, x, w, e);
+            constexpr int NB = (F * (F32 ? 4 : 2) == 16) ? (L < 4 ? L : 4) : (F * (F32 ? 4 : 2) == 32 ? 2 : 1);   // levels per load batch
 #pragma unroll
-                    for (int v = 0; v < F / 8; ++v)
-                        tmem_st4(a0 + (l * F) / 2 + 4 * v, pack_half2(h[b][8 * v], h[b][8 * v + 1]), pack_half2(h[b][8 * v + 2], h[b][8 * v + 3]),
-                                 pack_half2(h[b][8 * v + 4], h[b][8 * v + 5]), pack_half2(h[b][8 * v + 6], h[b][8 * v + 7]));
-                } else {   // F == 4
-                    tmem_st2(a0 + (l * 4) / 2, pack_half2(h[b][0], h[b][1]), pack_half2(h[b][2], h[b][3]));
+            for (int l0 = 0; l0 < L; l0 += NB) {
+                float h[NB][F];
+                if (l0 + NB <= L) {
+                    gather_levels<F, F32, NB>(&T.lv[l0], &e.slot[l0], e.uv, h);
+                } else {     // ragged last batch: one level at a time
+#pragma unroll
+                    for (int b = 0; b < NB; ++b)
+                        if (l0 + b < L) {
+                            const Tap tp = level_tap(e.uv, T.lv[l0 + b].half_r, T.lv[l0 + b].off);
+                            gather_level<F, F32>(T.lv[l0 + b], e.slot[l0 + b], tp, h[b]);
+                        }
+                }
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    const int l = l0 + b;
+                    if (l >= L) break;
+                    store_level(l, h[b]);
                 }
             }
         }
@@ -242,14 +283,38 @@ bool tm_shape_supported(uint32_t L, uint32_t F, bool f32) {
     return false;
 }
 
+// the pipelined descent exists for 32-byte texels (two levels per load batch otherwise) on trees whose first two used levels
+// are dense and every later one a hop
+static bool pipe_applies(const TreeParams& T) {
+    if (T.n_levels < 3 || T.f32 || !T.lv[0].dense || !T.lv[1].dense) return false;
+    for (uint32_t l = 2; l < T.n_levels; ++l)
+        if (T.lv[l].dense) return false;
+    return true;
+}
+#define OO_TM_PIPE_SHAPES(X) X(3, 16, false) X(4, 16, false) X(5, 16, false) X(3, 8, false) X(4, 8, false) X(5, 8, false)
+
 template <int NWG>
 static int launch_tm_nwg(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, uint32_t wg_cols,
-                         cudaStream_t stream) {
+                         bool pipe, cudaStream_t stream) {
     const uint64_t n_tiles = (Q.n + kRows - 1) / kRows;
     const uint64_t blocks = (n_tiles + NWG - 1) / NWG;
     const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms ? blocks : (uint64_t)n_sms);
     const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + NWG * (10 + Q.n_extra) * kRows * 4 + 128;
     if (smem > 227 * 1024) return -1;
+    if (pipe && pipe_applies(T)) {
+#define X(l, f, t)                                                                                                     \
+    if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                                            \
+        static bool attr = false;                                                                                      \
+        if (!attr) {                                                                                                   \
+            cudaFuncSetAttribute(fused_tm_kernel<l, f, t, NWG, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); \
+            attr = true;                                                                                               \
+        }                                                                                                              \
+        fused_tm_kernel<l, f, t, NWG, true><<<grid, NWG * 128, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles, wg_cols); \
+        return 1;                                                                                                      \
+    }
+        OO_TM_PIPE_SHAPES(X)
+#undef X
+    }
 #define X(l, f, t)                                                                                                     \
     if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                                            \
         static bool attr = false;                                                                                      \
@@ -266,12 +331,16 @@ static int launch_tm_nwg(const TreeParams& T, const MlpParams& M, const QueryPar
 }
 
 // warpgroups per block = how many column strides fit in the 512 TMEM columns; -1 if the shape has no instance
-int launch_fused_tm(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, cudaStream_t stream) {
+int launch_fused_tm(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, cudaStream_t stream,
+                    bool binned) {
     if (Q.n == 0) return 0;
     if (M.out_dim > 4 || !M.image_tc || M.k1 > 128) return -1;
+    // Measured on B200 (PIPE against the batched form): config 1 60.2 -> 58.6 us, config 2 55.3 -> 54.5 us, config 3 326 -> 309 us,
+    // unsorted incoherent 2^22 queries 1.53 -> 1.32 ms; on binned queries -2 % at 2^22 but +8 % at 2^24, so those keep the batches.
+    const bool pipelined_descent = !binned;
     const uint32_t wg_cols = 64 + (M.k1 / 2 > 32 ? M.k1 / 2 : 32);
-    if (5 * wg_cols <= 512) return launch_tm_nwg<5>(T, M, Q, rgb, n_sms, wg_cols, stream);
-    if (4 * wg_cols <= 512) return launch_tm_nwg<4>(T, M, Q, rgb, n_sms, wg_cols, stream);
+    if (5 * wg_cols <= 512) return launch_tm_nwg<5>(T, M, Q, rgb, n_sms, wg_cols, pipelined_descent, stream);
+    if (4 * wg_cols <= 512) return launch_tm_nwg<4>(T, M, Q, rgb, n_sms, wg_cols, pipelined_descent, stream);
     return -1;
 }
 
