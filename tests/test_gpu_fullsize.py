@@ -59,6 +59,24 @@ def test_config3_full_tree_sampled_queries():
     qi = gen.incoherent_queries(w.scene, 1 << 16, 0)
     ref = co.query(qi.x, qi.nrm, qi.wo)
     check_rgb(ctx.oo_query(_dev(qi.x), _dev(qi.nrm), _dev(qi.wo)).cpu().numpy(), ref)
+    # config 4 as bench.py --sweep 4 times it: 2^22 incoherent queries, unsorted and with OO_PRESORT_BIN at its default
+    # threshold; the oracle on every 61st query, the two launches against each other on all of them
+    qi = gen.incoherent_queries(w.scene, 1 << 22, 0)
+    xi, ni, wi = _dev(qi.x), _dev(qi.nrm), _dev(qi.wo)
+    plain = ctx.oo_query(xi, ni, wi)
+    ctx.oo_reserve(qi.n)
+    ctx.oo_set_presort("bin")
+    binned = ctx.oo_query(xi, ni, wi)
+    assert ctx.oo_get_info()["presorted_last_query"] == 1
+    assert torch.equal(plain, binned)
+    idx = np.arange(0, qi.n, 61)
+    qs = qi.take(idx)
+    check_rgb(binned.cpu().numpy()[idx], co.query(qs.x, qs.nrm, qs.wo))
+    fb = ctx.oo_encode(xi, wi)
+    assert ctx.oo_get_info()["presorted_last_encode"] == 1
+    ctx.oo_set_presort("none")
+    assert torch.equal(fb, ctx.oo_encode(xi, wi))
+    check_features(fb[torch.from_numpy(idx).cuda()].float().cpu().numpy(), co.encode(qs.x, qs.wo)[0])
 
 
 def test_paper_shapes_full_frame_sampled_queries():
