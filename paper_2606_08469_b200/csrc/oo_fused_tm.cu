@@ -34,7 +34,7 @@ __device__ __forceinline__ void relu_pack32(const uint32_t (&r)[32], uint32_t (&
 
 // PIPE (chosen at launch for fp16 trees whose first two used levels are dense and the rest hops, i.e. the BASELINE.json configs):
 // the hop chain and the gathers overlap.  Stage l resolves slot l from the hop load issued one stage earlier, issues the next
-// hop and the taps of level l, and consumes the taps of level l-2: a query exposes max(hop, taps) once per hop level plus one
+// hop and the taps of level l, and consumes the taps of level l-RD (RD = 2, or 3 for 16-byte texels): a query exposes max(hop, taps) once per hop level plus one
 // last gather (4 latencies for L = 5) instead of every hop and then every gather batch (6).  Same taps, same weights, same
 // accumulation order per level: bit-identical to the batched form.
 template <int L, int F, bool F32, int NWG, bool PIPE = false>
@@ -133,7 +133,8 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
                 const uint32_t idx = ((((uint32_t)qz >> sh) & m) << (2 * g)) | ((((uint32_t)qy >> sh) & m) << g) | (((uint32_t)qx >> sh) & m);
                 return prev >= 0 ? __ldg(lv.hop + (((size_t)prev << (3 * g)) + idx)) : -1;
             };
-            TapSet<F, F32> ring[2];
+            constexpr int RD = (F * (F32 ? 4 : 2) == 16 && L >= 4) ? 3 : 2;      // levels of taps in flight (16-byte texels: 2 -> 58.7, 3 -> 58.2, 4 -> 60.2 us on config 1)
+            TapSet<F, F32> ring[RD];
             int hv = hop_load(T.lv[2], dense_at(T.t_dense_off, T.t_depth, T.t_shift));
             issue_taps<F, F32>(T.lv[0], dense_at(T.lv[0].dense_off, T.lv[0].depth, T.lv[0].shift), uv, ring[0]);
             issue_taps<F, F32>(T.lv[1], dense_at(T.lv[1].dense_off, T.lv[1].depth, T.lv[1].shift), uv, ring[1]);
@@ -141,15 +142,17 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             for (int l = 2; l < L; ++l) {
                 const int slot = hv;
                 if (l + 1 < L) hv = hop_load(T.lv[l + 1], slot);
-                float h[F];
-                consume_taps<F, F32>(ring[l & 1], h);
-                store_level(l - 2, h);
-                issue_taps<F, F32>(T.lv[l], slot, uv, ring[l & 1]);
+                if (l >= RD) {
+                    float h[F];
+                    consume_taps<F, F32>(ring[l % RD], h);
+                    store_level(l - RD, h);
+                }
+                issue_taps<F, F32>(T.lv[l], slot, uv, ring[l % RD]);
             }
 #pragma unroll
-            for (int l = L - 2; l < L; ++l) {
+            for (int l = L - RD; l < L; ++l) {
                 float h[F];
-                consume_taps<F, F32>(ring[l & 1], h);
+                consume_taps<F, F32>(ring[l % RD], h);
                 store_level(l, h);
             }
         } else {
