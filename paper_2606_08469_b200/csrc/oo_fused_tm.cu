@@ -49,25 +49,28 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
     int32_t* s_dense = (int32_t*)smem;
     uint8_t* s_w = smem + dense_bytes;
     uint8_t* s_stage = s_w + ((M.image_tc_bytes + 127) & ~127u);
-    uint64_t* s_bar = (uint64_t*)(s_stage + NWG * q_bytes);
-    uint32_t* s_tmem = (uint32_t*)(s_bar + NWG);
+    uint64_t* s_bar = (uint64_t*)(s_stage + NWG * q_bytes);      // one per warpgroup, then tables, then weights
+    uint32_t* s_tmem = (uint32_t*)(s_bar + NWG + 2);
 
     const uint32_t wg = threadIdx.x >> 7, row = threadIdx.x & 127, warp = threadIdx.x >> 5;
-    {
-        const uint4* s = (const uint4*)T.dense;
-        uint4* d = (uint4*)s_dense;
-        for (uint32_t i = threadIdx.x; i < T.dense_ints / 4; i += NWG * 128) d[i] = __ldg(s + i);
-        s = (const uint4*)M.image_tc;
-        d = (uint4*)s_w;
-        for (uint32_t i = threadIdx.x; i < M.image_tc_bytes / 16; i += NWG * 128) d[i] = __ldg(s + i);
+    // Prologue: the descent tables and the weight image arrive by two bulk asynchronous copies that thread 0 issues before
+    // anything else; the tables are awaited by every thread before its first descent, the weights only by the warp that issues
+    // the MMAs, right before its first one (both travel through the async proxy: no proxy fence, no block barrier for them).
+    // Before: 512-640 threads looping LDG.128 -> STS over 54 KB of cold lines, then fence.proxy.async + __syncthreads.
+    const uint32_t bar_d = smem_u32(&s_bar[NWG]), bar_w = smem_u32(&s_bar[NWG + 1]);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < NWG + 2; ++k) mbar_init(smem_u32(&s_bar[k]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_expect_tx(bar_d, T.dense_ints * 4);
+        bulk_g2s(smem_u32(s_dense), T.dense, T.dense_ints * 4, bar_d);
+        mbar_expect_tx(bar_w, M.image_tc_bytes);
+        bulk_g2s(smem_u32(s_w), M.image_tc, M.image_tc_bytes, bar_w);
     }
-    if (threadIdx.x < NWG) mbar_init(smem_u32(&s_bar[threadIdx.x]), 1);
-    if (threadIdx.x == 0) asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     if (warp == 0) {
         tmem_alloc(smem_u32(s_tmem), 512);
         tmem_relinquish();
     }
-    fence_async_smem();          // the weight image was written with generic stores and is read by the tensor core
     fence_before_sync();
     __syncthreads();
     fence_after_sync();
@@ -103,6 +106,8 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
     // per SM on a few SMs.  Measured on B200: config 1 61.1 -> 60.1 us, config 3 333.3 -> 329.4 us.
     uint32_t tile = wg * gridDim.x + blockIdx.x;
     if (tile < n_tiles) prefetch(tile);
+    mbar_wait(bar_d, 0);                  // descent tables in shared memory
+    bool w_ready = false;
     for (; tile < n_tiles; tile += tile_stride) {
         float x[3], w[3];
         const bool valid = (uint64_t)tile * kRows + row < Q.n;
@@ -214,6 +219,10 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             fence_before_sync();
             named_bar(1 + wg, 128);
             if (leader_warp) {
+                if (!w_ready) {
+                    mbar_wait(bar_w, 0);      // weight image in shared memory (first MMA of this warpgroup only)
+                    w_ready = true;
+                }
                 fence_after_sync();
                 umma_group_ts<8>(tmem_wg + (odd ? 32u : 0u), tmem_wg + (odd ? 0u : 64u), smem_desc(w_addr + w_off, 1024, 128), 2048 >> 4,
                                  idesc_h, kt_n, bar);

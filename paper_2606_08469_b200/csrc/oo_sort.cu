@@ -223,12 +223,6 @@ constexpr int kBinItems = kTile / kBinThreads;      // 8 queries per thread
 constexpr int kBinDPT = kDigits / kBinThreads;      // 2 digits per thread in the scan
 constexpr uint32_t kBinSmemBytes = kTile * 9 * 4 + kTile * 4 + kTile * 2 + kDigits * 4 * 2 + (kBinThreads / 32) * 4 + 16;
 
-__device__ __forceinline__ void bulk_g2s(uint32_t saddr, const void* gptr, uint32_t bytes, uint32_t mbar) {
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(saddr), "l"(gptr),
-                 "r"(bytes), "r"(mbar)
-                 : "memory");
-}
-
 __global__ void __launch_bounds__(kBinThreads, 1) bin_scatter_kernel(const uint32_t* __restrict__ keys_in, uint64_t n, uint32_t shift,
                                                                      uint32_t n_tiles, const uint32_t* __restrict__ offsets,
                                                                      const BinPayload B, uint32_t* __restrict__ inv) {
@@ -269,7 +263,7 @@ __global__ void __launch_bounds__(kBinThreads, 1) bin_scatter_kernel(const uint3
     __syncthreads();
     if (bulk) {
         if (tid == 0) {
-            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(nf * 4u * n_arr) : "memory");
+            mbar_expect_tx(bar, nf * 4u * n_arr);
 #pragma unroll
             for (int a = 0; a < 3; ++a)
                 if (g[a]) bulk_g2s(smem_u32(s_pay + a * kTile * 3), g[a], nf * 4u, bar);

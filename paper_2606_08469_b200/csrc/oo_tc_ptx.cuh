@@ -33,6 +33,17 @@ __device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
         " @!p bra OO_WAIT_%=;\n}\n" ::"r"(mbar), "r"(parity)
         : "memory");
 }
+// Bulk asynchronous copy global -> shared (SASS UBLKCP): `bytes` and both addresses multiples of 16; completion is counted in
+// bytes on the mbarrier, which one thread arms with mbar_expect_tx first.  The data arrives through the async proxy: generic
+// loads may read it after mbar_wait, and tcgen05.mma (async proxy itself) needs no proxy fence.
+__device__ __forceinline__ void mbar_expect_tx(uint32_t mbar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(mbar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t saddr, const void* gptr, uint32_t bytes, uint32_t mbar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(saddr), "l"(gptr),
+                 "r"(bytes), "r"(mbar)
+                 : "memory");
+}
 __device__ __forceinline__ void cp_async4(uint32_t saddr, const void* gptr) {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(saddr), "l"(gptr) : "memory");
 }
