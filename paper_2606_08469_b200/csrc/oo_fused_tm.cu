@@ -309,8 +309,9 @@ template <int NWG>
 static int launch_tm_nwg(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, uint32_t wg_cols,
                          bool pipe, cudaStream_t stream) {
     const uint64_t n_tiles = (Q.n + kRows - 1) / kRows;
-    const uint64_t blocks = (n_tiles + NWG - 1) / NWG;
-    const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms ? blocks : (uint64_t)n_sms);
+    // one block per SM as soon as there is a tile for each: a small batch spreads over all SMs (a warpgroup alone on its SM
+    // finishes a tile faster than four sharing one) instead of filling every warpgroup of the first n_tiles / NWG SMs
+    const unsigned grid = (unsigned)(n_tiles < (uint64_t)n_sms ? n_tiles : (uint64_t)n_sms);
     const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + NWG * (10 + Q.n_extra) * kRows * 4 + 128;
     if (smem > 227 * 1024) return -1;
     if (pipe && pipe_applies(T)) {
