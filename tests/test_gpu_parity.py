@@ -276,6 +276,30 @@ def test_presort_bin_is_bit_identical(P):
         ctx.close()
 
 
+def test_presort_bin_extras_and_output_widths(P):
+    """OO_PRESORT_BIN with several extra scalars (moved column by column) and decoders of 1, 4 and 8 outputs (the generic
+    un-binning kernel; 8 outputs run on the mma.sync path): bit-identical to the unsorted call, which matches the oracle."""
+    n = 36000
+    for n_extra, out_dim in ((3, 4), (0, 1), (10, 8)):
+        w = gen.scene_workload(1, width=32, height=32, incoherent_n=n)
+        q = w.queries
+        if n_extra:
+            q.extra = gen.uniform_f32(7, 40 + n_extra, n * n_extra, 0.0, 1.0).reshape(n, n_extra)
+        L, F = len(w.tree.level_depth), w.atlas.F
+        w.mlp = gen.make_mlp(L * F + 6 + n_extra, 2, 5, out_dim=out_dim)
+        ctx = P.OctaOctree(0).upload_workload(w)
+        ctx.oo_reserve(n)
+        x, nr, wo, ex = _dev(q)
+        ref = ctx.oo_query(x, nr, wo, ex)
+        assert tuple(ref.shape) == (n, out_dim)
+        ctx.oo_set_presort("bin", min_queries=1)
+        got = ctx.oo_query(x, nr, wo, ex)
+        assert ctx.oo_get_info()["presorted_last_query"] == 1
+        assert torch.equal(got, ref)
+        check_rgb(ref.cpu().numpy(), O.query(w.tree, w.atlas.levels, w.mlp.weights, q.x, q.nrm, q.wo, q.extra))
+        ctx.close()
+
+
 def test_query_host_equals_query(P):
     w = gen.scene_workload(2, width=96, height=64)
     q = w.queries
