@@ -37,7 +37,12 @@ __device__ __forceinline__ void relu_pack32(const uint32_t (&r)[32], uint32_t (&
 // hop and the taps of level l, and consumes the taps of level l-RD (RD = 2, or 3 for 16-byte texels): a query exposes max(hop, taps) once per hop level plus one
 // last gather (4 latencies for L = 5) instead of every hop and then every gather batch (6).  Same taps, same weights, same
 // accumulation order per level: bit-identical to the batched form.
-template <int L, int F, bool F32, int NWG, bool PIPE = false>
+// KS (first layers wider than 64 inputs, L*F >= 64): layer 0 runs as TWO MMA groups over the same 32 A columns.  The first 64
+// inputs (the levels below feature 64) are multiplied as soon as they are stored; the rest of the row (later levels, attributes,
+// padding) is gathered and packed while that MMA is in flight, stored over the same columns once it has completed, and
+// accumulated by the second group.  A tile then needs 96 TMEM columns like the narrow configs instead of 64 + k1/2, so five
+// warpgroups fit where four did (config 3: k1 = 96, 112 columns), at the price of one more MMA round trip per tile.
+template <int L, int F, bool F32, int NWG, bool PIPE = false, bool KS = false>
 __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_constant__ TreeParams T,
                                                                const __grid_constant__ MlpParams M,
                                                                const __grid_constant__ QueryParams Q,
@@ -116,7 +121,16 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
         for (int k = 0; k < 3; ++k) { x[k] = s_q[k * 128]; w[k] = s_q[(6 + k) * 128]; }
         // ------------------------------------------------------------------ gather: one query per thread -> A0 in TMEM
         const uint32_t a0 = tmem_lane + 64;                          // layer 0 is even: A at [64, 64 + k1/2)
+        constexpr int N_LATE = KS ? (L * F - 64) / 2 : 0;            // packed halves of the levels past input 64 (KS)
+        uint32_t late[N_LATE > 0 ? N_LATE : 1];
         auto store_level = [&](int l, const float (&h)[F]) {
+            if constexpr (KS) {
+                if (l * F >= 64) {            // kept in registers until the first MMA group has read the A columns
+#pragma unroll
+                    for (int k = 0; k < F / 2; ++k) late[(l * F - 64) / 2 + k] = pack_half2(h[2 * k], h[2 * k + 1]);
+                    return;
+                }
+            }
             if constexpr (F % 8 == 0) {
 #pragma unroll
                 for (int v = 0; v < F / 8; ++v)
@@ -124,6 +138,21 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
                              pack_half2(h[8 * v + 4], h[8 * v + 5]), pack_half2(h[8 * v + 6], h[8 * v + 7]));
             } else {   // F == 4
                 tmem_st2(a0 + (l * 4) / 2, pack_half2(h[0], h[1]), pack_half2(h[2], h[3]));
+            }
+            if constexpr (KS) {
+                if ((l + 1) * F == 64) {      // inputs 0..63 of all 128 rows are in TMEM: first MMA group of layer 0
+                    tmem_wait_st();
+                    fence_before_sync();
+                    named_bar(1 + wg, 128);
+                    if (leader_warp) {
+                        if (!w_ready) {
+                            mbar_wait(bar_w, 0);
+                            w_ready = true;
+                        }
+                        fence_after_sync();
+                        umma_group_ts<4>(tmem_wg, tmem_wg + 64u, smem_desc(w_addr, 1024, 128), 2048 >> 4, idesc_h, 4u, bar);
+                    }
+                }
             }
         };
         if constexpr (PIPE && L >= 3) {
@@ -186,6 +215,14 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             }
         }
         uint32_t qi;
+        const uint32_t aA = KS ? a0 - 32 : a0;   // KS: input k >= 64 lives at column (k - 64) / 2 of the same A region
+        if constexpr (KS) {
+            mbar_wait(bar, phase);                // the first MMA group has read inputs 0..63
+            phase ^= 1;
+            fence_after_sync();
+#pragma unroll
+            for (int v = 0; v < N_LATE / 4; ++v) tmem_st4(a0 + 4 * v, late[4 * v], late[4 * v + 1], late[4 * v + 2], late[4 * v + 3]);
+        }
         {   // attributes + zero padding up to k1, read late from the staging buffer
             float v[24];
 #pragma unroll
@@ -200,20 +237,21 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             constexpr int c0 = (L * F) / 8;              // first 8-half unit (4 columns) holding attributes
             const uint32_t c_end = M.k1 / 8;
             if constexpr (lead == 0) {
-                tmem_st4(a0 + 4 * c0, pack_half2(v[0], v[1]), pack_half2(v[2], v[3]), pack_half2(v[4], v[5]), pack_half2(v[6], v[7]));
+                tmem_st4(aA + 4 * c0, pack_half2(v[0], v[1]), pack_half2(v[2], v[3]), pack_half2(v[4], v[5]), pack_half2(v[6], v[7]));
             } else {
-                tmem_st2(a0 + 4 * c0 + 2, pack_half2(v[4], v[5]), pack_half2(v[6], v[7]));
+                tmem_st2(aA + 4 * c0 + 2, pack_half2(v[4], v[5]), pack_half2(v[6], v[7]));
             }
             if (c0 + 1 < c_end)
-                tmem_st4(a0 + 4 * (c0 + 1), pack_half2(v[8], v[9]), pack_half2(v[10], v[11]), pack_half2(v[12], v[13]), pack_half2(v[14], v[15]));
+                tmem_st4(aA + 4 * (c0 + 1), pack_half2(v[8], v[9]), pack_half2(v[10], v[11]), pack_half2(v[12], v[13]), pack_half2(v[14], v[15]));
             if (c0 + 2 < c_end)
-                tmem_st4(a0 + 4 * (c0 + 2), pack_half2(v[16], v[17]), pack_half2(v[18], v[19]), pack_half2(v[20], v[21]), pack_half2(v[22], v[23]));
+                tmem_st4(aA + 4 * (c0 + 2), pack_half2(v[16], v[17]), pack_half2(v[18], v[19]), pack_half2(v[20], v[21]), pack_half2(v[22], v[23]));
         }
         if (tile + tile_stride < n_tiles) prefetch(tile + tile_stride);
         // ------------------------------------------------------------------ hidden layers
         uint32_t w_off = 0;
         for (uint32_t layer = 0; layer < M.n_hidden; ++layer) {
             const uint32_t kt_n = (layer == 0 ? M.k1 : 64u) >> 4;
+            const bool second = KS && layer == 0;         // layer 0's inputs 64.. : 4 K-steps further into W0, accumulating
             const bool odd = layer & 1u;
             tmem_wait_st();              // my row of A is in TMEM
             fence_before_sync();
@@ -224,8 +262,8 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
                     w_ready = true;
                 }
                 fence_after_sync();
-                umma_group_ts<8>(tmem_wg + (odd ? 32u : 0u), tmem_wg + (odd ? 0u : 64u), smem_desc(w_addr + w_off, 1024, 128), 2048 >> 4,
-                                 idesc_h, kt_n, bar);
+                umma_group_ts<8>(tmem_wg + (odd ? 32u : 0u), tmem_wg + (odd ? 0u : 64u), smem_desc(w_addr + w_off + (second ? 4u * 2048u : 0u), 1024, 128),
+                                 2048 >> 4, idesc_h, second ? kt_n - 4u : kt_n, bar, second ? 1u : 0u);
             }
             w_off += kt_n * 2 * 1024;
             mbar_wait(bar, phase);
@@ -305,40 +343,38 @@ static bool pipe_applies(const TreeParams& T) {
 }
 #define OO_TM_PIPE_SHAPES(X) X(3, 16, false) X(4, 16, false) X(5, 16, false) X(3, 8, false) X(4, 8, false) X(5, 8, false)
 
-template <int NWG>
-static int launch_tm_nwg(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, uint32_t wg_cols,
-                         bool pipe, cudaStream_t stream) {
+// the two-group first layer (KS) exists where the levels below input 64 fill those 64 inputs exactly
+static bool ks_applies(const TreeParams& T, const MlpParams& M) {
+    return M.k1 > 64 && T.n_levels * T.F >= 64 && T.F % 8 == 0 && 64 % T.F == 0;
+}
+#define OO_TM_KS_SHAPES(X) X(4, 16, false) X(5, 16, false)
+
+template <int NWG, bool PIPE, bool KS>
+static int launch_tm_variant(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, uint32_t wg_cols,
+                             cudaStream_t stream) {
     const uint64_t n_tiles = (Q.n + kRows - 1) / kRows;
     // one block per SM as soon as there is a tile for each: a small batch spreads over all SMs (a warpgroup alone on its SM
     // finishes a tile faster than four sharing one) instead of filling every warpgroup of the first n_tiles / NWG SMs
     const unsigned grid = (unsigned)(n_tiles < (uint64_t)n_sms ? n_tiles : (uint64_t)n_sms);
     const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + NWG * (10 + Q.n_extra) * kRows * 4 + 128;
     if (smem > 227 * 1024) return -1;
-    if (pipe && pipe_applies(T)) {
 #define X(l, f, t)                                                                                                     \
     if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                                            \
         static bool attr = false;                                                                                      \
         if (!attr) {                                                                                                   \
-            cudaFuncSetAttribute(fused_tm_kernel<l, f, t, NWG, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); \
+            cudaFuncSetAttribute(fused_tm_kernel<l, f, t, NWG, PIPE, KS>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); \
             attr = true;                                                                                               \
         }                                                                                                              \
-        fused_tm_kernel<l, f, t, NWG, true><<<grid, NWG * 128, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles, wg_cols); \
+        fused_tm_kernel<l, f, t, NWG, PIPE, KS><<<grid, NWG * 128, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles, wg_cols); \
         return 1;                                                                                                      \
     }
+    if constexpr (KS) {
+        OO_TM_KS_SHAPES(X)
+    } else if constexpr (PIPE) {
         OO_TM_PIPE_SHAPES(X)
-#undef X
+    } else {
+        OO_TM_SHAPES(X)
     }
-#define X(l, f, t)                                                                                                     \
-    if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                                            \
-        static bool attr = false;                                                                                      \
-        if (!attr) {                                                                                                   \
-            cudaFuncSetAttribute(fused_tm_kernel<l, f, t, NWG>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); \
-            attr = true;                                                                                               \
-        }                                                                                                              \
-        fused_tm_kernel<l, f, t, NWG><<<grid, NWG * 128, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles, wg_cols);    \
-        return 1;                                                                                                      \
-    }
-    OO_TM_SHAPES(X)
 #undef X
     return -1;
 }
@@ -350,10 +386,27 @@ int launch_fused_tm(const TreeParams& T, const MlpParams& M, const QueryParams& 
     if (M.out_dim > 4 || !M.image_tc || M.k1 > 128) return -1;
     // Measured on B200 (PIPE against the batched form): config 1 60.2 -> 58.6 us, config 2 55.3 -> 54.5 us, config 3 326 -> 309 us,
     // unsorted incoherent 2^22 queries 1.53 -> 1.32 ms; on binned queries -2 % at 2^22 but +8 % at 2^24, so those keep the batches.
-    const bool pipelined_descent = !binned;
+    const bool pipe = !binned && pipe_applies(T);
+    if (ks_applies(T, M)) {      // 96 columns per tile: five warpgroups
+        const int n = pipe ? launch_tm_variant<5, true, true>(T, M, Q, rgb, n_sms, 96, stream)
+                           : launch_tm_variant<5, false, true>(T, M, Q, rgb, n_sms, 96, stream);
+        if (n >= 0) return n;
+    }
     const uint32_t wg_cols = 64 + (M.k1 / 2 > 32 ? M.k1 / 2 : 32);
-    if (5 * wg_cols <= 512) return launch_tm_nwg<5>(T, M, Q, rgb, n_sms, wg_cols, pipelined_descent, stream);
-    if (4 * wg_cols <= 512) return launch_tm_nwg<4>(T, M, Q, rgb, n_sms, wg_cols, pipelined_descent, stream);
+    if (5 * wg_cols <= 512) {
+        if (pipe) {
+            const int n = launch_tm_variant<5, true, false>(T, M, Q, rgb, n_sms, wg_cols, stream);
+            if (n >= 0) return n;
+        }
+        return launch_tm_variant<5, false, false>(T, M, Q, rgb, n_sms, wg_cols, stream);
+    }
+    if (4 * wg_cols <= 512) {
+        if (pipe) {
+            const int n = launch_tm_variant<4, true, false>(T, M, Q, rgb, n_sms, wg_cols, stream);
+            if (n >= 0) return n;
+        }
+        return launch_tm_variant<4, false, false>(T, M, Q, rgb, n_sms, wg_cols, stream);
+    }
     return -1;
 }
 

@@ -123,11 +123,11 @@ __device__ __forceinline__ void umma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, ui
 // the TS counterpart of umma_group: K-step kt reads A columns a_tmem + 8*kt
 template <int KT_MAX>
 __device__ __forceinline__ void umma_group_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc0, uint32_t b_step16, uint32_t idesc,
-                                              uint32_t kt_n, uint32_t commit_bar) {
+                                              uint32_t kt_n, uint32_t commit_bar, uint32_t first_acc = 0) {
     if (elect_one()) {
 #pragma unroll
         for (uint32_t kt = 0; kt < (uint32_t)KT_MAX; ++kt)
-            if (kt < kt_n) umma_f16_ts(d_tmem, a_tmem + kt * 8, b_desc0 + kt * b_step16, idesc, kt);
+            if (kt < kt_n) umma_f16_ts(d_tmem, a_tmem + kt * 8, b_desc0 + kt * b_step16, idesc, kt | first_acc);
         umma_commit(commit_bar);
     }
     __syncwarp();
