@@ -865,7 +865,7 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
     } else if (p == OO_PATH_FUSED_TC) {
         n = launch_fused_tc(c->T, c->M, Q, d_rgb, c->n_sms, stream);
     } else {
-        n = launch_fused_tm(c->T, c->M, Q, d_rgb, c->n_sms, stream, c->info.presorted_last_query != 0);
+        n = launch_fused_tm(c->T, c->M, Q, d_rgb, c->n_sms, stream);
         if (n < 0 && c->path == OO_PATH_AUTO) {      // e.g. a first layer wider than TMEM allows: try shared-memory A, then mma.sync
             p = OO_PATH_FUSED_TC;
             n = launch_fused_tc(c->T, c->M, Q, d_rgb, c->n_sms, stream);

@@ -380,13 +380,13 @@ static int launch_tm_variant(const TreeParams& T, const MlpParams& M, const Quer
 }
 
 // warpgroups per block = how many column strides fit in the 512 TMEM columns; -1 if the shape has no instance
-int launch_fused_tm(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, cudaStream_t stream,
-                    bool binned) {
+int launch_fused_tm(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, cudaStream_t stream) {
     if (Q.n == 0) return 0;
     if (M.out_dim > 4 || !M.image_tc || M.k1 > 128) return -1;
     // Measured on B200 (PIPE against the batched form): config 1 60.2 -> 58.6 us, config 2 55.3 -> 54.5 us, config 3 326 -> 309 us,
-    // unsorted incoherent 2^22 queries 1.53 -> 1.32 ms; on binned queries -2 % at 2^22 but +8 % at 2^24, so those keep the batches.
-    const bool pipe = !binned && pipe_applies(T);
+    // unsorted incoherent 2^22 queries 1.53 -> 1.32 ms.  Binned queries: mixed with four warpgroups (-2 % at 2^22, +8 % at 2^24),
+    // a gain at every size once KS runs five (2^22 0.657 -> 0.632 ms, 2^24 2.40 -> 2.22 ms), so PIPE is used wherever it applies.
+    const bool pipe = pipe_applies(T);
     if (ks_applies(T, M)) {      // 96 columns per tile: five warpgroups
         const int n = pipe ? launch_tm_variant<5, true, true>(T, M, Q, rgb, n_sms, 96, stream)
                            : launch_tm_variant<5, false, true>(T, M, Q, rgb, n_sms, 96, stream);

@@ -115,7 +115,7 @@ int launch_fused_tc(const TreeParams& T, const MlpParams& M, const QueryParams& 
 bool fast_shape_supported(uint32_t L, uint32_t F, bool f32);
 bool tc_shape_supported(uint32_t L, uint32_t F, bool f32);
 int launch_fused_tm(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
-                    cudaStream_t stream, bool binned = false);
+                    cudaStream_t stream);
 bool tm_shape_supported(uint32_t L, uint32_t F, bool f32);
 // full query (oo_full_*.cu)
 struct FullModeH { uint32_t tri8, lookup, attrs_paper; };
