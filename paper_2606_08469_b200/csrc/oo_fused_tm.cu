@@ -156,39 +156,7 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             }
         };
         if constexpr (PIPE && L >= 3) {
-            const int qmax = (int)(1u << T.depth_eff) - 1;
-            const int qx = quantise(x[0], T.scale_eff, qmax), qy = quantise(x[1], T.scale_eff, qmax), qz = quantise(x[2], T.scale_eff, qmax);
-            const OctaUV uv = octa_project(w[0], w[1], w[2]);
-            auto dense_at = [&](uint32_t off, uint32_t d, uint32_t sh) {
-                return s_dense[off + (((qz >> sh) << (2 * d)) | ((qy >> sh) << d) | (qx >> sh))];
-            };
-            auto hop_load = [&](const LevelParams& lv, int prev) {
-                const uint32_t sh = lv.shift, g = lv.gap, m = (1u << g) - 1u;
-                const uint32_t idx = ((((uint32_t)qz >> sh) & m) << (2 * g)) | ((((uint32_t)qy >> sh) & m) << g) | (((uint32_t)qx >> sh) & m);
-                return prev >= 0 ? __ldg(lv.hop + (((size_t)prev << (3 * g)) + idx)) : -1;
-            };
-            constexpr int RD = (F * (F32 ? 4 : 2) == 16 && L >= 4) ? 3 : 2;      // levels of taps in flight (16-byte texels: 2 -> 58.7, 3 -> 58.2, 4 -> 60.2 us on config 1)
-            TapSet<F, F32> ring[RD];
-            int hv = hop_load(T.lv[2], dense_at(T.t_dense_off, T.t_depth, T.t_shift));
-            issue_taps<F, F32>(T.lv[0], dense_at(T.lv[0].dense_off, T.lv[0].depth, T.lv[0].shift), uv, ring[0]);
-            issue_taps<F, F32>(T.lv[1], dense_at(T.lv[1].dense_off, T.lv[1].depth, T.lv[1].shift), uv, ring[1]);
-#pragma unroll
-            for (int l = 2; l < L; ++l) {
-                const int slot = hv;
-                if (l + 1 < L) hv = hop_load(T.lv[l + 1], slot);
-                if (l >= RD) {
-                    float h[F];
-                    consume_taps<F, F32>(ring[l % RD], h);
-                    store_level(l - RD, h);
-                }
-                issue_taps<F, F32>(T.lv[l], slot, uv, ring[l % RD]);
-            }
-#pragma unroll
-            for (int l = L - RD; l < L; ++l) {
-                float h[F];
-                consume_taps<F, F32>(ring[l % RD], h);
-                store_level(l, h);
-            }
+            gather_pipelined<L, F, F32>(T, s_dense, x, w, store_level);
         } else {
             Encoded<L, F, F32> e;
             locate<L, F, F32>(T, s_dense, x, w, e);
@@ -333,14 +301,6 @@ bool tm_shape_supported(uint32_t L, uint32_t F, bool f32) {
     return false;
 }
 
-// the pipelined descent exists for 32-byte texels (two levels per load batch otherwise) on trees whose first two used levels
-// are dense and every later one a hop
-static bool pipe_applies(const TreeParams& T) {
-    if (T.n_levels < 3 || T.f32 || !T.lv[0].dense || !T.lv[1].dense) return false;
-    for (uint32_t l = 2; l < T.n_levels; ++l)
-        if (T.lv[l].dense) return false;
-    return true;
-}
 #define OO_TM_PIPE_SHAPES(X) X(3, 16, false) X(4, 16, false) X(5, 16, false) X(3, 8, false) X(4, 8, false) X(5, 8, false)
 
 // the two-group first layer (KS) exists where the levels below input 64 fill those 64 inputs exactly

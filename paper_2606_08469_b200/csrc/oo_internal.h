@@ -112,6 +112,14 @@ int launch_fused_mma(const TreeParams& T, const MlpParams& M, const QueryParams&
                      cudaStream_t stream);
 int launch_fused_tc(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
                     cudaStream_t stream);
+// The pipelined descent (gather_pipelined, oo_device.cuh) exists for fp16 trees whose first two used levels are dense and every
+// later one a hop, i.e. the BASELINE.json configs.
+inline bool pipe_applies(const TreeParams& T) {
+    if (T.n_levels < 3 || T.f32 || !T.lv[0].dense || !T.lv[1].dense) return false;
+    for (uint32_t l = 2; l < T.n_levels; ++l)
+        if (T.lv[l].dense) return false;
+    return true;
+}
 bool fast_shape_supported(uint32_t L, uint32_t F, bool f32);
 bool tc_shape_supported(uint32_t L, uint32_t F, bool f32);
 int launch_fused_tm(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
