@@ -29,7 +29,13 @@ UNIT = "Mqueries/s"
 
 def workload_for(cfg: int, rank: int = 0):
     import gen
-    w = gen.scene_workload(cfg, seed=0)
+    if cfg == 4:
+        # BASELINE.json configs[4], the incoherent distribution at 2^22 queries: config 3's scene, tree, atlas and MLP; queries =
+        # area-weighted surface samples in random order (the batch-size x distribution table is --sweep 4)
+        w = gen.scene_workload(3, seed=0, width=64, height=64, incoherent_n=1 << 22)
+        w.meta["width"], w.meta["height"], w.meta["incoherent"] = 2048, 2048, True   # width/height only cut the CPU oracle's sample into index ranges
+    else:
+        w = gen.scene_workload(cfg, seed=0)
     L, F = len(w.tree.level_depth), w.atlas.F
     n_extra = 0 if w.queries.extra is None else w.queries.extra.shape[1]
     texel = F * 2
@@ -38,9 +44,11 @@ def workload_for(cfg: int, rank: int = 0):
     dims = [w.mlp.in_dim] + [64] * w.mlp.n_hidden + [3]
     flops = 2 * sum(a * b for a, b in zip(dims[:-1], dims[1:]))
     desc = {
-        "workload": "BASELINE.json configs[%d]: %dx%d primary-hit frame (%d queries, scanline order), adaptive octree depth %d "
+        "workload": "BASELINE.json configs[%d]: %s (%d queries, %s), adaptive octree depth %d "
                     "(%d nodes), used depths %s, R_l %s, F=%d fp16, MLP %d->%dx64->3 exp" %
-                    (cfg, w.meta["width"], w.meta["height"], w.queries.n, w.tree.max_depth, w.tree.n_nodes,
+                    (cfg, "incoherent queries on the config-3 cache: x area-weighted on the scene surfaces, wo uniform on the hemisphere" if cfg == 4
+                     else "%dx%d primary-hit frame" % (w.meta["width"], w.meta["height"]), w.queries.n,
+                     "random order" if cfg == 4 else "scanline order", w.tree.max_depth, w.tree.n_nodes,
                      w.tree.level_depth, w.tree.level_res, F, w.mlp.in_dim, w.mlp.n_hidden),
         "queries_per_step": w.queries.n, "bytes_per_query": gather + io, "gather_bytes_per_query": gather,
         "flop_per_query": flops, "atlas_bytes": w.atlas.nbytes,
@@ -97,6 +105,8 @@ def oracle_sample(w, target_queries: int):
     stride = max(1, H // rows)
     ridx = np.arange(0, H, stride)[:rows]
     idx = (ridx[:, None] * W + np.arange(W)[None, :]).ravel()
+    if w.meta.get("incoherent"):
+        return w.queries.take(idx), "%d queries = %d runs of %d consecutive queries (every %dth run) of the random-order batch" % (len(idx), len(ridx), W, stride)
     return w.queries.take(idx), "%d queries = %d scanlines (every %dth row) of the %dx%d frame" % (len(idx), len(ridx), stride, W, H)
 
 
@@ -161,6 +171,8 @@ def run_ours(args):
     ctx = P.OctaOctree(local_rank).upload_workload(w)
     path = {"auto": P.PATH_AUTO, "mma": P.PATH_FUSED_MMA, "tc": P.PATH_FUSED_TC, "tm": P.PATH_FUSED_TC_TMEM, "unfused": P.PATH_UNFUSED, "generic": P.PATH_GENERIC}[args.path]
     ctx.oo_set_path(path)
+    if args.presort is None:
+        args.presort = "bin" if args.config == 4 else "none"
     ctx.oo_set_presort(args.presort)
     ctx.oo_reserve(q.n)
     cu = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
@@ -249,7 +261,8 @@ def run_ours(args):
                 "d2h_bytes_per_step": int(12 * q.n), "ms_per_step": mx_e2e, "api": "oo_query_host (pinned host buffers)", "checksum": checksum},
         "gpu_launches": int(launches),
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm, "traffic": traffic,
-                     "peak_source": which, "kernel": "fused encode+MLP (one launch per step)",
+                     "peak_source": which, "kernel": "fused encode+MLP (one launch per step)" if args.presort == "none" else
+                     "whole step: histogram + scan + bin_scatter + fused encode+MLP on the binned copy + unbin (the fused launch is ~3/4 of it; traffic is that launch's)",
                      "roofline_ms": max(byte_time, flop_time) * 1e3, "flop_time_ms": flop_time * 1e3, "byte_time_ms": byte_time * 1e3,
                      "frac_warm_l2": desc["bytes_per_query"] * q.n / (warm_ms * 1e-3) / 1e9 / hbm},
     }
@@ -552,7 +565,7 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=1, choices=[1, 2, 3])
+    ap.add_argument("--config", type=int, default=1, choices=[1, 2, 3, 4], help="BASELINE.json configs[k]; 4 = its incoherent distribution at 2^22 queries")
     ap.add_argument("--path", default="auto", choices=["auto", "mma", "tc", "tm", "unfused", "generic"])
     ap.add_argument("--ref-sample", type=int, default=1 << 22, help="queries in the cpu_baseline sample (capped at the frame)")
     ap.add_argument("--ref-budget", type=float, default=90.0, help="--impl reference: seconds of CPU work the W + K steps may take")
@@ -561,7 +574,7 @@ def main():
     ap.add_argument("--sweep-max-log2", type=int, default=24)
     ap.add_argument("--sweep-min-log2", type=int, default=16)
     ap.add_argument("--sweep-dist", default="both", choices=["both", "coherent", "incoherent"])
-    ap.add_argument("--presort", default="none", choices=["none", "bin"], help="oo_set_presort for the headline run")
+    ap.add_argument("--presort", default=None, choices=["none", "bin"], help="oo_set_presort for the run (default: bin for --config 4, none otherwise)")
     ap.add_argument("--quick", action="store_true", help="timed region only (no warm-L2 / e2e / CPU legs): the command ncu wraps")
     args = ap.parse_args()
     if args.sweep == 8:
