@@ -72,22 +72,8 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
         mbar_expect_tx(bar_w, M.image_tc_bytes);
         bulk_g2s(smem_u32(s_w), M.image_tc, M.image_tc_bytes, bar_w);
     }
-    if (warp == 0) {
-        tmem_alloc(smem_u32(s_tmem), 512);
-        tmem_relinquish();
-    }
-    fence_before_sync();
-    __syncthreads();
-    fence_after_sync();
-    const uint32_t tmem_wg = *s_tmem + wg * wg_cols;                 // this warpgroup's columns
-    const uint32_t tmem_lane = tmem_wg + ((row & ~31u) << 16);       // ... and this warp's 32 lanes
     float* s_q = (float*)(s_stage + wg * q_bytes) + row;             // word k of my row: s_q[k * 128]
-    const uint32_t w_addr = smem_u32(s_w), bar = smem_u32(&s_bar[wg]), q_addr = smem_u32(s_q);
-    uint32_t phase = 0;
-    const bool leader_warp = row < 32;
-    constexpr uint32_t idesc_h = instr_desc(128, 64), idesc_o = instr_desc(128, 16);
-    const uint32_t tile_stride = gridDim.x * NWG;
-
+    const uint32_t q_addr = smem_u32(s_q);
     auto prefetch = [&](uint32_t tile) {
         const uint64_t t = (uint64_t)tile * kRows + row;
         const uint64_t tt = t < Q.n ? t : Q.n - 1;
@@ -110,7 +96,22 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
     // round then land one per SM (a lone warpgroup finishes its tile about twice as fast as five sharing an SM) instead of five
     // per SM on a few SMs.  Measured on B200: config 1 61.1 -> 60.1 us, config 3 333.3 -> 329.4 us.
     uint32_t tile = wg * gridDim.x + blockIdx.x;
-    if (tile < n_tiles) prefetch(tile);
+    if (tile < n_tiles) prefetch(tile);       // the first tile's queries travel while TMEM is allocated and the tables arrive
+    if (warp == 0) {
+        tmem_alloc(smem_u32(s_tmem), 512);
+        tmem_relinquish();
+    }
+    fence_before_sync();
+    __syncthreads();
+    fence_after_sync();
+    const uint32_t tmem_wg = *s_tmem + wg * wg_cols;                 // this warpgroup's columns
+    const uint32_t tmem_lane = tmem_wg + ((row & ~31u) << 16);       // ... and this warp's 32 lanes
+    const uint32_t w_addr = smem_u32(s_w), bar = smem_u32(&s_bar[wg]);
+    uint32_t phase = 0;
+    const bool leader_warp = row < 32;
+    constexpr uint32_t idesc_h = instr_desc(128, 64), idesc_o = instr_desc(128, 16);
+    const uint32_t tile_stride = gridDim.x * NWG;
+
     mbar_wait(bar_d, 0);                  // descent tables in shared memory
     bool w_ready = false;
     for (; tile < n_tiles; tile += tile_stride) {
