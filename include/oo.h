@@ -108,7 +108,8 @@ typedef enum {
  *   kernel path over the binned copy, and a last kernel brings the RGB back to the caller's order.  Results are
  *   bit-identical to OO_PRESORT_NONE (queries are independent); what changes is which atlas pages the thread blocks touch
  *   at a time.  For incoherent queries out of an HBM-resident cache (configs[4]); screen-order frames are coherent already.
- *   Takes effect on the hot path (not the full query) when queries.perm is NULL and n >= min_queries of oo_set_presort (default 262144:
+ *   Takes effect (hot path and full query alike; a supplied queries.disparity moves with its query, a predicted one is
+ *   predicted on the binned copy) when queries.perm is NULL and n >= min_queries of oo_set_presort (default 262144:
  *   below that the extra launches cost more than they save); otherwise the call proceeds in the given order (oo_info.presorted_last_query says
  *   which).  oo_encode on OO_PATH_UNFUSED does the same with x and wo and stores every feature row at its query's index
  *   (oo_info.presorted_last_encode).  Needs oo_reserve(n). */

@@ -65,7 +65,7 @@ struct oo_ctx {
     uint64_t bin_min = 1u << 18;           // batches below this proceed unsorted (the extra launches cost more than they save)
     float *d_bx = nullptr, *d_bn = nullptr, *d_bw = nullptr, *d_be = nullptr;
     uint32_t *d_binv = nullptr, *d_bidx = nullptr;
-    float* d_brgb = nullptr;
+    float *d_brgb = nullptr, *d_bdisp = nullptr;
     uint64_t bin_rows = 0;
 
     // oo_query_host pipeline: copy-in and copy-out streams beside the caller's stream, one event pair per chunk
@@ -133,7 +133,7 @@ void free_scratch(oo_ctx* c) {
     void** ps[] = {(void**)&c->d_keys_a, (void**)&c->d_keys_b, (void**)&c->d_idx_a, (void**)&c->d_hist, (void**)&c->d_qx,
                    (void**)&c->d_qn,     (void**)&c->d_qw,     (void**)&c->d_qe,    (void**)&c->d_rgb, (void**)&c->d_qd};
     for (void** p : ps) free_dev(*p);
-    void** bs[] = {(void**)&c->d_bx, (void**)&c->d_bn, (void**)&c->d_bw, (void**)&c->d_be, (void**)&c->d_binv, (void**)&c->d_bidx, (void**)&c->d_brgb};
+    void** bs[] = {(void**)&c->d_bx, (void**)&c->d_bn, (void**)&c->d_bw, (void**)&c->d_be, (void**)&c->d_binv, (void**)&c->d_bidx, (void**)&c->d_brgb, (void**)&c->d_bdisp};
     for (void** p : bs) free_dev(*p);
     c->bin_rows = 0;
     c->reserved = 0;
@@ -672,7 +672,7 @@ static oo_status ensure_feat(oo_ctx* c, uint64_t bytes) {
 static oo_status ensure_bin(oo_ctx* c, uint64_t n) {
     if (n > c->reserved) return fail(c, OO_ERR_NOT_READY, "OO_PRESORT_BIN: call oo_reserve(%llu) first", (unsigned long long)n);
     if (c->bin_rows >= n) return OO_OK;
-    void** bs[] = {(void**)&c->d_bx, (void**)&c->d_bn, (void**)&c->d_bw, (void**)&c->d_be, (void**)&c->d_binv, (void**)&c->d_bidx, (void**)&c->d_brgb};
+    void** bs[] = {(void**)&c->d_bx, (void**)&c->d_bn, (void**)&c->d_bw, (void**)&c->d_be, (void**)&c->d_binv, (void**)&c->d_bidx, (void**)&c->d_brgb, (void**)&c->d_bdisp};
     for (void** b : bs) free_dev(*b);
     c->bin_rows = 0;
     const uint64_t rows = c->reserved;
@@ -683,7 +683,24 @@ static oo_status ensure_bin(oo_ctx* c, uint64_t n) {
     OO_CUDA(c, cudaMalloc((void**)&c->d_binv, rows * 4));
     OO_CUDA(c, cudaMalloc((void**)&c->d_bidx, rows * 4));
     OO_CUDA(c, cudaMalloc((void**)&c->d_brgb, rows * 4 * 8));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_bdisp, rows * 4));
     c->bin_rows = rows;
+    return OO_OK;
+}
+
+// a1' for oo_query: one counting pass on the top Morton bits moves the queries (and a caller-supplied d^) into the binned
+// scratch; *qb then describes the binned copy.  The chosen kernel runs over it into c->d_brgb and unbin restores the order.
+static bool bin_wanted(const oo_ctx* c, const oo_queries* q) {
+    return c->presort == OO_PRESORT_BIN && !q->perm && q->n >= c->bin_min;
+}
+static oo_status bin_for_query(oo_ctx* c, const oo_queries* q, oo_queries* qb, cudaStream_t stream) {
+    if (oo_status st = ensure_bin(c, q->n)) return st;
+    count(c, launch_bin_queries(make_qp(q), c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, nullptr,
+                                q->disparity ? c->d_bdisp : nullptr, stream));
+    *qb = *q;
+    qb->x = c->d_bx; qb->nrm = c->d_bn; qb->wo = c->d_bw;
+    qb->extra = q->n_extra && q->extra ? c->d_be : nullptr;
+    qb->disparity = q->disparity ? c->d_bdisp : nullptr;
     return OO_OK;
 }
 
@@ -729,7 +746,7 @@ extern "C" OO_API oo_status oo_encode(oo_ctx* c, const oo_queries* q, void* d_fe
         // a1': x and wo move into Morton bins; the encode kernel reads them in order and stores every row at its query's index
         if (oo_status st = ensure_bin(c, q->n)) return st;
         Q.nrm = nullptr; Q.extra = nullptr; Q.n_extra = 0;
-        count(c, launch_bin_queries(Q, c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, c->d_bidx, (cudaStream_t)cuda_stream));
+        count(c, launch_bin_queries(Q, c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, c->d_bidx, nullptr, (cudaStream_t)cuda_stream));
         Q.x = c->d_bx; Q.wo = c->d_bw; Q.out_idx = c->d_bidx;
         c->info.presorted_last_encode = 1;
     }
@@ -818,12 +835,20 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
         if (q->n == 0) return OO_OK;
         c->M.feat_dim = feat;
         oo_queries qd = *q;
+        float* out = d_rgb;
+        c->info.presorted_last_query = 0;
+        if (bin_wanted(c, q)) {      // bin first: the predictor's hash-grid gathers profit from the order too
+            if (oo_status st = bin_for_query(c, q, &qd, stream)) return st;
+            out = c->d_brgb;
+            c->info.presorted_last_query = 1;
+        }
         if (oo_status st = fill_disparity(c, &qd, stream)) return st;
         const QueryParams Q = make_qp(&qd);
-        const int n = c->M.width == 64 ? launch_fused_full_w64(c->T, c->M, Q, c->mode, d_rgb, c->n_sms, stream)
-                                       : launch_fused_full_w128(c->T, c->M, Q, c->mode, d_rgb, c->n_sms, stream);
+        const int n = c->M.width == 64 ? launch_fused_full_w64(c->T, c->M, Q, c->mode, out, c->n_sms, stream)
+                                       : launch_fused_full_w128(c->T, c->M, Q, c->mode, out, c->n_sms, stream);
         if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "no full-query kernel for F=%u %s, in_dim %u, out_dim %u", c->T.F, c->T.f32 ? "fp32" : "fp16", c->M.in_dim, c->M.out_dim);
         count(c, n);
+        if (c->info.presorted_last_query) count(c, launch_unbin(c->d_brgb, c->d_binv, q->n, c->M.out_dim, d_rgb, c->n_sms, stream));
         c->info.path_last_query = (uint32_t)OO_PATH_FULL;
         return check_async(c);
     }
@@ -841,12 +866,10 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
     int n = 0;
     float* const d_out = d_rgb;
     c->info.presorted_last_query = 0;
-    if (c->presort == OO_PRESORT_BIN && !q->perm && q->n >= c->bin_min) {
-        // a1': one radix pass on the top Morton bits moves the queries into the binned scratch; whichever kernel path was
-        // chosen then runs over the binned copy into binned RGB, and unbin_kernel restores the caller's order
-        if (oo_status st = ensure_bin(c, q->n)) return st;
-        count(c, launch_bin_queries(Q, c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, nullptr, stream));
-        Q.x = c->d_bx; Q.nrm = c->d_bn; Q.wo = c->d_bw; Q.extra = q->n_extra ? c->d_be : nullptr;
+    if (bin_wanted(c, q)) {
+        oo_queries qb;
+        if (oo_status st = bin_for_query(c, q, &qb, stream)) return st;
+        Q = make_qp(&qb);
         d_rgb = c->d_brgb;
         c->info.presorted_last_query = 1;
     }

@@ -143,7 +143,7 @@ int launch_morton_sort(const float* x, uint64_t n, uint32_t* keys_a, uint32_t* k
                        uint32_t* hist, cudaStream_t stream);
 size_t morton_sort_hist_ints(uint64_t n);
 int launch_bin_queries(const QueryParams& Q, uint32_t* keys, uint32_t* hist, float* sx, float* sn, float* sw, float* se,
-                       uint32_t* inv, uint32_t* idx, cudaStream_t stream);
+                       uint32_t* inv, uint32_t* idx, float* sdisp, cudaStream_t stream);
 int launch_unbin(const float* binned, const uint32_t* inv, uint64_t n, uint32_t out_dim, float* out, int n_sms, cudaStream_t stream);
 
 }  // namespace oo

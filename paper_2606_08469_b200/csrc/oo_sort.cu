@@ -217,6 +217,8 @@ struct BinPayload {
     uint32_t n_extra;
     float *sx, *sn, *sw, *se;
     uint32_t* idx;                       // optional: idx[binned position] = query index (oo_encode stores rows at it)
+    const float* disp;                   // optional per-query disparity d^ (full query, OO_LOOKUP_SHIFTED) and its binned copy
+    float* sdisp;
 };
 constexpr int kBinThreads = 512;
 constexpr int kBinItems = kTile / kBinThreads;      // 8 queries per thread
@@ -331,6 +333,8 @@ __global__ void __launch_bounds__(kBinThreads, 1) bin_scatter_kernel(const uint3
     }
     if (B.idx)
         for (uint32_t p = tid; p < tile_n; p += kBinThreads) B.idx[s_dst[p]] = (uint32_t)tile_base + s_src[p];
+    if (B.disp)
+        for (uint32_t p = tid; p < tile_n; p += kBinThreads) B.sdisp[s_dst[p]] = __ldg(B.disp + tile_base + s_src[p]);
     if (B.n_extra) {   // extras: gathered straight from the tile's own rows, written in runs
         const uint32_t ne = B.n_extra, nfe = tile_n * ne;
         for (uint32_t f = tid; f < nfe; f += kBinThreads) {
@@ -359,7 +363,7 @@ __global__ void __launch_bounds__(256) unbin_kernel(const float* __restrict__ bi
 }
 
 int launch_bin_queries(const QueryParams& Q, uint32_t* keys, uint32_t* hist, float* sx, float* sn, float* sw, float* se,
-                       uint32_t* inv, uint32_t* idx, cudaStream_t stream) {
+                       uint32_t* inv, uint32_t* idx, float* sdisp, cudaStream_t stream) {
     if (Q.n == 0) return 0;
     static bool attr = false;
     if (!attr) {
@@ -372,7 +376,7 @@ int launch_bin_queries(const QueryParams& Q, uint32_t* keys, uint32_t* hist, flo
     constexpr uint32_t shift = 30 - kBits;
     radix_hist_kernel<true, 1024><<<n_tiles, 1024, 0, stream>>>(Q.x, keys, Q.n, shift, n_tiles, hist, tot);
     scan_kernel<<<kDigits, kSortThreads, 0, stream>>>(hist, tot, n_tiles);
-    const BinPayload B{Q.x, Q.nrm, Q.wo, Q.extra, Q.extra ? Q.n_extra : 0u, sx, sn, sw, se, idx};
+    const BinPayload B{Q.x, Q.nrm, Q.wo, Q.extra, Q.extra ? Q.n_extra : 0u, sx, sn, sw, se, idx, sdisp ? Q.disparity : nullptr, sdisp};
     bin_scatter_kernel<<<n_tiles, kBinThreads, kBinSmemBytes, stream>>>(keys, Q.n, shift, n_tiles, hist, B, inv);
     return 3;
 }

@@ -175,6 +175,18 @@ def test_incoherent_queries_and_perm(P):
     b = ctx.oo_query(x, n, wo, ex, perm=perm, disparity=dd)
     torch.cuda.synchronize()
     assert torch.equal(a, b)
+    # OO_PRESORT_BIN moves the queries (the supplied d^ with them) into Morton bins in front of the full-query kernel too
+    ctx.oo_reserve(q.n)
+    ctx.oo_set_presort("bin", min_queries=1)
+    c = ctx.oo_query(x, n, wo, ex, disparity=dd)
+    assert ctx.oo_get_info()["presorted_last_query"] == 1 and torch.equal(a, c)
+    # ... and in front of the predictor when the query predicts d^ itself
+    net = gen.make_disparity_net(0)
+    ctx.oo_upload_disparity(net.res, net.hash_log2, net.tables, net.weights)
+    e = ctx.oo_query(x, n, wo, ex)
+    assert ctx.oo_get_info()["presorted_last_query"] == 1
+    ctx.oo_set_presort("none")
+    assert torch.equal(e, ctx.oo_query(x, n, wo, ex))
     ctx.close()
 
 
