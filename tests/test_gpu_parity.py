@@ -122,6 +122,24 @@ def test_non_canonical_levels_fall_back_to_generic(P):
     _run_all(P, w, f, s, t, rgb, expect_fast=False)
 
 
+@pytest.mark.parametrize("depths,res,F,H", [([2, 3, 4, 6], [16, 16, 8, 4], 8, 2), ([2, 3, 4, 6, 8], [16, 8, 8, 4, 4], 16, 4),
+                                            ([1, 2, 4, 5, 7], [8, 8, 8, 4, 2], 16, 3), ([3, 6, 8], [8, 8, 4], 8, 2)])
+def test_other_dense_hop_patterns_use_the_batched_gather(P, depths, res, F, H):
+    """Trees whose used levels are not 'two dense levels, then hops' (three dense levels in front of the hops, or only one):
+    the pipelined descent does not apply, so the tcgen05 paths run the batched gather -- for F = 16 and L*F >= 64 together
+    with the two-group first layer.  All paths against the oracle."""
+    scene = gen.make_scene("three", 2)
+    tree = gen.build_tree(scene, depths[-1]).set_levels(depths, res)
+    atlas = gen.make_atlas(tree, F, "f16", 2)
+    mlp = gen.make_mlp(len(depths) * F + 6, H, 2)
+    cam = gen.make_camera(112, 80, 2)
+    w = gen.Workload("pattern", tree, atlas, mlp, gen.raycast(scene, cam), scene, cam)
+    co = OC.from_workload(w)
+    q = w.queries
+    f, s, t = co.encode(q.x, q.wo)
+    _run_all(P, w, f, s, t, co.query(q.x, q.nrm, q.wo))
+
+
 def test_unspecialised_shape_falls_back_to_generic(P):
     """L=6 levels of F=8 has no template instance: AUTO -> generic; also out_act = none and out_dim = 5."""
     tree = gen.build_tree(None, 3, uniform=True)
