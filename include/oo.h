@@ -23,8 +23,14 @@
  *     stream has completed.  A second upload replaces the first.
  *   - Query and output buffers are owned by the caller.  Kernels are enqueued on the caller's stream (a cudaStream_t
  *     passed as void*; NULL = the legacy default stream) and the call returns without synchronising, except where
- *     stated.  Hot calls never allocate (call oo_reserve first if you use oo_sort_queries / oo_query_host).
- *   - Every call returns oo_status; nothing throws.  oo_last_error() describes the last failure on that context.
+ *     stated.  Hot calls never allocate: whatever scratch a call needs comes from oo_reserve (oo_sort_queries,
+ *     oo_query_host, OO_PRESORT_BIN, OO_PATH_GENERIC / OO_PATH_UNFUSED, disparity prediction); a call that finds it
+ *     missing returns OO_ERR_NOT_READY and launches nothing.
+ *   - Every call returns oo_status; nothing throws.  oo_last_error() describes the last failure on that context.  A
+ *     failed call leaves the context usable unless the CUDA context itself is lost (illegal address, launch failure,
+ *     ...: every later call then fails at once with OO_ERR_CUDA).  A non-fatal CUDA error that some other code left
+ *     pending on the calling thread is cleared by the next oo_ call that launches (it is not this library's to report).
+ *   - One context per device; several contexts, on the same or on different devices, may live in one process.
  *   - Not checked per query (result undefined, never a crash): non-finite inputs, wo = 0.  x outside [0,1]^3 is
  *     clamped componentwise (A16).
  *   - There is no CPU fallback: without a usable CUDA device oo_create fails.
@@ -144,10 +150,12 @@ typedef struct {
     uint32_t in_dim;
     uint32_t width;              /* 64, or 128 (the paper's decoder; runs on the full-query kernels) */
     uint32_t n_hidden;           /* 1..OO_MAX_HIDDEN */
-    uint32_t out_dim;            /* 1..8 (3 = RGB) */
-    const void* const* weights;  /* HOST array [n_hidden+1] of HOST pointers to fp16 matrices:
+    uint32_t out_dim;            /* 1..8 (3 = RGB); the full-query kernels: 1..4 */
+    const void* const* weights;  /* HOST array [n_hidden+1] of pointers to fp16 matrices:
                                     [width][in_dim], (n_hidden-1) x [width][width], [out_dim][width] */
     oo_out_act out_act;
+    uint32_t weights_on_device;  /* 0: weights[k] are HOST pointers; 1: DEVICE pointers on the context's device (e.g. a
+                                    trainer's parameters), read on the upload stream */
 } oo_mlp_desc;
 
 /* A batch of queries.  All arrays packed fp32.  For oo_encode / oo_query / oo_sort_queries they are DEVICE pointers,
@@ -194,6 +202,9 @@ typedef struct {
     uint32_t n_sms;
     uint32_t presorted_last_query; /* 1 if the last oo_query ran on binned queries (OO_PRESORT_BIN took effect) */
     uint32_t presorted_last_encode; /* the same for the last oo_encode */
+    uint32_t full_query;         /* 1 if oo_query runs the full-query kernel under the current tree / mode / decoder
+                                    (mode != 0, vertex maps or width 128), i.e. oo_query_debug's outputs are [n][L][J]... */
+    uint32_t n_neighbours;       /* J of the current mode: 8 (OO_SPATIAL_TRILINEAR8) or 1 */
 } oo_info;
 
 /* Create a context on a CUDA device.  Fails with OO_ERR_CUDA if the device is absent or is not compute capability
@@ -202,6 +213,10 @@ OO_API oo_status oo_create(oo_ctx** out, int cuda_device);
 OO_API void oo_destroy(oo_ctx* ctx);
 /* Message for the last non-OK status on ctx (valid until the next call on ctx); "" if none. */
 OO_API const char* oo_last_error(const oo_ctx* ctx);
+/* Informational, never an error: when the last oo_query resolved OO_PATH_AUTO to anything slower than the fused
+ * tensor-memory kernel (a shape without such an instance, a tree without a hop plan, ...) this says to what and for which
+ * shape; "" otherwise.  Valid until the next call on ctx. */
+OO_API const char* oo_last_note(const oo_ctx* ctx);
 
 /* Validate the tree (child indices in range and one level deeper, depth consistent, map_slot unique per level and
  * < level_slots), build the descent tables, and copy every atlas into library-owned border-padded maps
@@ -209,7 +224,10 @@ OO_API const char* oo_last_error(const oo_ctx* ctx);
 OO_API oo_status oo_upload_tree(oo_ctx* ctx, const oo_tree_desc* tree, void* cuda_stream);
 /* Copy the decoder weights into the library's padded shared-memory image.  Synchronises the stream. */
 OO_API oo_status oo_upload_mlp(oo_ctx* ctx, const oo_mlp_desc* mlp, void* cuda_stream);
-/* Pre-allocate scratch for up to max_queries (sort keys/buffers, staging for oo_query_host). */
+/* Pre-allocate every scratch buffer a hot call may need for up to max_queries queries: sort keys, staging for
+ * oo_query_host, the binned copy of OO_PRESORT_BIN (about 250 bytes per query in all), and, sized from the uploaded tree,
+ * the feature rows of OO_PATH_GENERIC / OO_PATH_UNFUSED (L * texel bytes per query): call it after oo_upload_tree, and
+ * again after uploading a tree with wider feature rows.  Never shrinks.  OO_ERR_OOM leaves the context usable. */
 OO_API oo_status oo_reserve(oo_ctx* ctx, uint64_t max_queries);
 /* Select the kernels used from now on (default OO_PATH_AUTO).  OO_ERR_UNSUPPORTED at query time if the uploaded
  * shapes have no such kernel. */
@@ -250,12 +268,27 @@ OO_API oo_status oo_encode_full(oo_ctx* ctx, const oo_queries* q, float* d_featu
  * launch as well). */
 OO_API oo_status oo_query(oo_ctx* ctx, const oo_queries* q, float* d_rgb, void* cuda_stream);
 
-/* The whole path from HOST buffers, as a chunked three-stage pipeline: the queries are split into up to 4 chunks
- * (environment variable OO_HOST_CHUNKS = 1..16 overrides the count;
- * whole 128-query tiles, at least 65,536 queries each); chunk i+1 is copied to the device on a library-owned copy-in
+/* oo_query that also reports which cell and which texels every query read -- from inside the very kernels oo_query
+ * runs: every fused kernel has a second, compile-time instance whose gather code hands the atlas slot and the base texel
+ * to an index sink at the point where it forms the texel address; this call selects those instances (same descent, same
+ * address arithmetic, same RGB bit for bit; slower by the extra stores).  It exists so that BASELINE.json's "node indices
+ * and texel indices bit-exact" can be checked on the timed kernels themselves rather than on oo_encode's.
+ * Hot path: d_slot DEVICE [n][L], d_index DEVICE [n][L][2] = (i0, j0), as oo_encode.  Full query (mode != 0, vertex maps or
+ * width 128): d_slot [n][L][J], d_index [n][L][J][3], as oo_encode_full.  Either may be NULL.  Rows land at the query's
+ * own index whatever the processing order (perm, OO_PRESORT_BIN). */
+OO_API oo_status oo_query_debug(oo_ctx* ctx, const oo_queries* q, float* d_rgb, int32_t* d_slot, int16_t* d_index,
+                         void* cuda_stream);
+
+/* Number of chunks oo_query_host splits a batch into: 1..16, or 0 (default) = chosen from the batch size (one chunk
+ * below 131,072 queries, else about 262,144 queries per chunk, 2..8 chunks). */
+OO_API oo_status oo_set_host_chunks(oo_ctx* ctx, uint32_t n_chunks);
+
+/* The whole path from HOST buffers, as a chunked three-stage pipeline: the queries are split into chunks of whole
+ * 128-query tiles (see oo_set_host_chunks); chunk i+1 is copied to the device on a library-owned copy-in
  * stream while oo_query runs chunk i on the caller's stream and chunk i-1's RGB returns to h_rgb (HOST [n][out_dim]) on
  * a library-owned copy-out stream.  Work starts after everything already enqueued on the caller's stream; the call
- * returns after all three streams have finished (it synchronises).  q->perm must be NULL.  Pinned host memory lets the
+ * returns after all three streams have finished (it synchronises), on failure too: no copy from or to the caller's
+ * buffers is in flight when it returns, whatever the status.  q->perm must be NULL.  Pinned host memory lets the
  * copies overlap; pageable memory works but serialises.  Needs oo_reserve(n).  Launches one fused kernel per chunk. */
 OO_API oo_status oo_query_host(oo_ctx* ctx, const oo_queries* q, float* h_rgb, void* cuda_stream);
 

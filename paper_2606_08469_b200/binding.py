@@ -19,7 +19,8 @@ _STATUS = {0: "OO_OK", 1: "OO_ERR_INVALID_ARG", 2: "OO_ERR_NOT_READY", 3: "OO_ER
 
 EXPORTED_SYMBOLS = ["oo_create", "oo_destroy", "oo_last_error", "oo_upload_tree", "oo_upload_mlp", "oo_reserve", "oo_set_path",
                     "oo_get_info", "oo_sort_queries", "oo_encode", "oo_query", "oo_query_host", "oo_read_padded_map", "oo_set_mode",
-                    "oo_encode_full", "oo_upload_scene", "oo_raycast", "oo_upload_disparity", "oo_predict_disparity", "oo_set_presort"]
+                    "oo_encode_full", "oo_upload_scene", "oo_raycast", "oo_upload_disparity", "oo_predict_disparity", "oo_set_presort",
+                    "oo_query_debug", "oo_set_host_chunks", "oo_last_note"]
 
 
 class OOError(RuntimeError):
@@ -37,7 +38,7 @@ class _TreeDesc(C.Structure):
 
 class _MlpDesc(C.Structure):
     _fields_ = [("in_dim", C.c_uint32), ("width", C.c_uint32), ("n_hidden", C.c_uint32), ("out_dim", C.c_uint32),
-                ("weights", C.c_void_p), ("out_act", C.c_int)]
+                ("weights", C.c_void_p), ("out_act", C.c_int), ("weights_on_device", C.c_uint32)]
 
 
 class _Queries(C.Structure):
@@ -67,7 +68,8 @@ class _Info(C.Structure):
     _fields_ = [("launches", C.c_uint64), ("query_launches", C.c_uint64), ("node_table_bytes", C.c_uint64),
                 ("atlas_bytes", C.c_uint64), ("path_last_query", C.c_uint32), ("path_last_encode", C.c_uint32),
                 ("hop_plan_ok", C.c_uint32), ("n_sms", C.c_uint32),
-                ("presorted_last_query", C.c_uint32), ("presorted_last_encode", C.c_uint32)]
+                ("presorted_last_query", C.c_uint32), ("presorted_last_encode", C.c_uint32),
+                ("full_query", C.c_uint32), ("n_neighbours", C.c_uint32)]
 
 
 _lib = None
@@ -91,6 +93,10 @@ def load_library():
     L.oo_destroy.restype = None
     L.oo_last_error.argtypes = [vp]
     L.oo_last_error.restype = C.c_char_p
+    L.oo_last_note.argtypes = [vp]
+    L.oo_last_note.restype = C.c_char_p
+    L.oo_query_debug.argtypes = [vp, C.POINTER(_Queries), vp, vp, vp, vp]
+    L.oo_set_host_chunks.argtypes = [vp, u32]
     L.oo_upload_tree.argtypes = [vp, C.POINTER(_TreeDesc), vp]
     L.oo_upload_mlp.argtypes = [vp, C.POINTER(_MlpDesc), vp]
     L.oo_reserve.argtypes = [vp, u64]
@@ -109,7 +115,7 @@ def load_library():
     L.oo_upload_disparity.argtypes = [vp, C.POINTER(_DisparityDesc), vp]
     L.oo_predict_disparity.argtypes = [vp, C.POINTER(_Queries), vp, vp, vp]
     for name in EXPORTED_SYMBOLS:
-        if name not in ("oo_destroy", "oo_last_error"):
+        if name not in ("oo_destroy", "oo_last_error", "oo_last_note"):
             getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -182,11 +188,18 @@ class OctaOctree:
         del dev
 
     def oo_upload_mlp(self, weights: Sequence, out_act: str = "exp"):
+        """weights: fp16 matrices [out][in], numpy arrays (host) or torch CUDA tensors (oo_mlp_desc.weights_on_device)."""
         import numpy as np
-        ws = [np.ascontiguousarray(w, np.float16) for w in weights]
-        ptrs = (C.c_void_p * len(ws))(*[w.ctypes.data for w in ws])
+        torch = self._torch
+        on_dev = all(isinstance(w, torch.Tensor) and w.is_cuda for w in weights)
+        if on_dev:
+            ws = [w.to(dtype=torch.float16).contiguous() for w in weights]
+            ptrs = (C.c_void_p * len(ws))(*[w.data_ptr() for w in ws])
+        else:
+            ws = [np.ascontiguousarray(w, np.float16) for w in weights]
+            ptrs = (C.c_void_p * len(ws))(*[w.ctypes.data for w in ws])
         d = _MlpDesc(ws[0].shape[1], ws[0].shape[0], len(ws) - 1, ws[-1].shape[0], C.cast(ptrs, C.c_void_p),
-                     {"none": OO_ACT_NONE, "exp": OO_ACT_EXP}[out_act])
+                     {"none": OO_ACT_NONE, "exp": OO_ACT_EXP}[out_act], 1 if on_dev else 0)
         self._check(self._L.oo_upload_mlp(self._ctx, C.byref(d), self._stream()))
         self.out_dim = int(ws[-1].shape[0])
 
@@ -293,6 +306,28 @@ class OctaOctree:
             rgb = torch.empty((n, self.out_dim), dtype=torch.float32, device=self.device)
         self._check(self._L.oo_query(self._ctx, C.byref(q), C.c_void_p(rgb.data_ptr()), self._stream()))
         return rgb
+
+    def oo_query_debug(self, x, nrm, wo, extra=None, perm=None, rgb=None, disparity=None):
+        """oo_query through the fused kernels' debug instances: (rgb, slot, index).  Hot path: slot [n][L] int32, index
+        [n][L][2] int16; full query: slot [n][L][J], index [n][L][J][3]."""
+        torch = self._torch
+        q, n = self._queries(x, nrm, wo, extra, perm, disparity)
+        if rgb is None:
+            rgb = torch.empty((n, self.out_dim), dtype=torch.float32, device=self.device)
+        info = self.oo_get_info()
+        full = bool(info["full_query"])
+        shape = (n, self.n_levels, info["n_neighbours"]) if full else (n, self.n_levels)
+        slot = torch.full(shape, -2, dtype=torch.int32, device=self.device)
+        index = torch.full(shape + ((3,) if full else (2,)), -32768, dtype=torch.int16, device=self.device)
+        self._check(self._L.oo_query_debug(self._ctx, C.byref(q), C.c_void_p(rgb.data_ptr()), C.c_void_p(slot.data_ptr()),
+                                           C.c_void_p(index.data_ptr()), self._stream()))
+        return rgb, slot, index
+
+    def oo_set_host_chunks(self, n_chunks: int = 0):
+        self._check(self._L.oo_set_host_chunks(self._ctx, int(n_chunks)))
+
+    def oo_last_note(self) -> str:
+        return self._L.oo_last_note(self._ctx).decode()
 
     def oo_query_host(self, x, nrm, wo, extra=None, rgb=None, disparity=None):
         """x, nrm, wo, extra, rgb: CPU tensors (pinned for asynchronous copies) or numpy arrays.  Synchronous."""

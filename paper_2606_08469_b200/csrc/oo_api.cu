@@ -19,7 +19,8 @@ struct oo_ctx {
     int device = 0;
     int n_sms = 148;
     std::string err;
-    cudaError_t sticky = cudaSuccess;
+    std::string note;                      // informational: how the last upload / query resolved OO_PATH_AUTO (oo_last_note)
+    cudaError_t sticky = cudaSuccess;      // a context-fatal CUDA error seen earlier (illegal address, launch failure, ...)
     oo_path path = OO_PATH_AUTO;
     FullModeH mode{0, 0, 0};
     oo_info info{};
@@ -57,19 +58,19 @@ struct oo_ctx {
 
     // scratch
     uint64_t reserved = 0;
-    void* d_feat = nullptr;    uint64_t feat_bytes = 0;
+    void* d_feat = nullptr;    uint64_t feat_bytes = 0;   // feature rows of OO_PATH_GENERIC / OO_PATH_UNFUSED (sized by oo_reserve)
     uint32_t *d_keys_a = nullptr, *d_keys_b = nullptr, *d_idx_a = nullptr, *d_hist = nullptr;
     float *d_qx = nullptr, *d_qn = nullptr, *d_qw = nullptr, *d_qe = nullptr, *d_rgb = nullptr, *d_qd = nullptr;
-    // OO_PRESORT_BIN: the binned copy of the queries and their original indices (allocated on first use, `reserved` rows)
+    // OO_PRESORT_BIN: the binned copy of the queries and their original indices (allocated by oo_reserve, `reserved` rows)
     oo_presort presort = OO_PRESORT_NONE;
     uint64_t bin_min = 1u << 18;           // batches below this proceed unsorted (the extra launches cost more than they save)
     float *d_bx = nullptr, *d_bn = nullptr, *d_bw = nullptr, *d_be = nullptr;
     uint32_t *d_binv = nullptr, *d_bidx = nullptr;
     float *d_brgb = nullptr, *d_bdisp = nullptr;
-    uint64_t bin_rows = 0;
 
     // oo_query_host pipeline: copy-in and copy-out streams beside the caller's stream, one event pair per chunk
     static constexpr int kMaxChunks = 16;
+    int host_chunks = 0;                   // oo_set_host_chunks: 0 = chosen from the batch size
     bool have_pipe = false;
     cudaStream_t s_h2d = nullptr, s_d2h = nullptr;
     cudaEvent_t ev_start = nullptr, ev_out = nullptr, ev_in[kMaxChunks] = {}, ev_k[kMaxChunks] = {};
@@ -87,11 +88,26 @@ oo_status fail(oo_ctx* c, oo_status st, const char* fmt, ...) {
     return st;
 }
 
+// Errors after which the CUDA context is unusable: only these are latched (every later call on the oo_ctx then fails at
+// once).  Anything else -- an allocation that did not fit, a launch configuration the device rejects, an invalid argument --
+// is reported for the call that caused it, cleared, and the context stays usable.
+bool is_fatal(cudaError_t e) {
+    switch (e) {
+        case cudaErrorIllegalAddress: case cudaErrorLaunchFailure: case cudaErrorIllegalInstruction: case cudaErrorMisalignedAddress:
+        case cudaErrorInvalidAddressSpace: case cudaErrorInvalidPc: case cudaErrorHardwareStackError: case cudaErrorLaunchTimeout:
+        case cudaErrorAssert: case cudaErrorECCUncorrectable: case cudaErrorDeviceUninitialized: case cudaErrorDevicesUnavailable:
+            return true;
+        default:
+            return false;
+    }
+}
+
 #define OO_CUDA(c, call)                                                                                      \
     do {                                                                                                      \
         cudaError_t e_ = (call);                                                                              \
         if (e_ != cudaSuccess) {                                                                              \
-            (c)->sticky = e_;                                                                                 \
+            (void)cudaGetLastError(); /* clear the thread's error state: the failure is reported here */      \
+            if (is_fatal(e_)) (c)->sticky = e_;                                                               \
             return fail((c), e_ == cudaErrorMemoryAllocation ? OO_ERR_OOM : OO_ERR_CUDA, "%s: %s", #call,     \
                         cudaGetErrorString(e_));                                                              \
         }                                                                                                     \
@@ -135,7 +151,6 @@ void free_scratch(oo_ctx* c) {
     for (void** p : ps) free_dev(*p);
     void** bs[] = {(void**)&c->d_bx, (void**)&c->d_bn, (void**)&c->d_bw, (void**)&c->d_be, (void**)&c->d_binv, (void**)&c->d_bidx, (void**)&c->d_brgb, (void**)&c->d_bdisp};
     for (void** p : bs) free_dev(*p);
-    c->bin_rows = 0;
     c->reserved = 0;
 }
 
@@ -156,14 +171,34 @@ void free_pipe(oo_ctx* c) {
 
 bool is_pow2(uint32_t v) { return v && !(v & (v - 1)); }
 
-oo_status check_async(oo_ctx* c) {
+// Before the library launches anything: fail at once on a context that already saw a fatal error; a fatal error pending on
+// the calling thread (whoever caused it, the CUDA context is gone) is latched and reported; a pending NON-fatal error of the
+// thread -- some other library's rejected launch, say -- is not ours to report: it is cleared so that the check after our own
+// launches sees only them.
+oo_status check_before(oo_ctx* c) {
     if (c->sticky != cudaSuccess) return fail(c, OO_ERR_CUDA, "earlier CUDA failure: %s", cudaGetErrorString(c->sticky));
-    cudaError_t e = cudaPeekAtLastError();
-    if (e != cudaSuccess) {
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess && is_fatal(e)) {
         c->sticky = e;
         return fail(c, OO_ERR_CUDA, "asynchronous CUDA failure: %s", cudaGetErrorString(e));
     }
     return OO_OK;
+}
+// After the library's own launches: cudaGetLastError (which clears) reports what they produced.
+oo_status check_after(oo_ctx* c) {
+    const cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) return OO_OK;
+    if (is_fatal(e)) c->sticky = e;
+    return fail(c, OO_ERR_CUDA, "kernel launch failed: %s", cudaGetErrorString(e));
+}
+// A launcher's return value: > 0 launches (counted), -1 no such kernel, kLaunchCudaError a CUDA call failed on the way.
+oo_status launch_failed(oo_ctx* c, int n, const char* what) {
+    if (n == kLaunchCudaError) {
+        const cudaError_t e = cudaGetLastError();
+        if (is_fatal(e)) c->sticky = e;
+        return fail(c, OO_ERR_CUDA, "%s: %s", what, cudaGetErrorString(e));
+    }
+    return fail(c, OO_ERR_UNSUPPORTED, "%s: no kernel for this shape", what);
 }
 
 oo_status check_queries(oo_ctx* c, const oo_queries* q, bool need_nrm) {
@@ -236,6 +271,7 @@ extern "C" OO_API void oo_destroy(oo_ctx* c) {
 }
 
 extern "C" OO_API const char* oo_last_error(const oo_ctx* c) { return c ? c->err.c_str() : "context is NULL"; }
+extern "C" OO_API const char* oo_last_note(const oo_ctx* c) { return c ? c->note.c_str() : ""; }
 
 extern "C" OO_API oo_status oo_set_path(oo_ctx* c, oo_path path) {
     if (!c) return OO_ERR_INVALID_ARG;
@@ -267,6 +303,8 @@ extern "C" OO_API oo_status oo_get_info(const oo_ctx* c, oo_info* out) {
     if (!c || !out) return OO_ERR_INVALID_ARG;
     *out = c->info;
     out->hop_plan_ok = c->plan_ok ? 1u : 0u;
+    out->full_query = c->mode.tri8 || c->mode.lookup || c->mode.attrs_paper || (c->have_tree && c->T.vertex) || (c->have_mlp && c->M.width != 64);
+    out->n_neighbours = c->mode.tri8 ? 8u : 1u;
     return OO_OK;
 }
 
@@ -526,31 +564,48 @@ extern "C" OO_API oo_status oo_upload_mlp(oo_ctx* c, const oo_mlp_desc* m, void*
     const uint32_t W = m->width;
     if (m->n_hidden < 1 || m->n_hidden > OO_MAX_HIDDEN) return fail(c, OO_ERR_INVALID_ARG, "n_hidden %u outside 1..%d", m->n_hidden, OO_MAX_HIDDEN);
     if (m->out_dim < 1 || m->out_dim > 8) return fail(c, OO_ERR_INVALID_ARG, "out_dim %u outside 1..8", m->out_dim);
-    if (m->in_dim < 7 || m->in_dim > OO_MAX_LEVELS * 32 + 6 + OO_MAX_EXTRA) return fail(c, OO_ERR_INVALID_ARG, "in_dim %u out of range", m->in_dim);
+    // widest input the ABI describes: L*F <= OO_MAX_LEVELS*32 features + 9 attributes (OO_ATTRS_PAPER) + OO_MAX_EXTRA extras
+    if (m->in_dim < 7 || m->in_dim > OO_MAX_LEVELS * 32 + 9 + OO_MAX_EXTRA) return fail(c, OO_ERR_INVALID_ARG, "in_dim %u outside 7..%d", m->in_dim, OO_MAX_LEVELS * 32 + 9 + OO_MAX_EXTRA);
     if (m->out_act != OO_ACT_NONE && m->out_act != OO_ACT_EXP) return fail(c, OO_ERR_INVALID_ARG, "unknown out_act");
     for (uint32_t k = 0; k <= m->n_hidden; ++k)
         if (!m->weights[k]) return fail(c, OO_ERR_INVALID_ARG, "weights[%u] is NULL", k);
     cudaStream_t stream = (cudaStream_t)cuda_stream;
     DeviceGuard g(c->device);
+    // weights_on_device: the matrices are DEVICE buffers (e.g. a trainer's parameters): bring them to the host first, the
+    // padded images are built there either way (a few tens of KB, once per upload)
+    std::vector<std::vector<uint16_t>> staged;
+    std::vector<const void*> host_w(m->n_hidden + 1);
+    for (uint32_t k = 0; k <= m->n_hidden; ++k) host_w[k] = m->weights[k];
+    if (m->weights_on_device) {
+        staged.resize(m->n_hidden + 1);
+        for (uint32_t k = 0; k <= m->n_hidden; ++k) {
+            const size_t rows = k == m->n_hidden ? m->out_dim : W, cols = k == 0 ? m->in_dim : W;
+            staged[k].resize(rows * cols);
+            OO_CUDA(c, cudaMemcpyAsync(staged[k].data(), m->weights[k], rows * cols * 2, cudaMemcpyDeviceToHost, stream));
+            host_w[k] = staged[k].data();
+        }
+        OO_CUDA(c, cudaStreamSynchronize(stream));
+    }
+    const void* const* weights = host_w.data();
     const uint32_t k1 = (m->in_dim + 15) & ~15u;
     const uint32_t s0 = k1 + 8, s1 = 72;
     const size_t halves = (size_t)64 * s0 + (size_t)(m->n_hidden - 1) * 64 * s1 + (size_t)16 * s1;
     std::vector<uint16_t> img(halves, 0);     // the mma.sync image (width 64 only; left zero otherwise and never used)
-    const uint16_t* w0 = (const uint16_t*)m->weights[0];
+    const uint16_t* w0 = (const uint16_t*)weights[0];
     if (W == 64)
     for (uint32_t o = 0; o < 64; ++o)
         for (uint32_t i = 0; i < m->in_dim; ++i) img[(size_t)o * s0 + i] = w0[(size_t)o * m->in_dim + i];
     size_t off = (size_t)64 * s0;
     for (uint32_t k = 1; W == 64 && k < m->n_hidden; ++k) {
-        const uint16_t* w = (const uint16_t*)m->weights[k];
+        const uint16_t* w = (const uint16_t*)weights[k];
         for (uint32_t o = 0; o < 64; ++o)
             for (uint32_t i = 0; i < 64; ++i) img[off + (size_t)o * s1 + i] = w[(size_t)o * 64 + i];
         off += (size_t)64 * s1;
     }
-    const uint16_t* wl = (const uint16_t*)m->weights[m->n_hidden];
+    const uint16_t* wl = (const uint16_t*)weights[m->n_hidden];
     for (uint32_t o = 0; W == 64 && o < m->out_dim; ++o)
         for (uint32_t i = 0; i < 64; ++i) img[off + (size_t)o * s1 + i] = wl[(size_t)o * 64 + i];
-    const std::vector<uint16_t> tc = make_tc_image(m->in_dim, W, m->n_hidden, m->out_dim, m->weights);
+    const std::vector<uint16_t> tc = make_tc_image(m->in_dim, W, m->n_hidden, m->out_dim, weights);
     const size_t tc_halves = tc.size();
     free_dev(c->d_image);
     free_dev(c->d_image_tc);
@@ -640,11 +695,32 @@ extern "C" OO_API oo_status oo_upload_disparity(oo_ctx* c, const oo_disparity_de
 // ---------------------------------------------------------------------------------------------------------------------
 // scratch
 // ---------------------------------------------------------------------------------------------------------------------
+// Bytes of feature scratch OO_PATH_GENERIC / OO_PATH_UNFUSED need for n queries of the uploaded tree (0 without a tree)
+static uint64_t feat_bytes_for(const oo_ctx* c, uint64_t n) {
+    return c->have_tree ? n * (uint64_t)c->T.n_levels * c->T.texel_bytes : 0;
+}
+
 extern "C" OO_API oo_status oo_reserve(oo_ctx* c, uint64_t n) {
     if (!c) return OO_ERR_INVALID_ARG;
-    if (n <= c->reserved) return OO_OK;
+    if (c->sticky != cudaSuccess) return fail(c, OO_ERR_CUDA, "earlier CUDA failure: %s", cudaGetErrorString(c->sticky));
     DeviceGuard g(c->device);
+    // feature rows of the unfused paths depend on the uploaded tree: (re)sized here even when the row count is unchanged,
+    // so that "oo_upload_tree, then oo_reserve" is always enough and no hot call has to allocate
+    const uint64_t rows = std::max(n, c->reserved);
+    const uint64_t fb = feat_bytes_for(c, rows);
+    if (fb > c->feat_bytes) {
+        free_dev(c->d_feat);
+        c->feat_bytes = 0;
+        OO_CUDA(c, cudaMalloc(&c->d_feat, fb));
+        c->feat_bytes = fb;
+    }
+    if (n <= c->reserved) return OO_OK;
+    void* keep_feat = c->d_feat;
+    const uint64_t keep_fb = c->feat_bytes;
+    c->d_feat = nullptr;
     free_scratch(c);
+    c->d_feat = keep_feat;
+    c->feat_bytes = keep_fb;
     OO_CUDA(c, cudaMalloc((void**)&c->d_keys_a, n * 4));
     OO_CUDA(c, cudaMalloc((void**)&c->d_keys_b, n * 4));
     OO_CUDA(c, cudaMalloc((void**)&c->d_idx_a, n * 4));
@@ -655,37 +731,28 @@ extern "C" OO_API oo_status oo_reserve(oo_ctx* c, uint64_t n) {
     OO_CUDA(c, cudaMalloc((void**)&c->d_qe, n * 4 * OO_MAX_EXTRA));
     OO_CUDA(c, cudaMalloc((void**)&c->d_rgb, n * 4 * 8));
     OO_CUDA(c, cudaMalloc((void**)&c->d_qd, n * 4));
+    // OO_PRESORT_BIN: the binned copy of the queries, both index maps, the binned RGB and d^
+    OO_CUDA(c, cudaMalloc((void**)&c->d_bx, n * 12));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_bn, n * 12));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_bw, n * 12));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_be, n * 4 * OO_MAX_EXTRA));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_binv, n * 4));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_bidx, n * 4));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_brgb, n * 4 * 8));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_bdisp, n * 4));
     c->reserved = n;
     return OO_OK;
 }
 
-static oo_status ensure_feat(oo_ctx* c, uint64_t bytes) {
+// Hot calls never allocate: the scratch they need must have been reserved.
+static oo_status need_feat(oo_ctx* c, uint64_t bytes) {
     if (bytes <= c->feat_bytes) return OO_OK;
-    free_dev(c->d_feat);
-    c->feat_bytes = 0;
-    OO_CUDA(c, cudaMalloc(&c->d_feat, bytes));
-    c->feat_bytes = bytes;
-    return OO_OK;
+    return fail(c, OO_ERR_NOT_READY, "OO_PATH_GENERIC / OO_PATH_UNFUSED keep the feature rows in scratch: call oo_reserve(n) after oo_upload_tree (need %llu bytes, have %llu)",
+                (unsigned long long)bytes, (unsigned long long)c->feat_bytes);
 }
-
-// OO_PRESORT_BIN scratch: the binned copy of the queries, both index maps and the binned RGB (`reserved` rows)
-static oo_status ensure_bin(oo_ctx* c, uint64_t n) {
-    if (n > c->reserved) return fail(c, OO_ERR_NOT_READY, "OO_PRESORT_BIN: call oo_reserve(%llu) first", (unsigned long long)n);
-    if (c->bin_rows >= n) return OO_OK;
-    void** bs[] = {(void**)&c->d_bx, (void**)&c->d_bn, (void**)&c->d_bw, (void**)&c->d_be, (void**)&c->d_binv, (void**)&c->d_bidx, (void**)&c->d_brgb, (void**)&c->d_bdisp};
-    for (void** b : bs) free_dev(*b);
-    c->bin_rows = 0;
-    const uint64_t rows = c->reserved;
-    OO_CUDA(c, cudaMalloc((void**)&c->d_bx, rows * 12));
-    OO_CUDA(c, cudaMalloc((void**)&c->d_bn, rows * 12));
-    OO_CUDA(c, cudaMalloc((void**)&c->d_bw, rows * 12));
-    OO_CUDA(c, cudaMalloc((void**)&c->d_be, rows * 4 * OO_MAX_EXTRA));
-    OO_CUDA(c, cudaMalloc((void**)&c->d_binv, rows * 4));
-    OO_CUDA(c, cudaMalloc((void**)&c->d_bidx, rows * 4));
-    OO_CUDA(c, cudaMalloc((void**)&c->d_brgb, rows * 4 * 8));
-    OO_CUDA(c, cudaMalloc((void**)&c->d_bdisp, rows * 4));
-    c->bin_rows = rows;
-    return OO_OK;
+static oo_status need_bin(oo_ctx* c, uint64_t n) {
+    if (n <= c->reserved) return OO_OK;
+    return fail(c, OO_ERR_NOT_READY, "OO_PRESORT_BIN: call oo_reserve(%llu) first", (unsigned long long)n);
 }
 
 // a1' for oo_query: one counting pass on the top Morton bits moves the queries (and a caller-supplied d^) into the binned
@@ -693,10 +760,12 @@ static oo_status ensure_bin(oo_ctx* c, uint64_t n) {
 static bool bin_wanted(const oo_ctx* c, const oo_queries* q) {
     return c->presort == OO_PRESORT_BIN && !q->perm && q->n >= c->bin_min;
 }
-static oo_status bin_for_query(oo_ctx* c, const oo_queries* q, oo_queries* qb, cudaStream_t stream) {
-    if (oo_status st = ensure_bin(c, q->n)) return st;
-    count(c, launch_bin_queries(make_qp(q), c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, nullptr,
-                                q->disparity ? c->d_bdisp : nullptr, stream));
+static oo_status bin_for_query(oo_ctx* c, const oo_queries* q, oo_queries* qb, cudaStream_t stream, bool want_idx = false) {
+    if (oo_status st = need_bin(c, q->n)) return st;
+    const int k = launch_bin_queries(make_qp(q), c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv,
+                                     want_idx ? c->d_bidx : nullptr, q->disparity ? c->d_bdisp : nullptr, stream);
+    if (k < 0) return launch_failed(c, k, "bin pass");
+    count(c, k);
     *qb = *q;
     qb->x = c->d_bx; qb->nrm = c->d_bn; qb->wo = c->d_bw;
     qb->extra = q->n_extra && q->extra ? c->d_be : nullptr;
@@ -712,10 +781,12 @@ extern "C" OO_API oo_status oo_sort_queries(oo_ctx* c, const oo_queries* q, uint
     if (!q || (q->n && (!q->x || !d_perm_out))) return fail(c, OO_ERR_INVALID_ARG, "NULL argument");
     if (q->n >= (1ull << 32)) return fail(c, OO_ERR_UNSUPPORTED, "more than 2^32-1 queries per call");
     if (q->n > c->reserved) return fail(c, OO_ERR_NOT_READY, "call oo_reserve(%llu) first", (unsigned long long)q->n);
-    if (oo_status st = check_async(c)) return st;
+    if (oo_status st = check_before(c)) return st;
     DeviceGuard g(c->device);
-    count(c, launch_morton_sort(q->x, q->n, c->d_keys_a, c->d_keys_b, c->d_idx_a, d_perm_out, c->d_hist, (cudaStream_t)cuda_stream));
-    return check_async(c);
+    const int k = launch_morton_sort(q->x, q->n, c->d_keys_a, c->d_keys_b, c->d_idx_a, d_perm_out, c->d_hist, (cudaStream_t)cuda_stream);
+    if (k < 0) return launch_failed(c, k, "Morton sort");
+    count(c, k);
+    return check_after(c);
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
@@ -734,7 +805,7 @@ extern "C" OO_API oo_status oo_encode(oo_ctx* c, const oo_queries* q, void* d_fe
     if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "no tree uploaded");
     if (c->T.vertex) return fail(c, OO_ERR_UNSUPPORTED, "oo_encode reads texel maps; use oo_encode_full for vertex maps");
     if (oo_status st = check_queries(c, q, false)) return st;
-    if (oo_status st = check_async(c)) return st;
+    if (oo_status st = check_before(c)) return st;
     if (q->n == 0) return OO_OK;
     DeviceGuard g(c->device);
     const oo_path p = resolve_encode_path(c);
@@ -744,18 +815,20 @@ extern "C" OO_API oo_status oo_encode(oo_ctx* c, const oo_queries* q, void* d_fe
     c->info.presorted_last_encode = 0;
     if (c->presort == OO_PRESORT_BIN && p == OO_PATH_UNFUSED && !q->perm && q->n >= c->bin_min) {
         // a1': x and wo move into Morton bins; the encode kernel reads them in order and stores every row at its query's index
-        if (oo_status st = ensure_bin(c, q->n)) return st;
+        if (oo_status st = need_bin(c, q->n)) return st;
         Q.nrm = nullptr; Q.extra = nullptr; Q.n_extra = 0;
-        count(c, launch_bin_queries(Q, c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, c->d_bidx, nullptr, (cudaStream_t)cuda_stream));
+        const int k = launch_bin_queries(Q, c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, c->d_bidx, nullptr, (cudaStream_t)cuda_stream);
+        if (k < 0) return launch_failed(c, k, "bin pass");
+        count(c, k);
         Q.x = c->d_bx; Q.wo = c->d_bw; Q.out_idx = c->d_bidx;
         c->info.presorted_last_encode = 1;
     }
     int n = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Q, O, c->tree_max_depth, (cudaStream_t)cuda_stream)
                                  : launch_encode_fast(c->T, Q, O, c->n_sms, (cudaStream_t)cuda_stream);
-    if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "encode kernel missing");
+    if (n < 0) return launch_failed(c, n, "encode kernel");
     count(c, n);
     c->info.path_last_encode = (uint32_t)p;
-    return check_async(c);
+    return check_after(c);
 }
 
 // the full-query kernels are needed as soon as anything differs from the hot path
@@ -778,12 +851,12 @@ static oo_status predict_disparity(oo_ctx* c, const oo_queries* q, float* d_out,
     if (!c->have_disp) return fail(c, OO_ERR_NOT_READY, "no disparity predictor uploaded");
     if (oo_status st = check_queries(c, q, true)) return st;
     if (q->n && !d_out) return fail(c, OO_ERR_INVALID_ARG, "disparity output is NULL");
-    if (oo_status st = check_async(c)) return st;
+    if (oo_status st = check_before(c)) return st;
     if (q->n == 0) return OO_OK;
     const int n = launch_disparity(c->G, c->MD, make_qp(q), d_out, d_features, c->n_sms, stream);
-    if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "no disparity kernel for this predictor");
+    if (n < 0) return launch_failed(c, n, "disparity kernel");
     count(c, n);
-    return check_async(c);
+    return check_after(c);
 }
 
 // OO_LOOKUP_SHIFTED without a caller-supplied d^: run the predictor into the context's scratch and point the queries at it.
@@ -806,20 +879,39 @@ extern "C" OO_API oo_status oo_encode_full(oo_ctx* c, const oo_queries* q, float
     if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "no tree uploaded");
     if (oo_status st = check_queries(c, q, false)) return st;
     if (oo_status st = check_full(c, q)) return st;
-    if (oo_status st = check_async(c)) return st;
+    if (oo_status st = check_before(c)) return st;
     if (q->n == 0) return OO_OK;
     DeviceGuard g(c->device);
     oo_queries qd = *q;
     if (oo_status st = fill_disparity(c, &qd, (cudaStream_t)cuda_stream)) return st;
     q = &qd;
     const int n = launch_encode_full(c->T, make_qp(q), c->mode, d_features, d_slot, d_cell, c->n_sms, (cudaStream_t)cuda_stream);
-    if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "no full-query encode kernel for F=%u %s", c->T.F, c->T.f32 ? "fp32" : "fp16");
+    if (n < 0) return launch_failed(c, n, "full-query encode kernel (F, dtype)");
     count(c, n);
     c->info.path_last_encode = (uint32_t)OO_PATH_FULL;
-    return check_async(c);
+    return check_after(c);
 }
 
-static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cudaStream_t stream) {
+// Debug outputs of oo_query_debug (null for oo_query)
+struct DebugOut {
+    int32_t* slot = nullptr;
+    int16_t* index = nullptr;
+    bool on() const { return slot || index; }
+};
+
+static const char* path_name(oo_path p) {
+    switch (p) {
+        case OO_PATH_GENERIC: return "OO_PATH_GENERIC";
+        case OO_PATH_UNFUSED: return "OO_PATH_UNFUSED";
+        case OO_PATH_FUSED_MMA: return "OO_PATH_FUSED_MMA";
+        case OO_PATH_FUSED_TC: return "OO_PATH_FUSED_TC";
+        case OO_PATH_FUSED_TC_TMEM: return "OO_PATH_FUSED_TC_TMEM";
+        case OO_PATH_FULL: return "OO_PATH_FULL";
+        default: return "OO_PATH_AUTO";
+    }
+}
+
+static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cudaStream_t stream, const DebugOut& dbg = DebugOut()) {
     if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "no tree uploaded");
     if (!c->have_mlp) return fail(c, OO_ERR_NOT_READY, "no MLP uploaded");
     if (oo_status st = check_queries(c, q, true)) return st;
@@ -828,87 +920,120 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
     const uint32_t n_attr = c->mode.attrs_paper ? 9u : 6u;
     if (c->M.in_dim != feat + n_attr + q->n_extra)
         return fail(c, OO_ERR_NOT_READY, "MLP in_dim %u != L*F + %u + n_extra = %u", c->M.in_dim, n_attr, feat + n_attr + q->n_extra);
-    if (needs_full(c)) {
+    const bool full = needs_full(c);
+    if (full) {
         if (oo_status st = check_full(c, q)) return st;
         if (c->path != OO_PATH_AUTO) return fail(c, OO_ERR_UNSUPPORTED, "the full query has one kernel; oo_set_path(OO_PATH_AUTO)");
-        if (oo_status st = check_async(c)) return st;
-        if (q->n == 0) return OO_OK;
-        c->M.feat_dim = feat;
-        oo_queries qd = *q;
-        float* out = d_rgb;
-        c->info.presorted_last_query = 0;
-        if (bin_wanted(c, q)) {      // bin first: the predictor's hash-grid gathers profit from the order too
-            if (oo_status st = bin_for_query(c, q, &qd, stream)) return st;
-            out = c->d_brgb;
-            c->info.presorted_last_query = 1;
-        }
-        if (oo_status st = fill_disparity(c, &qd, stream)) return st;
-        const QueryParams Q = make_qp(&qd);
-        const int n = c->M.width == 64 ? launch_fused_full_w64(c->T, c->M, Q, c->mode, out, c->n_sms, stream)
-                                       : launch_fused_full_w128(c->T, c->M, Q, c->mode, out, c->n_sms, stream);
-        if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "no full-query kernel for F=%u %s, in_dim %u, out_dim %u", c->T.F, c->T.f32 ? "fp32" : "fp16", c->M.in_dim, c->M.out_dim);
-        count(c, n);
-        if (c->info.presorted_last_query) count(c, launch_unbin(c->d_brgb, c->d_binv, q->n, c->M.out_dim, d_rgb, c->n_sms, stream));
-        c->info.path_last_query = (uint32_t)OO_PATH_FULL;
-        return check_async(c);
     }
-    if (oo_status st = check_async(c)) return st;
+    if (oo_status st = check_before(c)) return st;
     if (q->n == 0) return OO_OK;
     c->M.feat_dim = feat;
-    const bool fast = c->plan_ok && fast_shape_supported(c->T.n_levels, c->T.F, c->T.f32 != 0);
-    oo_path p = c->path;
-    if (p == OO_PATH_AUTO)
-        p = !fast ? OO_PATH_GENERIC
-                  : (tm_shape_supported(c->T.n_levels, c->T.F, c->T.f32 != 0) && c->M.out_dim <= 4 ? OO_PATH_FUSED_TC_TMEM : OO_PATH_FUSED_MMA);
-    if (p != OO_PATH_GENERIC && !fast)
-        return fail(c, OO_ERR_UNSUPPORTED, "no specialised kernel for L=%u F=%u (or the tree has no hop plan); use OO_PATH_GENERIC/AUTO", c->T.n_levels, c->T.F);
-    QueryParams Q = make_qp(q);
-    int n = 0;
-    float* const d_out = d_rgb;
+    // ---- a1 inside the query: bin the queries first (the predictor's hash-grid gathers profit from the order too)
+    oo_queries qd = *q;
+    float* out = d_rgb;
     c->info.presorted_last_query = 0;
     if (bin_wanted(c, q)) {
-        oo_queries qb;
-        if (oo_status st = bin_for_query(c, q, &qb, stream)) return st;
-        Q = make_qp(&qb);
-        d_rgb = c->d_brgb;
+        if (oo_status st = bin_for_query(c, q, &qd, stream, dbg.on())) return st;
+        out = c->d_brgb;
         c->info.presorted_last_query = 1;
     }
-    if (p == OO_PATH_GENERIC || p == OO_PATH_UNFUSED) {
-        const uint64_t bytes = q->n * (uint64_t)feat * (c->T.f32 ? 4 : 2);
-        if (oo_status st = ensure_feat(c, bytes)) return st;
-        EncodeOut O{c->d_feat, nullptr, nullptr};
-        // features are indexed by the query's own index, so perm only changes the processing order
-        n = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Q, O, c->tree_max_depth, stream)
-                                 : launch_encode_fast(c->T, Q, O, c->n_sms, stream);
-        if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "encode kernel missing");
-        count(c, n);
-        n = launch_mlp_rows(c->T, c->M, Q, c->d_feat, d_rgb, c->n_sms, stream);
-    } else if (p == OO_PATH_FUSED_MMA) {
-        n = launch_fused_mma(c->T, c->M, Q, d_rgb, c->n_sms, stream);
-    } else if (p == OO_PATH_FUSED_TC) {
-        n = launch_fused_tc(c->T, c->M, Q, d_rgb, c->n_sms, stream);
+    QueryParams Q;
+    int n = 0;
+    oo_path p = c->path;
+    if (full) {
+        if (oo_status st = fill_disparity(c, &qd, stream)) return st;
+        Q = make_qp(&qd);
+        Q.dbg_slot = dbg.slot; Q.dbg_texel = dbg.index;
+        if (c->info.presorted_last_query && dbg.on()) Q.out_idx = c->d_bidx;
+        if (dbg.on())
+            n = c->M.width == 64 ? launch_fused_full_w64_dbg(c->T, c->M, Q, c->mode, out, c->n_sms, stream)
+                                 : launch_fused_full_w128_dbg(c->T, c->M, Q, c->mode, out, c->n_sms, stream);
+        else
+            n = c->M.width == 64 ? launch_fused_full_w64(c->T, c->M, Q, c->mode, out, c->n_sms, stream)
+                                 : launch_fused_full_w128(c->T, c->M, Q, c->mode, out, c->n_sms, stream);
+        if (n < 0) return launch_failed(c, n, "full-query kernel (F, dtype, in_dim <= 128, out_dim <= 4)");
+        p = OO_PATH_FULL;
     } else {
-        n = launch_fused_tm(c->T, c->M, Q, d_rgb, c->n_sms, stream);
-        if (n < 0 && c->path == OO_PATH_AUTO) {      // e.g. a first layer wider than TMEM allows: try shared-memory A, then mma.sync
-            p = OO_PATH_FUSED_TC;
-            n = launch_fused_tc(c->T, c->M, Q, d_rgb, c->n_sms, stream);
-            if (n < 0) {
-                p = OO_PATH_FUSED_MMA;
-                n = launch_fused_mma(c->T, c->M, Q, d_rgb, c->n_sms, stream);
+        const bool fast = c->plan_ok && fast_shape_supported(c->T.n_levels, c->T.F, c->T.f32 != 0);
+        if (p == OO_PATH_AUTO) p = !fast ? OO_PATH_GENERIC : OO_PATH_FUSED_TC_TMEM;
+        if (p != OO_PATH_GENERIC && !fast)
+            return fail(c, OO_ERR_UNSUPPORTED, "no specialised kernel for L=%u F=%u (or the tree has no hop plan); use OO_PATH_GENERIC/AUTO", c->T.n_levels, c->T.F);
+        Q = make_qp(&qd);
+        Q.dbg_slot = dbg.slot; Q.dbg_texel = dbg.index;
+        if (c->info.presorted_last_query && dbg.on()) Q.out_idx = c->d_bidx;
+        // OO_PATH_AUTO walks down the chain until a kernel exists for the shape: activations in tensor memory -> A tile in
+        // shared memory -> mma.sync -> features through HBM.  An explicit path runs that kernel or fails.
+        const bool walk = c->path == OO_PATH_AUTO;
+        n = -1;
+        if (p == OO_PATH_FUSED_TC_TMEM) {
+            n = dbg.on() ? launch_fused_tm_dbg(c->T, c->M, Q, out, c->n_sms, stream) : launch_fused_tm(c->T, c->M, Q, out, c->n_sms, stream);
+            if (n == -1 && walk) p = OO_PATH_FUSED_TC;
+        }
+        if (n == -1 && p == OO_PATH_FUSED_TC) {
+            n = launch_fused_tc(c->T, c->M, Q, out, c->n_sms, stream, dbg.on());
+            if (n == -1 && walk) p = OO_PATH_FUSED_MMA;
+        }
+        if (n == -1 && p == OO_PATH_FUSED_MMA) {
+            n = launch_fused_mma(c->T, c->M, Q, out, c->n_sms, stream, dbg.on());
+            if (n == -1 && walk) p = OO_PATH_UNFUSED;
+        }
+        if (n == -1 && (p == OO_PATH_GENERIC || p == OO_PATH_UNFUSED)) {
+            const uint64_t bytes = q->n * (uint64_t)c->T.n_levels * c->T.texel_bytes;
+            if (oo_status st = need_feat(c, bytes)) return st;
+            // the encode kernels are their own debug instances: they take the index outputs as they are
+            QueryParams Qe = Q;
+            if (c->info.presorted_last_query) Qe.out_idx = nullptr;     // features stay in processing order for the MLP kernel ...
+            EncodeOut O{c->d_feat, nullptr, nullptr};
+            if (dbg.on() && !c->info.presorted_last_query) { O.slot = dbg.slot; O.texel = dbg.index; }
+            n = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Qe, O, c->tree_max_depth, stream) : launch_encode_fast(c->T, Qe, O, c->n_sms, stream);
+            if (n < 0) return launch_failed(c, n, "encode kernel");
+            count(c, n);
+            if (dbg.on() && c->info.presorted_last_query) {             // ... so binned debug rows take a second, index-only pass
+                QueryParams Qi = Q;
+                Qi.out_idx = c->d_bidx;
+                EncodeOut Oi{nullptr, dbg.slot, dbg.index};
+                const int k = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Qi, Oi, c->tree_max_depth, stream) : launch_encode_fast(c->T, Qi, Oi, c->n_sms, stream);
+                if (k < 0) return launch_failed(c, k, "encode kernel");
+                count(c, k);
             }
+            n = launch_mlp_rows(c->T, c->M, Qe, c->d_feat, out, c->n_sms, stream);
+        }
+        if (n < 0) return launch_failed(c, n, path_name(p));
+        if (walk && p != OO_PATH_FUSED_TC_TMEM) {
+            char buf[256];
+            snprintf(buf, sizeof buf, "OO_PATH_AUTO resolved to %s for L=%u F=%u %s, in_dim %u, out_dim %u%s", path_name(p), c->T.n_levels, c->T.F,
+                     c->T.f32 ? "fp32" : "fp16", c->M.in_dim, c->M.out_dim, c->plan_ok ? "" : " (the tree has no hop plan)");
+            c->note = buf;
+        } else {
+            c->note.clear();
         }
     }
-    if (n < 0) return fail(c, OO_ERR_UNSUPPORTED, "requested kernel path %d is not available for this shape", (int)p);
     count(c, n);
-    if (c->info.presorted_last_query) count(c, launch_unbin(c->d_brgb, c->d_binv, q->n, c->M.out_dim, d_out, c->n_sms, stream));
+    if (c->info.presorted_last_query) count(c, launch_unbin(c->d_brgb, c->d_binv, q->n, c->M.out_dim, d_rgb, c->n_sms, stream));
     c->info.path_last_query = (uint32_t)p;
-    return check_async(c);
+    return check_after(c);
 }
 
 extern "C" OO_API oo_status oo_query(oo_ctx* c, const oo_queries* q, float* d_rgb, void* cuda_stream) {
     if (!c) return OO_ERR_INVALID_ARG;
     DeviceGuard g(c->device);
     return query_device(c, q, d_rgb, (cudaStream_t)cuda_stream);
+}
+
+extern "C" OO_API oo_status oo_query_debug(oo_ctx* c, const oo_queries* q, float* d_rgb, int32_t* d_slot, int16_t* d_index, void* cuda_stream) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    DeviceGuard g(c->device);
+    DebugOut dbg;
+    dbg.slot = d_slot;
+    dbg.index = d_index;
+    return query_device(c, q, d_rgb, (cudaStream_t)cuda_stream, dbg);
+}
+
+extern "C" OO_API oo_status oo_set_host_chunks(oo_ctx* c, uint32_t n_chunks) {
+    if (!c) return OO_ERR_INVALID_ARG;
+    if (n_chunks > (uint32_t)oo_ctx::kMaxChunks) return fail(c, OO_ERR_INVALID_ARG, "n_chunks %u outside 0..%d", n_chunks, oo_ctx::kMaxChunks);
+    c->host_chunks = (int)n_chunks;
+    return OO_OK;
 }
 
 extern "C" OO_API oo_status oo_query_host(oo_ctx* c, const oo_queries* q, float* h_rgb, void* cuda_stream) {
@@ -935,43 +1060,58 @@ extern "C" OO_API oo_status oo_query_host(oo_ctx* c, const oo_queries* q, float*
     }
     // Chunked three-stage pipeline: copy-in of chunk i+1 (s_h2d) overlaps the kernel of chunk i (caller's stream) and the
     // copy-out of chunk i-1 (s_d2h); PCIe is full duplex, so a frame costs about its copy-in time instead of the sum of the three.
-    // Chunks are whole multiples of 128-query tiles and at least 64 Ki queries, so every chunk still fills the persistent grid.
-    // Measured on B200 (config 1, pinned buffers): 1 chunk 1.07-1.10 ms, 2: 0.99, 4: 0.98, 8: 1.01-1.03, 16: 1.15 ms; copy-in slows
-    // ~12 % while copy-out shares the link, so the floor is ~0.85 ms of copy-in + the last chunk's kernel and copy-out.
+    // Chunks are whole multiples of 128-query tiles.  The exposed tail is the LAST chunk's kernel + copy-out and the exposed head
+    // the FIRST chunk's copy-in, so the chunk count follows the batch size (oo_set_host_chunks overrides): about 256 Ki queries per
+    // chunk, at least 2 and at most 8 chunks from 128 Ki queries on, one chunk below that.
+    // Measured on B200 (config 1, pinned buffers): 1 chunk 1.07-1.10 ms, 2: 0.99, 4: 0.98, 8: 1.01-1.03, 16: 1.15 ms.
     const uint64_t n = q->n;
-    static const int want = [] { const char* e = getenv("OO_HOST_CHUNKS"); const int v = e ? atoi(e) : 0; return v > 0 ? std::min(v, oo_ctx::kMaxChunks) : 4; }();
+    int want = c->host_chunks;
+    if (want <= 0) want = n < (1u << 17) ? 1 : (int)std::min<uint64_t>(8, std::max<uint64_t>(2, n >> 18));
     uint64_t chunk = (n + want - 1) / want;
-    chunk = std::max<uint64_t>((chunk + 127) & ~127ull, 65536);
+    chunk = (chunk + 127) & ~127ull;
     const int n_chunks = (int)((n + chunk - 1) / chunk);
     const uint32_t od = c->M.out_dim;
-    OO_CUDA(c, cudaEventRecord(c->ev_start, stream));
-    OO_CUDA(c, cudaStreamWaitEvent(c->s_h2d, c->ev_start, 0));
-    OO_CUDA(c, cudaStreamWaitEvent(c->s_d2h, c->ev_start, 0));
+    // any failure below leaves copies from / to the caller's host buffers in flight on the library's streams: drain all three
+    // before returning, so that the caller may free or reuse its buffers whatever the status
+    auto drain = [&](oo_status st) {
+        cudaStreamSynchronize(c->s_h2d); cudaStreamSynchronize(c->s_d2h); cudaStreamSynchronize(stream);
+        return st;
+    };
+#define OO_PIPE(call)                                                                                                         \
+    do {                                                                                                                      \
+        cudaError_t e_ = (call);                                                                                              \
+        if (e_ != cudaSuccess) {                                                                                              \
+            (void)cudaGetLastError();                                                                                         \
+            if (is_fatal(e_)) c->sticky = e_;                                                                                 \
+            return drain(fail(c, OO_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)));                                      \
+        }                                                                                                                     \
+    } while (0)
+    OO_PIPE(cudaEventRecord(c->ev_start, stream));
+    OO_PIPE(cudaStreamWaitEvent(c->s_h2d, c->ev_start, 0));
+    OO_PIPE(cudaStreamWaitEvent(c->s_d2h, c->ev_start, 0));
     for (int i = 0; i < n_chunks; ++i) {
         const uint64_t o = (uint64_t)i * chunk, m = std::min(chunk, n - o);
-        OO_CUDA(c, cudaMemcpyAsync(c->d_qx + o * 3, q->x + o * 3, m * 12, cudaMemcpyHostToDevice, c->s_h2d));
-        OO_CUDA(c, cudaMemcpyAsync(c->d_qn + o * 3, q->nrm + o * 3, m * 12, cudaMemcpyHostToDevice, c->s_h2d));
-        OO_CUDA(c, cudaMemcpyAsync(c->d_qw + o * 3, q->wo + o * 3, m * 12, cudaMemcpyHostToDevice, c->s_h2d));
-        if (q->n_extra) OO_CUDA(c, cudaMemcpyAsync(c->d_qe + o * q->n_extra, q->extra + o * q->n_extra, m * 4 * q->n_extra, cudaMemcpyHostToDevice, c->s_h2d));
-        if (q->disparity) OO_CUDA(c, cudaMemcpyAsync(c->d_qd + o, q->disparity + o, m * 4, cudaMemcpyHostToDevice, c->s_h2d));
-        OO_CUDA(c, cudaEventRecord(c->ev_in[i], c->s_h2d));
-        OO_CUDA(c, cudaStreamWaitEvent(stream, c->ev_in[i], 0));
+        OO_PIPE(cudaMemcpyAsync(c->d_qx + o * 3, q->x + o * 3, m * 12, cudaMemcpyHostToDevice, c->s_h2d));
+        OO_PIPE(cudaMemcpyAsync(c->d_qn + o * 3, q->nrm + o * 3, m * 12, cudaMemcpyHostToDevice, c->s_h2d));
+        OO_PIPE(cudaMemcpyAsync(c->d_qw + o * 3, q->wo + o * 3, m * 12, cudaMemcpyHostToDevice, c->s_h2d));
+        if (q->n_extra) OO_PIPE(cudaMemcpyAsync(c->d_qe + o * q->n_extra, q->extra + o * q->n_extra, m * 4 * q->n_extra, cudaMemcpyHostToDevice, c->s_h2d));
+        if (q->disparity) OO_PIPE(cudaMemcpyAsync(c->d_qd + o, q->disparity + o, m * 4, cudaMemcpyHostToDevice, c->s_h2d));
+        OO_PIPE(cudaEventRecord(c->ev_in[i], c->s_h2d));
+        OO_PIPE(cudaStreamWaitEvent(stream, c->ev_in[i], 0));
         oo_queries dq = *q;
         dq.n = m;
         dq.x = c->d_qx + o * 3; dq.nrm = c->d_qn + o * 3; dq.wo = c->d_qw + o * 3;
         dq.extra = q->n_extra ? c->d_qe + o * q->n_extra : nullptr;
         dq.disparity = q->disparity ? c->d_qd + o : nullptr;
-        if (oo_status st = query_device(c, &dq, c->d_rgb + o * od, stream)) {
-            cudaStreamSynchronize(c->s_h2d); cudaStreamSynchronize(c->s_d2h); cudaStreamSynchronize(stream);
-            return st;
-        }
-        OO_CUDA(c, cudaEventRecord(c->ev_k[i], stream));
-        OO_CUDA(c, cudaStreamWaitEvent(c->s_d2h, c->ev_k[i], 0));
-        OO_CUDA(c, cudaMemcpyAsync(h_rgb + o * od, c->d_rgb + o * od, m * 4 * od, cudaMemcpyDeviceToHost, c->s_d2h));
+        if (oo_status st = query_device(c, &dq, c->d_rgb + o * od, stream)) return drain(st);
+        OO_PIPE(cudaEventRecord(c->ev_k[i], stream));
+        OO_PIPE(cudaStreamWaitEvent(c->s_d2h, c->ev_k[i], 0));
+        OO_PIPE(cudaMemcpyAsync(h_rgb + o * od, c->d_rgb + o * od, m * 4 * od, cudaMemcpyDeviceToHost, c->s_d2h));
     }
-    OO_CUDA(c, cudaEventRecord(c->ev_out, c->s_d2h));
-    OO_CUDA(c, cudaStreamWaitEvent(stream, c->ev_out, 0));
-    OO_CUDA(c, cudaStreamSynchronize(stream));
+    OO_PIPE(cudaEventRecord(c->ev_out, c->s_d2h));
+    OO_PIPE(cudaStreamWaitEvent(stream, c->ev_out, 0));
+    OO_PIPE(cudaStreamSynchronize(stream));
+#undef OO_PIPE
     return OO_OK;
 }
 
@@ -1012,14 +1152,14 @@ extern "C" OO_API oo_status oo_raycast(oo_ctx* c, const oo_camera_desc* cam, flo
         cr = r[0] * r[0] + r[1] * r[1] + r[2] * r[2];
     }
     if (!(fl > 0.0) || !(cr > 0.0)) return fail(c, OO_ERR_INVALID_ARG, "degenerate camera: look == eye, or up parallel to the view direction");
-    if (oo_status st = check_async(c)) return st;
+    if (oo_status st = check_before(c)) return st;
     if (n == 0) return OO_OK;
     DeviceGuard g(c->device);
     const int k = launch_raycast((const double*)c->d_spheres, c->n_spheres, c->scene_lo, c->scene_hi, cam->eye, cam->look, cam->up,
                                  cam->vfov_deg, cam->width, cam->height, d_x, d_nrm, d_wo, d_surf, (cudaStream_t)cuda_stream);
-    if (k < 0) return fail(c, OO_ERR_UNSUPPORTED, "ray-cast kernel unavailable for this scene size");
+    if (k < 0) return launch_failed(c, k, "ray-cast kernel (scene size)");
     count(c, k);
-    return check_async(c);
+    return check_after(c);
 }
 
 extern "C" OO_API oo_status oo_read_padded_map(oo_ctx* c, uint32_t level, uint32_t slot, void* h_out) {

@@ -221,12 +221,9 @@ int launch_disparity(const GridParams& G, const MlpParams& M, const QueryParams&
     const uint64_t blocks = (n_tiles + kNWG - 1) / kNWG;
     const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms ? blocks : (uint64_t)n_sms);
     const uint32_t smem = ((M.image_tc_bytes + 127) & ~127u) + 128;
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(disparity_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024);
-        attr = true;
-    }
     if (smem > 64 * 1024) return -1;
+    static std::atomic<uint64_t> opted{0};
+    if (!opt_in_smem(opted, (const void*)disparity_kernel, 64 * 1024)) return kLaunchCudaError;
     disparity_kernel<<<grid, kNWG * 128, smem, stream>>>(G, M, Q, disparity, features, (uint32_t)n_tiles);
     return 1;
 }

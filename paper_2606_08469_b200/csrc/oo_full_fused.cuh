@@ -19,7 +19,7 @@
 
 namespace oo {
 
-template <int F, bool F32, bool VERTEX, bool TRI8, bool SHIFTED, int W, int KS, int NTEAM>
+template <int F, bool F32, bool VERTEX, bool TRI8, bool SHIFTED, int W, int KS, int NTEAM, bool DBG>
 __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
     fused_full_kernel(const __grid_constant__ TreeParams T, const __grid_constant__ MlpParams M,
                       const __grid_constant__ QueryParams Q, const __grid_constant__ FullMode mode, float* __restrict__ rgb,
@@ -111,7 +111,13 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
         {
             Station<NJ> st;
             station_init<NJ>(T, s_dense, x, st);
-            const FullDebug dbg{nullptr, nullptr};
+            FullDebug dbg{nullptr, nullptr};
+            if constexpr (DBG) {         // oo_query_debug: this query's [L][NJ] slot and [L][NJ][3] index rows (binned: out_idx's)
+                const uint64_t t = (uint64_t)tile * 128 + row;
+                const uint64_t r = Q.out_idx ? Q.out_idx[t < Q.n ? t : Q.n - 1] : __float_as_uint(s_q[9 * 128]);
+                if (valid && Q.dbg_slot) dbg.slot = Q.dbg_slot + r * L * NJ;
+                if (valid && Q.dbg_texel) dbg.cell = Q.dbg_texel + r * L * NJ * 3;
+            }
             for (uint32_t l = 0; l < L; ++l) {
                 const bool mine = KS == 1 || (l % KS) == part;
                 float h[F];
@@ -245,7 +251,7 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
-template <int F, bool F32, bool VERTEX, bool TRI8, bool SHIFTED, int W, int KS, int NTEAM>
+template <int F, bool F32, bool VERTEX, bool TRI8, bool SHIFTED, int W, int KS, int NTEAM, bool DBG>
 static int launch_full_inst(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const FullModeH& mode, float* rgb,
                             int n_sms, uint32_t team_cols, cudaStream_t stream) {
     const uint64_t n_tiles = (Q.n + 127) / 128;
@@ -253,12 +259,9 @@ static int launch_full_inst(const TreeParams& T, const MlpParams& M, const Query
     const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms ? blocks : (uint64_t)n_sms);
     const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + NTEAM * (11 + Q.n_extra) * 128 * 4 + 128;
     if (smem > 227 * 1024) return -1;
-    auto kern = fused_full_kernel<F, F32, VERTEX, TRI8, SHIFTED, W, KS, NTEAM>;
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
-        attr = true;
-    }
+    auto kern = fused_full_kernel<F, F32, VERTEX, TRI8, SHIFTED, W, KS, NTEAM, DBG>;
+    static std::atomic<uint64_t> opted{0};
+    if (!opt_in_smem(opted, (const void*)kern, 227 * 1024)) return kLaunchCudaError;
     kern<<<grid, NTEAM * KS * 128, smem, stream>>>(T, M, Q, mode, rgb, (uint32_t)n_tiles, team_cols);
     return 1;
 }
@@ -268,13 +271,13 @@ static int launch_full_inst(const TreeParams& T, const MlpParams& M, const Query
     X(f, t, true, false, false) X(f, t, true, false, true) X(f, t, true, true, false) X(f, t, true, true, true)
 
 // dispatch over (F, dtype, vertex, tri8, shifted) for a fixed (W, KS, NTEAM)
-template <int W, int KS, int NTEAM>
+template <int W, int KS, int NTEAM, bool DBG>
 static int launch_full_w(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const FullModeH& mode, float* rgb,
                          int n_sms, uint32_t team_cols, cudaStream_t stream) {
     const bool vertex = T.vertex != 0, tri8 = mode.tri8 != 0, shifted = mode.lookup == OO_LOOKUP_SHIFTED;
 #define X(f, t, v, s8, sh)                                                                                 \
     if (T.F == f && (T.f32 != 0) == t && vertex == v && tri8 == s8 && shifted == sh)                       \
-        return launch_full_inst<f, t, v, s8, sh, W, KS, NTEAM>(T, M, Q, mode, rgb, n_sms, team_cols, stream);
+        return launch_full_inst<f, t, v, s8, sh, W, KS, NTEAM, DBG>(T, M, Q, mode, rgb, n_sms, team_cols, stream);
     OO_FULL_MODES(X, 4, true)
     OO_FULL_MODES(X, 8, false)
     OO_FULL_MODES(X, 16, false)

@@ -1,16 +1,16 @@
-// oo_full_fused_w128.cu — instances of the fused full-query kernel (oo_full_fused.cuh) for decoders of width 128:
+// oo_full_fused_w128.cu — the product instances of the fused full-query kernel (oo_full_fused.cuh) for decoders of width 128:
 // teams of 2 x 128 threads, 2 teams (tiles in flight) per SM.
 #include "oo_full_fused.cuh"
 
 namespace oo {
 
 int launch_fused_full_w128(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const FullModeH& mode, float* rgb,
-                           int n_sms, cudaStream_t stream) {
+        int n_sms, cudaStream_t stream) {
     if (Q.n == 0) return 0;
     if (M.out_dim > 4 || !M.image_tc || M.k1 > 128 || M.width != 128) return -1;
     const uint32_t team_cols = 128 + (M.k1 / 2 > 128 / 2 ? M.k1 / 2 : 128 / 2);
     if (2 * team_cols > 512) return -1;
-    return launch_full_w<128, 2, 2>(T, M, Q, mode, rgb, n_sms, team_cols, stream);
+    return launch_full_w<128, 2, 2, false>(T, M, Q, mode, rgb, n_sms, team_cols, stream);
 }
 
 }  // namespace oo

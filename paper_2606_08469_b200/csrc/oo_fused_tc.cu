@@ -32,7 +32,7 @@ constexpr int kTileRows = 128;
 // shared; every warpgroup owns an A tile, 64 TMEM columns, an mbarrier and a query staging buffer into which the NEXT
 // tile's (x, n, wo, extra, index) are prefetched with cp.async while the current tile is gathered and decoded, so the
 // cold HBM latency of the query stream is hidden behind the previous tile.
-template <int L, int F, bool F32, int NWG, int MINB>
+template <int L, int F, bool F32, int NWG, int MINB, bool DBG>
 __global__ void __launch_bounds__(NWG * 128, MINB) fused_tc_kernel(const __grid_constant__ TreeParams T,
                                                                 const __grid_constant__ MlpParams M,
                                                                 const __grid_constant__ QueryParams Q,
@@ -121,19 +121,25 @@ __global__ void __launch_bounds__(NWG * 128, MINB) fused_tc_kernel(const __grid_
         // ------------------------------------------------------------------ gather: one query per thread
         Encoded<L, F, F32> e;
         locate<L, F, F32>(T, s_dense, x, w, e);
+        uint64_t dbg_row = 0;
+        if constexpr (DBG) {             // where this query's index rows go: its own index (binned queries: out_idx's)
+            const uint64_t t = (uint64_t)tile * kTileRows + row;
+            dbg_row = Q.out_idx ? Q.out_idx[t < Q.n ? t : Q.n - 1] : __float_as_uint(s_q[9 * 128]);
+        }
+        const auto dbg = make_dbg<DBG>(Q, L, dbg_row, valid);
         uint8_t* a_row = s_a + row * 16;
         constexpr int NB = (F * (F32 ? 4 : 2) == 16) ? (L < 4 ? L : 4) : (F * (F32 ? 4 : 2) == 32 ? 2 : 1);   // levels per load batch (<= 64 data registers)
 #pragma unroll
         for (int l0 = 0; l0 < L; l0 += NB) {
             float h[NB][F];
             if (l0 + NB <= L) {
-                gather_levels<F, F32, NB>(&T.lv[l0], &e.slot[l0], e.uv, h);
+                gather_levels<F, F32, NB>(&T.lv[l0], &e.slot[l0], e.uv, h, dbg, l0);
             } else {     // ragged last batch: one level at a time
 #pragma unroll
                 for (int b = 0; b < NB; ++b)
                     if (l0 + b < L) {
                         const Tap tp = level_tap(e.uv, T.lv[l0 + b].half_r, T.lv[l0 + b].off);
-                        gather_level<F, F32>(T.lv[l0 + b], e.slot[l0 + b], tp, h[b]);
+                        gather_level<F, F32>(T.lv[l0 + b], e.slot[l0 + b], tp, h[b], dbg, l0 + b);
                     }
             }
 #pragma unroll
@@ -271,7 +277,7 @@ bool tc_shape_supported(uint32_t L, uint32_t F, bool f32) {
     return false;
 }
 
-template <int NWG, int MINB>
+template <int NWG, int MINB, bool DBG>
 static int launch_tc_nwg(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, uint32_t smem,
                          cudaStream_t stream) {
     const uint64_t n_tiles = (Q.n + kTileRows - 1) / kTileRows;
@@ -279,12 +285,9 @@ static int launch_tc_nwg(const TreeParams& T, const MlpParams& M, const QueryPar
     const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms * MINB ? blocks : (uint64_t)n_sms * MINB);
 #define X(l, f, t)                                                                                                        \
     if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                                               \
-        static bool attr = false;                                                                                         \
-        if (!attr) {                                                                                                      \
-            cudaFuncSetAttribute(fused_tc_kernel<l, f, t, NWG, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024); \
-            attr = true;                                                                                                  \
-        }                                                                                                                 \
-        fused_tc_kernel<l, f, t, NWG, MINB><<<grid, NWG * 128, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles);                \
+        static std::atomic<uint64_t> opted{0};                                                                            \
+        if (!opt_in_smem(opted, (const void*)fused_tc_kernel<l, f, t, NWG, MINB, DBG>, 227 * 1024)) return kLaunchCudaError; \
+        fused_tc_kernel<l, f, t, NWG, MINB, DBG><<<grid, NWG * 128, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles);     \
         return 1;                                                                                                         \
     }
     OO_TC_SHAPES(X)
@@ -293,7 +296,8 @@ static int launch_tc_nwg(const TreeParams& T, const MlpParams& M, const QueryPar
 }
 
 // Largest warpgroup count per SM-resident block whose shared memory fits (6, else 4); -1 if the shape has no instance.
-int launch_fused_tc(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, cudaStream_t stream) {
+template <bool DBG>
+static int launch_fused_tc_impl(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, cudaStream_t stream) {
     if (Q.n == 0) return 0;
     if (M.out_dim > 4 || !M.image_tc) return -1;
     const uint32_t a_chunks = (M.k1 > 64 ? M.k1 : 64) / 8;
@@ -301,10 +305,15 @@ int launch_fused_tc(const TreeParams& T, const MlpParams& M, const QueryParams& 
     const uint32_t fixed = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + 64 + 64;
     const uint32_t limit = 227 * 1024;
     // residency: measured on config 1 (B200): 3 warpgroups x 2 blocks/SM 72.9 us, 6 x 1 75.4 us, 5 x 1 78.6 us, 4 x 1 80.7 us
-    if (2 * (fixed + 3 * per_wg + 1024) <= 228 * 1024) return launch_tc_nwg<3, 2>(T, M, Q, rgb, n_sms, fixed + 3 * per_wg, stream);
-    if (fixed + 6 * per_wg <= limit) return launch_tc_nwg<6, 1>(T, M, Q, rgb, n_sms, fixed + 6 * per_wg, stream);
-    if (fixed + 4 * per_wg <= limit) return launch_tc_nwg<4, 1>(T, M, Q, rgb, n_sms, fixed + 4 * per_wg, stream);
+    if (2 * (fixed + 3 * per_wg + 1024) <= 228 * 1024) return launch_tc_nwg<3, 2, DBG>(T, M, Q, rgb, n_sms, fixed + 3 * per_wg, stream);
+    if (fixed + 6 * per_wg <= limit) return launch_tc_nwg<6, 1, DBG>(T, M, Q, rgb, n_sms, fixed + 6 * per_wg, stream);
+    if (fixed + 4 * per_wg <= limit) return launch_tc_nwg<4, 1, DBG>(T, M, Q, rgb, n_sms, fixed + 4 * per_wg, stream);
     return -1;
+}
+
+// dbg: the instances with the index sink compiled in (oo_query_debug)
+int launch_fused_tc(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, cudaStream_t stream, bool dbg) {
+    return dbg ? launch_fused_tc_impl<true>(T, M, Q, rgb, n_sms, stream) : launch_fused_tc_impl<false>(T, M, Q, rgb, n_sms, stream);
 }
 
 }  // namespace oo

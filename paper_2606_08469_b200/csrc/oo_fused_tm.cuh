@@ -1,0 +1,382 @@
+// oo_fused_tm.cuh — fused encode + MLP on tcgen05 with the activations resident in TENSOR MEMORY (OO_PATH_FUSED_TC_TMEM).
+//
+// Same arithmetic as oo_fused_tc.cu; the A operand of every layer lives in TMEM instead of shared memory:
+//   gather (registers, fp32) -> fp16 row -> tcgen05.st into this thread's TMEM lane (two halves per 32-bit column)
+//   -> tcgen05.mma.kind::f16 with A from TMEM, B (weights) from shared memory, D in TMEM
+//   -> tcgen05.ld own row of D -> ReLU -> fp16 -> tcgen05.st as the next layer's A -> ... -> output layer -> exp -> RGB.
+// What that buys (ncu, config 1, oo_fused_tc.cu): the shared-memory A tile cost 540 of ~1500 L1 data-pipe wavefronts per
+// 128-query tile (l1tex 66 % busy, the busiest unit) and 2 x 100 KB of shared memory that left the gathers ~28 KB of L1.
+// Here a block needs only the descent tables, the weight image and 5 KB of query staging per warpgroup.
+//
+// TMEM columns of one warpgroup (stride S = 64 + max(32, k1/2)); D is 64 fp32 columns, A is K/2 columns:
+//   even layer:  A at [64, 64 + K/2)   D at [0, 64)
+//   odd  layer:  A at [0, 32)          D at [32, 96)
+// so the epilogue of a layer writes the next A over columns of D that it has already read (own lane only):
+//   even: ld D[0,32) -> st A'[0,16);  ld D[32,64) -> st A'[16,32)
+//   odd : ld D[64,96) -> st A'[80,96) (k = 32..63);  ld D[32,64) -> st A'[64,80) (k = 0..31)
+// One persistent block per SM (it allocates all 512 columns) with NWG = 512 / S warpgroups (5 when k1 <= 64).
+//
+// Included by oo_fused_tm.cu (DBG = false: the product instances) and oo_fused_tm_dbg.cu (DBG = true: the same kernels with
+// the index sink of oo_query_debug compiled in, see IndexDbg in oo_device.cuh).
+#pragma once
+#include <cstdio>
+
+#include "oo_device.cuh"
+#include "oo_tc_ptx.cuh"
+
+namespace oo {
+
+namespace {
+constexpr int kRows = 128;
+
+// ReLU + fp16 pack of 32 accumulator columns -> 16 registers
+__device__ __forceinline__ void relu_pack32(const uint32_t (&r)[32], uint32_t (&p)[16]) {
+#pragma unroll
+    for (int c = 0; c < 16; ++c) p[c] = pack_half2_relu(__uint_as_float(r[2 * c]), __uint_as_float(r[2 * c + 1]));
+}
+}  // namespace
+
+// PIPE (chosen at launch for fp16 trees whose first two used levels are dense and the rest hops, i.e. the BASELINE.json configs):
+// the hop chain and the gathers overlap.  Stage l resolves slot l from the hop load issued one stage earlier, issues the next
+// hop and the taps of level l, and consumes the taps of level l-RD (RD = 2, or 3 for 16-byte texels): a query exposes max(hop, taps) once per hop level plus one
+// last gather (4 latencies for L = 5) instead of every hop and then every gather batch (6).  Same taps, same weights, same
+// accumulation order per level: bit-identical to the batched form.
+// KS (first layers wider than 64 inputs, L*F >= 64): layer 0 runs as TWO MMA groups over the same 32 A columns.  The first 64
+// inputs (the levels below feature 64) are multiplied as soon as they are stored; the rest of the row (later levels, attributes,
+// padding) is gathered and packed while that MMA is in flight, stored over the same columns once it has completed, and
+// accumulated by the second group.  A tile then needs 96 TMEM columns like the narrow configs instead of 64 + k1/2, so five
+// warpgroups fit where four did (config 3: k1 = 96, 112 columns), at the price of one more MMA round trip per tile.
+template <int L, int F, bool F32, int NWG, bool PIPE = false, bool KS = false, bool DBG = false>
+__global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_constant__ TreeParams T,
+                                                               const __grid_constant__ MlpParams M,
+                                                               const __grid_constant__ QueryParams Q,
+                                                               float* __restrict__ rgb, uint32_t n_tiles, uint32_t wg_cols) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    const uint32_t dense_bytes = (T.dense_ints * 4 + 127) & ~127u;
+    const uint32_t q_words = 10 + Q.n_extra;                         // x3 n3 wo3 index extras, each [128] words
+    const uint32_t q_bytes = q_words * kRows * 4;
+    int32_t* s_dense = (int32_t*)smem;
+    uint8_t* s_w = smem + dense_bytes;
+    uint8_t* s_stage = s_w + ((M.image_tc_bytes + 127) & ~127u);
+    uint64_t* s_bar = (uint64_t*)(s_stage + NWG * q_bytes);      // one per warpgroup, then tables, then weights
+    uint32_t* s_tmem = (uint32_t*)(s_bar + NWG + 2);
+
+    const uint32_t wg = threadIdx.x >> 7, row = threadIdx.x & 127, warp = threadIdx.x >> 5;
+    // Prologue: the descent tables and the weight image arrive by two bulk asynchronous copies that thread 0 issues before
+    // anything else; the tables are awaited by every thread before its first descent, the weights only by the warp that issues
+    // the MMAs, right before its first one (both travel through the async proxy: no proxy fence, no block barrier for them).
+    // Before: 512-640 threads looping LDG.128 -> STS over 54 KB of cold lines, then fence.proxy.async + __syncthreads.
+    const uint32_t bar_d = smem_u32(&s_bar[NWG]), bar_w = smem_u32(&s_bar[NWG + 1]);
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int k = 0; k < NWG + 2; ++k) mbar_init(smem_u32(&s_bar[k]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        mbar_expect_tx(bar_d, T.dense_ints * 4);
+        bulk_g2s(smem_u32(s_dense), T.dense, T.dense_ints * 4, bar_d);
+        mbar_expect_tx(bar_w, M.image_tc_bytes);
+        bulk_g2s(smem_u32(s_w), M.image_tc, M.image_tc_bytes, bar_w);
+    }
+    float* s_q = (float*)(s_stage + wg * q_bytes) + row;             // word k of my row: s_q[k * 128]
+    const uint32_t q_addr = smem_u32(s_q);
+    auto prefetch = [&](uint32_t tile) {
+        const uint64_t t = (uint64_t)tile * kRows + row;
+        const uint64_t tt = t < Q.n ? t : Q.n - 1;
+        const uint32_t qi = Q.perm ? __ldg(Q.perm + tt) : (uint32_t)tt;
+        const float* px = Q.x + (size_t)qi * 3;
+        const float* pn = Q.nrm + (size_t)qi * 3;
+        const float* pw = Q.wo + (size_t)qi * 3;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+            cp_async4(q_addr + (k) * 512, px + k);
+            cp_async4(q_addr + (3 + k) * 512, pn + k);
+            cp_async4(q_addr + (6 + k) * 512, pw + k);
+        }
+        for (uint32_t k = 0; k < Q.n_extra; ++k) cp_async4(q_addr + (10 + k) * 512, Q.extra + (size_t)qi * Q.n_extra + k);
+        s_q[9 * 128] = __uint_as_float(qi);
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+
+    // Warpgroup wg of block b takes tiles wg*grid + b, + grid*NWG, ...: the n_tiles mod (grid*NWG) tiles of the last, partial
+    // round then land one per SM (a lone warpgroup finishes its tile about twice as fast as five sharing an SM) instead of five
+    // per SM on a few SMs.  Measured on B200: config 1 61.1 -> 60.1 us, config 3 333.3 -> 329.4 us.
+    uint32_t tile = wg * gridDim.x + blockIdx.x;
+    if (tile < n_tiles) prefetch(tile);       // the first tile's queries travel while TMEM is allocated and the tables arrive
+    if (warp == 0) {
+        tmem_alloc(smem_u32(s_tmem), 512);
+        tmem_relinquish();
+    }
+    fence_before_sync();
+    __syncthreads();
+    fence_after_sync();
+    const uint32_t tmem_wg = *s_tmem + wg * wg_cols;                 // this warpgroup's columns
+    const uint32_t tmem_lane = tmem_wg + ((row & ~31u) << 16);       // ... and this warp's 32 lanes
+    const uint32_t w_addr = smem_u32(s_w), bar = smem_u32(&s_bar[wg]);
+    uint32_t phase = 0;
+    const bool leader_warp = row < 32;
+    constexpr uint32_t idesc_h = instr_desc(128, 64), idesc_o = instr_desc(128, 16);
+    const uint32_t tile_stride = gridDim.x * NWG;
+
+    mbar_wait(bar_d, 0);                  // descent tables in shared memory
+    bool w_ready = false;
+    for (; tile < n_tiles; tile += tile_stride) {
+        float x[3], w[3];
+        const bool valid = (uint64_t)tile * kRows + row < Q.n;
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+#pragma unroll
+        for (int k = 0; k < 3; ++k) { x[k] = s_q[k * 128]; w[k] = s_q[(6 + k) * 128]; }
+        // ------------------------------------------------------------------ gather: one query per thread -> A0 in TMEM
+        const uint32_t a0 = tmem_lane + 64;                          // layer 0 is even: A at [64, 64 + k1/2)
+        uint64_t dbg_row = 0;
+        if constexpr (DBG) {             // where this query's index rows go: its own index (binned queries: out_idx's)
+            const uint64_t t = (uint64_t)tile * kRows + row;
+            dbg_row = Q.out_idx ? Q.out_idx[t < Q.n ? t : Q.n - 1] : __float_as_uint(s_q[9 * 128]);
+        }
+        const auto dbg = make_dbg<DBG>(Q, L, dbg_row, valid);
+        constexpr int N_LATE = KS ? (L * F - 64) / 2 : 0;            // packed halves of the levels past input 64 (KS)
+        uint32_t late[N_LATE > 0 ? N_LATE : 1];
+        auto store_level = [&](int l, const float (&h)[F]) {
+            if constexpr (KS) {
+                if (l * F >= 64) {            // kept in registers until the first MMA group has read the A columns
+#pragma unroll
+                    for (int k = 0; k < F / 2; ++k) late[(l * F - 64) / 2 + k] = pack_half2(h[2 * k], h[2 * k + 1]);
+                    return;
+                }
+            }
+            if constexpr (F % 8 == 0) {
+#pragma unroll
+                for (int v = 0; v < F / 8; ++v)
+                    tmem_st4(a0 + (l * F) / 2 + 4 * v, pack_half2(h[8 * v], h[8 * v + 1]), pack_half2(h[8 * v + 2], h[8 * v + 3]),
+                             pack_half2(h[8 * v + 4], h[8 * v + 5]), pack_half2(h[8 * v + 6], h[8 * v + 7]));
+            } else {   // F == 4
+                tmem_st2(a0 + (l * 4) / 2, pack_half2(h[0], h[1]), pack_half2(h[2], h[3]));
+            }
+            if constexpr (KS) {
+                if ((l + 1) * F == 64) {      // inputs 0..63 of all 128 rows are in TMEM: first MMA group of layer 0
+                    tmem_wait_st();
+                    fence_before_sync();
+                    named_bar(1 + wg, 128);
+                    if (leader_warp) {
+                        if (!w_ready) {
+                            mbar_wait(bar_w, 0);
+                            w_ready = true;
+                        }
+                        fence_after_sync();
+                        umma_group_ts<4>(tmem_wg, tmem_wg + 64u, smem_desc(w_addr, 1024, 128), 2048 >> 4, idesc_h, 4u, bar);
+                    }
+                }
+            }
+        };
+        if constexpr (PIPE && L >= 3) {
+            gather_pipelined<L, F, F32>(T, s_dense, x, w, store_level, dbg);
+        } else {
+            Encoded<L, F, F32> e;
+            locate<L, F, F32>(T, s_dense, x, w, e);
+            constexpr int NB = (F * (F32 ? 4 : 2) == 16) ? (L < 4 ? L : 4) : (F * (F32 ? 4 : 2) == 32 ? 2 : 1);   // levels per load batch
+#pragma unroll
+            for (int l0 = 0; l0 < L; l0 += NB) {
+                float h[NB][F];
+                if (l0 + NB <= L) {
+                    gather_levels<F, F32, NB>(&T.lv[l0], &e.slot[l0], e.uv, h, dbg, l0);
+                } else {     // ragged last batch: one level at a time
+#pragma unroll
+                    for (int b = 0; b < NB; ++b)
+                        if (l0 + b < L) {
+                            const Tap tp = level_tap(e.uv, T.lv[l0 + b].half_r, T.lv[l0 + b].off);
+                            gather_level<F, F32>(T.lv[l0 + b], e.slot[l0 + b], tp, h[b], dbg, l0 + b);
+                        }
+                }
+#pragma unroll
+                for (int b = 0; b < NB; ++b) {
+                    const int l = l0 + b;
+                    if (l >= L) break;
+                    store_level(l, h[b]);
+                }
+            }
+        }
+        uint32_t qi;
+        const uint32_t aA = KS ? a0 - 32 : a0;   // KS: input k >= 64 lives at column (k - 64) / 2 of the same A region
+        if constexpr (KS) {
+            mbar_wait(bar, phase);                // the first MMA group has read inputs 0..63
+            phase ^= 1;
+            fence_after_sync();
+#pragma unroll
+            for (int v = 0; v < N_LATE / 4; ++v) tmem_st4(a0 + 4 * v, late[4 * v], late[4 * v + 1], late[4 * v + 2], late[4 * v + 3]);
+        }
+        {   // attributes + zero padding up to k1, read late from the staging buffer
+            float v[24];
+#pragma unroll
+            for (int k = 0; k < 24; ++k) v[k] = 0.0f;
+            constexpr int lead = (L * F) % 8;            // 0 or 4: position of n inside its 8-half unit
+#pragma unroll
+            for (int k = 0; k < 3; ++k) { v[lead + k] = s_q[(3 + k) * 128]; v[lead + 3 + k] = w[k]; }
+#pragma unroll
+            for (int k = 0; k < OO_MAX_EXTRA; ++k)
+                if ((uint32_t)k < Q.n_extra) v[lead + 6 + k] = s_q[(10 + k) * 128];
+            qi = __float_as_uint(s_q[9 * 128]);
+            constexpr int c0 = (L * F) / 8;              // first 8-half unit (4 columns) holding attributes
+            const uint32_t c_end = M.k1 / 8;
+            if constexpr (lead == 0) {
+                tmem_st4(aA + 4 * c0, pack_half2(v[0], v[1]), pack_half2(v[2], v[3]), pack_half2(v[4], v[5]), pack_half2(v[6], v[7]));
+            } else {
+                tmem_st2(aA + 4 * c0 + 2, pack_half2(v[4], v[5]), pack_half2(v[6], v[7]));
+            }
+            if (c0 + 1 < c_end)
+                tmem_st4(aA + 4 * (c0 + 1), pack_half2(v[8], v[9]), pack_half2(v[10], v[11]), pack_half2(v[12], v[13]), pack_half2(v[14], v[15]));
+            if (c0 + 2 < c_end)
+                tmem_st4(aA + 4 * (c0 + 2), pack_half2(v[16], v[17]), pack_half2(v[18], v[19]), pack_half2(v[20], v[21]), pack_half2(v[22], v[23]));
+        }
+        if (tile + tile_stride < n_tiles) prefetch(tile + tile_stride);
+        // ------------------------------------------------------------------ hidden layers
+        uint32_t w_off = 0;
+        for (uint32_t layer = 0; layer < M.n_hidden; ++layer) {
+            const uint32_t kt_n = (layer == 0 ? M.k1 : 64u) >> 4;
+            const bool second = KS && layer == 0;         // layer 0's inputs 64.. : 4 K-steps further into W0, accumulating
+            const bool odd = layer & 1u;
+            tmem_wait_st();              // my row of A is in TMEM
+            fence_before_sync();
+            named_bar(1 + wg, 128);
+            if (leader_warp) {
+                if (!w_ready) {
+                    mbar_wait(bar_w, 0);      // weight image in shared memory (first MMA of this warpgroup only)
+                    w_ready = true;
+                }
+                fence_after_sync();
+                umma_group_ts<8>(tmem_wg + (odd ? 32u : 0u), tmem_wg + (odd ? 0u : 64u), smem_desc(w_addr + w_off + (second ? 4u * 2048u : 0u), 1024, 128),
+                                 2048 >> 4, idesc_h, second ? kt_n - 4u : kt_n, bar, second ? 1u : 0u);
+            }
+            w_off += kt_n * 2 * 1024;
+            mbar_wait(bar, phase);
+            phase ^= 1;
+            fence_after_sync();
+            // epilogue: my row of D -> ReLU -> fp16 -> my row of the next layer's A (over columns of D already read)
+            // both halves of D are requested before the single wait::ld, so the second TMEM read hides behind the first
+            uint32_t r0[32], r1[32], p[16];
+            if (!odd) {
+                tmem_ld32(tmem_lane, r0);
+                tmem_ld32(tmem_lane + 32, r1);
+                tmem_wait_ld();
+                relu_pack32(r0, p);
+                tmem_st16(tmem_lane, p);
+                relu_pack32(r1, p);
+                tmem_st16(tmem_lane + 16, p);
+            } else {
+                tmem_ld32(tmem_lane + 64, r0);
+                tmem_ld32(tmem_lane + 32, r1);
+                tmem_wait_ld();
+                relu_pack32(r0, p);
+                tmem_st16(tmem_lane + 80, p);
+                relu_pack32(r1, p);
+                tmem_st16(tmem_lane + 64, p);
+            }
+        }
+        // ------------------------------------------------------------------ output layer (N = 16, K = 64)
+        const bool odd = M.n_hidden & 1u;
+        tmem_wait_st();
+        fence_before_sync();
+        named_bar(1 + wg, 128);
+        if (leader_warp) {
+            fence_after_sync();
+            umma_group_ts<4>(tmem_wg + (odd ? 32u : 0u), tmem_wg + (odd ? 0u : 64u), smem_desc(w_addr + w_off, 256, 128), 512 >> 4, idesc_o, 4u, bar);
+        }
+        mbar_wait(bar, phase);
+        phase ^= 1;
+        fence_after_sync();
+        // the output MMA is N = 16 wide: columns 0..3 always, 4..7 (into the same registers) only for out_dim > 4
+        const uint32_t o_addr = tmem_lane + (odd ? 32u : 0u);
+        for (uint32_t c0 = 0; c0 < M.out_dim; c0 += 4) {
+            uint32_t o[4];
+            tmem_ld4(o_addr + c0, o);
+            tmem_wait_ld();
+            if (valid) {
+#pragma unroll
+                for (uint32_t c = 0; c < 4; ++c)
+                    if (c0 + c < M.out_dim) {
+                        const float z = __uint_as_float(o[c]);
+                        rgb[(size_t)qi * M.out_dim + c0 + c] = M.out_act == OO_ACT_EXP ? fast_exp(z) : z;
+                    }
+            }
+        }
+    }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
+    fence_before_sync();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc(*s_tmem, 512);
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// every L whose first layer fits the 128-input limit of the TMEM A region (L*F + 6 + extras <= 128)
+#define OO_TM_SHAPES(X)                                                                                                   \
+    X(1, 8, false) X(2, 8, false) X(3, 8, false) X(4, 8, false) X(5, 8, false) X(6, 8, false) X(7, 8, false) X(8, 8, false) \
+    X(1, 16, false) X(2, 16, false) X(3, 16, false) X(4, 16, false) X(5, 16, false) X(6, 16, false) X(7, 16, false)       \
+    X(1, 4, true) X(2, 4, true) X(3, 4, true) X(4, 4, true) X(5, 4, true) X(6, 4, true) X(7, 4, true) X(8, 4, true)
+
+#define OO_TM_PIPE_SHAPES(X)                                                                   \
+    X(3, 16, false) X(4, 16, false) X(5, 16, false) X(6, 16, false) X(7, 16, false)            \
+    X(3, 8, false) X(4, 8, false) X(5, 8, false) X(6, 8, false) X(7, 8, false) X(8, 8, false)
+
+// the two-group first layer (KS) exists where the levels below input 64 fill those 64 inputs exactly
+static bool ks_applies(const TreeParams& T, const MlpParams& M) {
+    return M.k1 > 64 && T.n_levels * T.F >= 64 && T.F % 8 == 0 && 64 % T.F == 0;
+}
+#define OO_TM_KS_SHAPES(X) X(4, 16, false) X(5, 16, false) X(6, 16, false) X(7, 16, false) X(8, 8, false)
+
+template <int NWG, bool PIPE, bool KS, bool DBG>
+static int launch_tm_variant(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, uint32_t wg_cols,
+                             cudaStream_t stream) {
+    const uint64_t n_tiles = (Q.n + kRows - 1) / kRows;
+    // one block per SM as soon as there is a tile for each: a small batch spreads over all SMs (a warpgroup alone on its SM
+    // finishes a tile faster than four sharing one) instead of filling every warpgroup of the first n_tiles / NWG SMs
+    const unsigned grid = (unsigned)(n_tiles < (uint64_t)n_sms ? n_tiles : (uint64_t)n_sms);
+    const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + NWG * (10 + Q.n_extra) * kRows * 4 + 128;
+    if (smem > 227 * 1024) return -1;
+#define X(l, f, t)                                                                                                     \
+    if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                                            \
+        static std::atomic<uint64_t> opted{0};                                                                         \
+        if (!opt_in_smem(opted, (const void*)fused_tm_kernel<l, f, t, NWG, PIPE, KS, DBG>, 227 * 1024)) return kLaunchCudaError; \
+        fused_tm_kernel<l, f, t, NWG, PIPE, KS, DBG><<<grid, NWG * 128, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles, wg_cols); \
+        return 1;                                                                                                      \
+    }
+    if constexpr (KS) {
+        OO_TM_KS_SHAPES(X)
+    } else if constexpr (PIPE) {
+        OO_TM_PIPE_SHAPES(X)
+    } else {
+        OO_TM_SHAPES(X)
+    }
+#undef X
+    return -1;
+}
+
+// warpgroups per block = how many column strides fit in the 512 TMEM columns; -1 if the shape has no instance
+template <bool DBG>
+static int launch_fused_tm_impl(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, cudaStream_t stream) {
+    if (Q.n == 0) return 0;
+    if (M.out_dim > 8 || !M.image_tc || M.k1 > 128) return -1;
+    // Measured on B200 (PIPE against the batched form): config 1 60.2 -> 58.6 us, config 2 55.3 -> 54.5 us, config 3 326 -> 309 us,
+    // unsorted incoherent 2^22 queries 1.53 -> 1.32 ms.  Binned queries: mixed with four warpgroups (-2 % at 2^22, +8 % at 2^24),
+    // a gain at every size once KS runs five (2^22 0.657 -> 0.632 ms, 2^24 2.40 -> 2.22 ms), so PIPE is used wherever it applies.
+    const bool pipe = pipe_applies(T);
+    if (ks_applies(T, M)) {      // 96 columns per tile: five warpgroups
+        const int n = pipe ? launch_tm_variant<5, true, true, DBG>(T, M, Q, rgb, n_sms, 96, stream)
+                           : launch_tm_variant<5, false, true, DBG>(T, M, Q, rgb, n_sms, 96, stream);
+        if (n != -1) return n;
+    }
+    const uint32_t wg_cols = 64 + (M.k1 / 2 > 32 ? M.k1 / 2 : 32);
+    if (5 * wg_cols <= 512) {
+        if (pipe) {
+            const int n = launch_tm_variant<5, true, false, DBG>(T, M, Q, rgb, n_sms, wg_cols, stream);
+            if (n != -1) return n;
+        }
+        return launch_tm_variant<5, false, false, DBG>(T, M, Q, rgb, n_sms, wg_cols, stream);
+    }
+    if (4 * wg_cols <= 512) {
+        if (pipe) {
+            const int n = launch_tm_variant<4, true, false, DBG>(T, M, Q, rgb, n_sms, wg_cols, stream);
+            if (n != -1) return n;
+        }
+        return launch_tm_variant<4, false, false, DBG>(T, M, Q, rgb, n_sms, wg_cols, stream);
+    }
+    return -1;
+}
+
+}  // namespace oo

@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <string>
 
 #include "oo.h"
@@ -59,7 +60,10 @@ struct QueryParams {
     uint32_t n_extra;
     const uint32_t* perm;
     const float* disparity;  // [n] or nullptr (OO_LOOKUP_SHIFTED)
-    const uint32_t* out_idx; // encode_fast_kernel only (OO_PRESORT_BIN): thread t reads query t and stores its rows at out_idx[t]
+    const uint32_t* out_idx; // encode kernels and the debug instances (OO_PRESORT_BIN): thread t reads query t and stores its
+                             // feature / index rows at out_idx[t] (the query's index in the caller's order)
+    int32_t* dbg_slot;       // oo_query_debug only (read by the DBG instances of the fused kernels): [n][L] (full query [n][L][J])
+    int16_t* dbg_texel;      // ... and [n][L][2] (full query [n][L][J][3]); either may be null
 };
 
 // Decoder image: the padded, shared-memory-ready copy of the weights (built by oo_upload_mlp).
@@ -100,18 +104,34 @@ struct EncodeOut {
 };
 
 // ---------------------------------------------------------------------------------------------------------------
-// Launchers (oo_kernels.cu / oo_sort.cu).  Each returns the number of kernels it launched, or -1 if the requested
-// specialisation does not exist.  All launches go to `stream`.
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a PER-DEVICE attribute of a kernel: a context on device 1 created after one
+// on device 0 in the same process needs the opt-in again.  Every launch site therefore owns one bit per device ordinal
+// (`mask`, a function-local static of that site, one per kernel instance) and opts in the first time it launches on the
+// current device.  Returns false when the CUDA call fails (the launcher then returns kLaunchCudaError).
+constexpr int kLaunchCudaError = -2;
+inline bool opt_in_smem(std::atomic<uint64_t>& mask, const void* kernel, int bytes) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return false;
+    const uint64_t bit = (unsigned)dev < 64u ? 1ull << dev : 0ull;       // ordinals >= 64: opt in on every launch
+    if (bit && (mask.load(std::memory_order_acquire) & bit)) return true;
+    if (cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) != cudaSuccess) return false;
+    if (bit) mask.fetch_or(bit, std::memory_order_release);
+    return true;
+}
+
+// Launchers (oo_kernels.cu / oo_sort.cu).  Each returns the number of kernels it launched, -1 if the requested
+// specialisation does not exist, or kLaunchCudaError if a CUDA call made on the way failed.  All launches go to `stream`.
 int launch_pad_atlas(const void* src, void* dst, uint64_t slots, uint32_t R, uint32_t texel_bytes, cudaStream_t stream);
 int launch_encode_generic(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, uint32_t tree_max_depth,
                           cudaStream_t stream);
 int launch_encode_fast(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, int n_sms, cudaStream_t stream);
 int launch_mlp_rows(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const void* features, float* rgb,
                     int n_sms, cudaStream_t stream);
+// dbg = true selects the instances with the index sink compiled in (oo_query_debug; QueryParams::dbg_slot / dbg_texel)
 int launch_fused_mma(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
-                     cudaStream_t stream);
+                     cudaStream_t stream, bool dbg = false);
 int launch_fused_tc(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
-                    cudaStream_t stream);
+                    cudaStream_t stream, bool dbg = false);
 // The pipelined descent (gather_pipelined, oo_device.cuh) exists for fp16 trees whose first two used levels are dense and every
 // later one a hop, i.e. the BASELINE.json configs.
 inline bool pipe_applies(const TreeParams& T) {
@@ -124,6 +144,8 @@ bool fast_shape_supported(uint32_t L, uint32_t F, bool f32);
 bool tc_shape_supported(uint32_t L, uint32_t F, bool f32);
 int launch_fused_tm(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
                     cudaStream_t stream);
+int launch_fused_tm_dbg(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
+                        cudaStream_t stream);
 bool tm_shape_supported(uint32_t L, uint32_t F, bool f32);
 // full query (oo_full_*.cu)
 struct FullModeH { uint32_t tri8, lookup, attrs_paper; };
@@ -133,6 +155,10 @@ int launch_fused_full_w64(const TreeParams& T, const MlpParams& M, const QueryPa
                           int n_sms, cudaStream_t stream);
 int launch_fused_full_w128(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const FullModeH& mode, float* rgb,
                            int n_sms, cudaStream_t stream);
+int launch_fused_full_w64_dbg(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const FullModeH& mode, float* rgb,
+                              int n_sms, cudaStream_t stream);
+int launch_fused_full_w128_dbg(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const FullModeH& mode, float* rgb,
+                               int n_sms, cudaStream_t stream);
 // g_psi: d^ [n] (and optionally the hash-grid features [n][2G] fp32); M is the predictor's own decoder image (out_dim 1)
 int launch_disparity(const GridParams& G, const MlpParams& M, const QueryParams& Q, float* disparity, float* features, int n_sms,
                      cudaStream_t stream);

@@ -47,6 +47,7 @@ __global__ void __launch_bounds__(256) encode_generic_kernel(const __grid_consta
     const uint64_t t = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x;
     if (t >= Q.n) return;
     const uint64_t qi = Q.perm ? Q.perm[t] : t;
+    const uint64_t oi = Q.out_idx ? Q.out_idx[t] : qi;          // where this query's rows go (binned queries: its own index)
     float x[3], w[3];
     load3(Q.x, qi, x);
     load3(Q.wo, qi, w);
@@ -60,10 +61,10 @@ __global__ void __launch_bounds__(256) encode_generic_kernel(const __grid_consta
         const int node = descend_plain(T.child, qx, qy, qz, (int)tree_depth, (int)lv.depth);
         const int slot = node >= 0 ? __ldg(T.map_slot + node) : -1;
         const Tap tp = level_tap(uv, lv.half_r, lv.off);
-        if (O.slot) O.slot[qi * L + l] = slot;
+        if (O.slot) O.slot[oi * L + l] = slot;
         if (O.texel) {
-            O.texel[(qi * L + l) * 2] = (int16_t)tp.i0;
-            O.texel[(qi * L + l) * 2 + 1] = (int16_t)tp.j0;
+            O.texel[(oi * L + l) * 2] = (int16_t)tp.i0;
+            O.texel[(oi * L + l) * 2 + 1] = (int16_t)tp.j0;
         }
         if (!O.features) continue;
         const float w00 = (1.0f - tp.fx) * (1.0f - tp.fy), w10 = tp.fx * (1.0f - tp.fy), w01 = (1.0f - tp.fx) * tp.fy,
@@ -90,8 +91,8 @@ __global__ void __launch_bounds__(256) encode_generic_kernel(const __grid_consta
                     h = fmaf(w11, __half2float(b[F + c]), h);
                 }
             }
-            if (T.f32) ((float*)O.features)[qi * LF + l * F + c] = h;
-            else ((__half*)O.features)[qi * LF + l * F + c] = __float2half_rn(h);
+            if (T.f32) ((float*)O.features)[oi * LF + l * F + c] = h;
+            else ((__half*)O.features)[oi * LF + l * F + c] = __float2half_rn(h);
         }
     }
 }
@@ -248,11 +249,8 @@ int launch_mlp_rows(const TreeParams& T, const MlpParams& M, const QueryParams& 
     if (Q.n == 0) return 0;
     if (M.feat_dim % 8 != 0) return -1;
     const uint32_t smem = mlp_smem_bytes(M, kMlpThreads);
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(mlp_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        attr = true;
-    }
+    static std::atomic<uint64_t> opted{0};
+    if (!opt_in_smem(opted, (const void*)mlp_rows_kernel, 200 * 1024)) return kLaunchCudaError;
     const uint64_t n_tiles = (Q.n + 31) / 32;
     const uint64_t blocks = (n_tiles + 7) / 8;
     const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms * 2 ? blocks : (uint64_t)n_sms * 2);
@@ -267,7 +265,7 @@ int launch_mlp_rows(const TreeParams& T, const MlpParams& M, const QueryParams& 
 // =====================================================================================================================
 constexpr int kFusedThreads = 256;
 
-template <int L, int F, bool F32>
+template <int L, int F, bool F32, bool DBG>
 __global__ void __launch_bounds__(kFusedThreads, 2) fused_mma_kernel(const __grid_constant__ TreeParams T,
                                                                      const __grid_constant__ MlpParams M,
                                                                      const __grid_constant__ QueryParams Q,
@@ -295,12 +293,13 @@ __global__ void __launch_bounds__(kFusedThreads, 2) fused_mma_kernel(const __gri
         Encoded<L, F, F32> e;
         locate<L, F, F32>(T, s_dense, x, w, e);
         uint8_t* row = s_a + lane * a_stride;
+        const auto dbg = make_dbg<DBG>(Q, L, Q.out_idx ? Q.out_idx[tt] : qi, valid);
 #pragma unroll
         for (int l = 0; l < L; ++l) {
             const LevelParams& lv = T.lv[l];
             const Tap tp = level_tap(e.uv, lv.half_r, lv.off);
             float h[F];
-            gather_level<F, F32>(lv, e.slot[l], tp, h);
+            gather_level<F, F32>(lv, e.slot[l], tp, h, dbg, l);
 #pragma unroll
             for (int v = 0; v < F / 8 + (F % 8 ? 1 : 0); ++v) {
                 if constexpr (F % 8 == 0) {
@@ -331,7 +330,14 @@ __global__ void __launch_bounds__(kFusedThreads, 2) fused_mma_kernel(const __gri
 // ---------------------------------------------------------------------------------------------------------------------
 // Dispatch over the instantiated (L, F, dtype) shapes.
 // ---------------------------------------------------------------------------------------------------------------------
+// encode_fast_kernel (and with it OO_PATH_UNFUSED and the gate of every specialised path): every L up to OO_MAX_LEVELS for the
+// three texel formats the configs and the paper use (fp16 F = 8 / 16, fp32 F = 4)
 #define OO_SHAPES(X)                                                                                       \
+    X(1, 8, false) X(2, 8, false) X(3, 8, false) X(4, 8, false) X(5, 8, false) X(6, 8, false) X(7, 8, false) X(8, 8, false)         \
+    X(1, 16, false) X(2, 16, false) X(3, 16, false) X(4, 16, false) X(5, 16, false) X(6, 16, false) X(7, 16, false) X(8, 16, false) \
+    X(1, 4, true) X(2, 4, true) X(3, 4, true) X(4, 4, true) X(5, 4, true) X(6, 4, true) X(7, 4, true) X(8, 4, true)
+// fused_mma_kernel (the mma.sync fallback): the BASELINE.json shapes; other shapes fall through to OO_PATH_UNFUSED
+#define OO_MMA_SHAPES(X)                                                                                   \
     X(1, 8, false) X(2, 8, false) X(3, 8, false) X(4, 8, false) X(5, 8, false)                             \
     X(2, 16, false) X(3, 16, false) X(4, 16, false) X(5, 16, false)                                        \
     X(1, 4, true) X(2, 4, true) X(3, 4, true) X(4, 4, true)
@@ -358,8 +364,9 @@ int launch_encode_fast(const TreeParams& T, const QueryParams& Q, const EncodeOu
     return -1;
 }
 
-int launch_fused_mma(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
-                     cudaStream_t stream) {
+template <bool DBG>
+static int launch_fused_mma_impl(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms,
+                                 cudaStream_t stream) {
     if (Q.n == 0) return 0;
     const uint32_t smem = ((T.dense_ints * 4 + 15) & ~15u) + mlp_smem_bytes(M, kFusedThreads);
     const uint64_t n_tiles = (Q.n + 31) / 32;
@@ -367,17 +374,19 @@ int launch_fused_mma(const TreeParams& T, const MlpParams& M, const QueryParams&
     const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms * 2 ? blocks : (uint64_t)n_sms * 2);
 #define X(l, f, t)                                                                                                   \
     if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                                          \
-        static bool attr = false;                                                                                    \
-        if (!attr) {                                                                                                 \
-            cudaFuncSetAttribute(fused_mma_kernel<l, f, t>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024); \
-            attr = true;                                                                                             \
-        }                                                                                                            \
-        fused_mma_kernel<l, f, t><<<grid, kFusedThreads, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles);           \
+        static std::atomic<uint64_t> opted{0};                                                                       \
+        if (!opt_in_smem(opted, (const void*)fused_mma_kernel<l, f, t, DBG>, 200 * 1024)) return kLaunchCudaError;   \
+        fused_mma_kernel<l, f, t, DBG><<<grid, kFusedThreads, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles);      \
         return 1;                                                                                                    \
     }
-    OO_SHAPES(X)
+    OO_MMA_SHAPES(X)
 #undef X
     return -1;
+}
+
+// dbg: the instances with the index sink compiled in (oo_query_debug)
+int launch_fused_mma(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, cudaStream_t stream, bool dbg) {
+    return dbg ? launch_fused_mma_impl<true>(T, M, Q, rgb, n_sms, stream) : launch_fused_mma_impl<false>(T, M, Q, rgb, n_sms, stream);
 }
 
 }  // namespace oo

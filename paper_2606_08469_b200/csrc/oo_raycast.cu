@@ -148,11 +148,8 @@ int launch_raycast(const double* d_spheres, uint32_t n_spheres, double lo, doubl
     C.lo = lo; C.hi = hi; C.width = width; C.height = height; C.n_spheres = n_spheres;
     const uint32_t smem = n_spheres * (8 * sizeof(double) + 8 * sizeof(float));
     if (smem > 220 * 1024) return -1;
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(raycast_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 220 * 1024);
-        attr = true;
-    }
+    static std::atomic<uint64_t> opted{0};
+    if (!opt_in_smem(opted, (const void*)raycast_kernel, 220 * 1024)) return kLaunchCudaError;
     raycast_kernel<<<(unsigned)((n + kRayThreads - 1) / kRayThreads), kRayThreads, smem, stream>>>(C, d_spheres, x, nrm, wo, surf);
     return 1;
 }

@@ -365,11 +365,8 @@ __global__ void __launch_bounds__(256) unbin_kernel(const float* __restrict__ bi
 int launch_bin_queries(const QueryParams& Q, uint32_t* keys, uint32_t* hist, float* sx, float* sn, float* sw, float* se,
                        uint32_t* inv, uint32_t* idx, float* sdisp, cudaStream_t stream) {
     if (Q.n == 0) return 0;
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(bin_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kBinSmemBytes);
-        attr = true;
-    }
+    static std::atomic<uint64_t> opted{0};
+    if (!opt_in_smem(opted, (const void*)bin_scatter_kernel, (int)kBinSmemBytes)) return kLaunchCudaError;
     const uint32_t n_tiles = (uint32_t)((Q.n + kTile - 1) / kTile);
     uint32_t* tot = hist + (size_t)n_tiles * kDigits;
     cudaMemsetAsync(tot, 0, sizeof(uint32_t) * kDigits, stream);

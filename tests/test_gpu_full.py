@@ -71,6 +71,17 @@ def _check(P, tree, atlas, dtype, mlp, q, mode, disparity=None, check_cells=True
     full = mode != FO.Mode() or mlp.width != 64
     assert info["path_last_query"] == (P.PATH_FULL if full else P.PATH_FUSED_TC_TMEM)
     assert info["path_last_encode"] == P.PATH_FULL
+    # the same indices out of the fused kernel that produced the RGB (its debug instance): neighbour slots against the oracle,
+    # index decisions against the oracle where a cell exists (and, everywhere, against oo_encode_full's)
+    rgb_d, s_d, c_d = ctx.oo_query_debug(x, n, wo, ex, disparity=dd)
+    torch.cuda.synchronize()
+    assert torch.equal(rgb_d, rgb)
+    if full:
+        assert np.array_equal(s_d.cpu().numpy().astype(np.int64), ref_s), "fused kernel: neighbour slots differ"
+        assert torch.equal(c_d, c), "fused kernel: directional index decisions differ from oo_encode_full's"
+    else:
+        assert np.array_equal(s_d.cpu().numpy().astype(np.int64), ref_s[:, :, 0])
+        assert torch.equal(c_d, c[:, :, 0, :2])
     ctx.close()
     return err
 

@@ -33,7 +33,41 @@ def test_config1_full_frame_all_queries():
     fe, sl, tx = ctx.oo_encode(x, wo, want_debug=True)
     check_indices(sl.cpu().numpy(), tx.cpu().numpy(), s, t)
     check_features(fe.float().cpu().numpy(), f)
+    # the indices of the TIMED kernel itself (fused_tm_kernel's debug instance: same descent + gather code), all 1 M queries
+    rgb_d, s_d, t_d = ctx.oo_query_debug(x, n, wo)
+    assert ctx.oo_get_info()["path_last_query"] == P.PATH_FUSED_TC_TMEM and torch.equal(rgb_d, got)
+    check_indices(s_d.cpu().numpy(), t_d.cpu().numpy(), s, t)
     print("cfg1 full: rgb max-abs %.3g mean-abs %.3g" % (mx, mean))
+
+
+def test_config2_full_frame_all_queries():
+    """configs[2] at full size: 1280x720 = 921,600 queries with the per-pixel roughness input (MLP input 39), every query
+    against the C oracle; scanline order, Morton-sorted (oo_sort_queries + perm) and OO_PRESORT_BIN give the same bytes."""
+    import paper_2606_08469_b200 as P
+    w = gen.scene_workload(2)
+    q = w.queries
+    assert q.n == 1280 * 720 and q.extra is not None and q.extra.shape == (q.n, 1) and w.mlp.in_dim == 39
+    co = OC.from_workload(w)
+    ref = co.query(q.x, q.nrm, q.wo, q.extra)
+    f, s, t = co.encode(q.x, q.wo)
+    ctx = P.OctaOctree(0).upload_workload(w)
+    ctx.oo_reserve(q.n)
+    x, n, wo, ex = _dev(q.x), _dev(q.nrm), _dev(q.wo), _dev(q.extra)
+    got, s_d, t_d = ctx.oo_query_debug(x, n, wo, ex)
+    assert ctx.oo_get_info()["path_last_query"] == P.PATH_FUSED_TC_TMEM
+    mx, mean = check_rgb(got.cpu().numpy(), ref)
+    check_indices(s_d.cpu().numpy(), t_d.cpu().numpy(), s, t)
+    plain = ctx.oo_query(x, n, wo, ex)
+    assert torch.equal(plain, got)
+    perm = ctx.oo_sort_queries(x)
+    assert torch.equal(ctx.oo_query(x, n, wo, ex, perm=perm), plain)
+    ctx.oo_set_presort("bin")
+    assert torch.equal(ctx.oo_query(x, n, wo, ex), plain) and ctx.oo_get_info()["presorted_last_query"] == 1
+    rgb_b, s_b, t_b = ctx.oo_query_debug(x, n, wo, ex)          # binned: index rows still land at the query's own index
+    assert torch.equal(rgb_b, plain) and torch.equal(s_b, s_d) and torch.equal(t_b, t_d)
+    ctx.oo_set_presort("none")
+    check_features(ctx.oo_encode(x, wo).float().cpu().numpy(), f)
+    print("cfg2 full: rgb max-abs %.3g mean-abs %.3g" % (mx, mean))
 
 
 def test_config3_full_tree_sampled_queries():
@@ -55,6 +89,21 @@ def test_config3_full_tree_sampled_queries():
     fe, sl, tx = ctx.oo_encode(_dev(qs.x), _dev(qs.wo), want_debug=True)
     check_indices(sl.cpu().numpy(), tx.cpu().numpy(), s, t)
     check_features(fe.float().cpu().numpy(), f)
+    # ALL 4 M queries: the timed kernel's own indices (its debug instance) against oo_encode's kernel bit for bit -- two different
+    # descents (pipelined hop chain vs descend_plan), both checked against the oracle on the sample above -- and its RGB against
+    # a second CUDA path (features through HBM + the mma.sync MLP) within the north-star bars
+    ctx.oo_reserve(q.n)
+    rgb_d, s_d, t_d = ctx.oo_query_debug(x, n, wo)
+    assert torch.equal(rgb_d, torch.from_numpy(got).cuda())
+    _, s_e, t_e = ctx.oo_encode(x, wo, want_debug=True)
+    assert torch.equal(s_d, s_e) and torch.equal(t_d, t_e)
+    check_indices(s_d[::61].cpu().numpy(), t_d[::61].cpu().numpy(), s, t)
+    del s_e, t_e, s_d, t_d
+    ctx.oo_set_path(P.PATH_UNFUSED)
+    second = ctx.oo_query(x, n, wo).cpu().numpy()
+    ctx.oo_set_path(P.PATH_AUTO)
+    check_rgb(got, second.astype(np.float64))
+    del second
     # incoherent distribution (config 4) on the same tree
     qi = gen.incoherent_queries(w.scene, 1 << 16, 0)
     ref = co.query(qi.x, qi.nrm, qi.wo)
@@ -103,6 +152,48 @@ def test_paper_shapes_full_frame_sampled_queries():
     ref_f, ref_s = FO.encode_full(w.tree, w.atlas.levels, qs.x, qs.nrm, qs.wo, mode, d[idx], return_debug=True)
     ref = FO.query_full(w.tree, w.atlas.levels, w.mlp.weights, qs.x, qs.nrm, qs.wo, qs.extra, "exp", mode, d[idx])
     assert np.array_equal(slots.cpu().numpy()[idx].astype(np.int64), ref_s)
+    # the fused kernel's own neighbour slots and index decisions (its debug instance) against oo_encode_full's, all 1 M queries
+    rgb_d, s_d, c_d = ctx.oo_query_debug(x, n, wo, ex, disparity=dd)
+    _, _, cells = ctx.oo_encode_full(x, n, wo, dd, want_debug=True)
+    assert torch.equal(rgb_d, got) and torch.equal(s_d, slots) and torch.equal(c_d, cells)
+    del rgb_d, s_d, c_d, cells
     check_features(feat.cpu().numpy()[idx], ref_f)
     mx, mean = check_rgb(got.cpu().numpy()[idx], ref)
     print("paper shapes full frame: rgb max-abs %.3g mean-abs %.3g on %d sampled queries" % (mx, mean, len(idx)))
+
+
+@pytest.mark.parametrize("dist", ["coherent", "incoherent"])
+def test_config4_2pow24_queries(dist):
+    """configs[4] at its largest batch, 2^24 queries on the config-3 cache, as bench.py --sweep 4 times it: the coherent
+    stream (screen-order hits of a 4096x4096 frame) and the incoherent one (area-weighted surface samples, random order).
+    The oracle on a stride sample; the unsorted and the OO_PRESORT_BIN call against each other on all 16.8 M queries, bit
+    for bit; the fused kernel's own indices against oo_encode's on all of them."""
+    import paper_2606_08469_b200 as P
+    w = gen.scene_workload(3, seed=0, width=64, height=64)
+    n = 1 << 24
+    q = gen.raycast(w.scene, gen.make_camera(4096, 4096, 0)) if dist == "coherent" else gen.incoherent_queries(w.scene, n, 0)
+    assert q.n == n
+    ctx = P.OctaOctree(0).upload_workload(w)
+    ctx.oo_reserve(n)
+    x, nr, wo = _dev(q.x), _dev(q.nrm), _dev(q.wo)
+    plain = ctx.oo_query(x, nr, wo)
+    assert ctx.oo_get_info()["path_last_query"] == P.PATH_FUSED_TC_TMEM
+    ctx.oo_set_presort("bin")
+    binned = ctx.oo_query(x, nr, wo)
+    assert ctx.oo_get_info()["presorted_last_query"] == 1
+    assert torch.equal(plain, binned)
+    del binned
+    ctx.oo_set_presort("none")
+    idx = np.arange(0, n, 251)                                   # ~67 k queries across the whole batch
+    qs = q.take(idx)
+    co = OC.from_workload(w)
+    mx, mean = check_rgb(plain.cpu().numpy()[idx], co.query(qs.x, qs.nrm, qs.wo))
+    f, s, t = co.encode(qs.x, qs.wo)
+    rgb_d, s_d, t_d = ctx.oo_query_debug(x, nr, wo)
+    assert torch.equal(rgb_d, plain)
+    del rgb_d
+    check_indices(s_d[::251].cpu().numpy(), t_d[::251].cpu().numpy(), s, t)
+    fe, s_e, t_e = ctx.oo_encode(x, wo, want_debug=True)
+    assert torch.equal(s_d, s_e) and torch.equal(t_d, t_e)
+    check_features(fe[::251].float().cpu().numpy(), f)
+    print("cfg4 2^24 %s: rgb max-abs %.3g mean-abs %.3g on %d sampled queries" % (dist, mx, mean, len(idx)))

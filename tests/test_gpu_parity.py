@@ -35,6 +35,7 @@ def _paths(P, ctx):
 
 def _run_all(P, w, ref_feat, ref_slot, ref_tex, ref_rgb, expect_fast=True):
     ctx = P.OctaOctree(0).upload_workload(w)
+    ctx.oo_reserve(w.queries.n)                      # OO_PATH_GENERIC / OO_PATH_UNFUSED keep their feature rows in scratch
     x, n, wo, ex = _dev(w.queries)
     results = {}
     for path in _paths(P, ctx):
@@ -42,12 +43,19 @@ def _run_all(P, w, ref_feat, ref_slot, ref_tex, ref_rgb, expect_fast=True):
         try:
             rgb = ctx.oo_query(x, n, wo, ex)
         except P.OOError as e:
-            if e.status == 3 and path in (P.PATH_FUSED_TC, P.PATH_FUSED_TC_TMEM):      # tcgen05 variant not available for this shape
+            if e.status == 3 and path in (P.PATH_FUSED_MMA, P.PATH_FUSED_TC, P.PATH_FUSED_TC_TMEM):      # no instance of that kernel for this shape
                 continue
             raise
         torch.cuda.synchronize()
         results[path] = rgb.cpu().numpy()
         check_rgb(results[path], ref_rgb)
+        # north_star "node indices and texel indices bit-exact" on the kernel that produced this RGB: the debug instance of the
+        # same kernel (same descent and gather code + an index sink) reports the slot and base texel it gathered from
+        rgb_d, s_d, t_d = ctx.oo_query_debug(x, n, wo, ex)
+        torch.cuda.synchronize()
+        assert ctx.oo_get_info()["path_last_query"] == path
+        assert torch.equal(rgb_d, rgb), "the debug instance of path %d computes a different RGB" % path
+        check_indices(s_d.cpu().numpy(), t_d.cpu().numpy(), ref_slot, ref_tex)
         if path in (P.PATH_GENERIC, P.PATH_UNFUSED):
             f, s, t = ctx.oo_encode(x, wo, want_debug=True)
             torch.cuda.synchronize()
@@ -55,12 +63,13 @@ def _run_all(P, w, ref_feat, ref_slot, ref_tex, ref_rgb, expect_fast=True):
             check_features(f.float().cpu().numpy(), ref_feat)
     if expect_fast:
         assert P.PATH_FUSED_MMA in results and P.PATH_FUSED_TC in results and P.PATH_FUSED_TC_TMEM in results
+    if P.PATH_FUSED_MMA in results:
         # same arithmetic in the same order: the fused and unfused specialised paths agree bit for bit
         assert np.array_equal(results[P.PATH_FUSED_MMA], results[P.PATH_UNFUSED])
     ctx.oo_set_path(P.PATH_AUTO)
     rgb = ctx.oo_query(x, n, wo, ex).cpu().numpy()
     info = ctx.oo_get_info()
-    assert info["path_last_query"] == (P.PATH_FUSED_TC_TMEM if expect_fast else P.PATH_GENERIC)
+    assert info["path_last_query"] == (P.PATH_GENERIC if expect_fast is False else P.PATH_FUSED_TC_TMEM)
     check_rgb(rgb, ref_rgb)
     assert info["query_launches"] > 0
     ctx.close()
@@ -141,26 +150,61 @@ def test_other_dense_hop_patterns_use_the_batched_gather(P, depths, res, F, H):
 
 
 def test_unspecialised_shape_falls_back_to_generic(P):
-    """L=6 levels of F=8 has no template instance: AUTO -> generic; also out_act = none and out_dim = 5."""
-    tree = gen.build_tree(None, 3, uniform=True)
-    tree = gen.build_tree(gen.make_scene("three", 1), 6).set_levels([1, 2, 3, 4, 5, 6], [8, 8, 4, 4, 2, 2])
-    atlas = gen.make_atlas(tree, 8, "f16", 1)
-    mlp = gen.make_mlp(6 * 8 + 6, 3, 1, out_dim=5, out_act="none")
+    """F = 32 fp16 (64-byte texels) has no template instance: AUTO -> generic, and oo_last_note says so; also out_act = none
+    and out_dim = 5.  The generic path keeps its feature rows in reserved scratch (hot calls never allocate)."""
     scene = gen.make_scene("three", 1)
-    w = gen.Workload("L6", tree, atlas, mlp, gen.raycast(scene, gen.make_camera(70, 50, 1)), scene)
+    tree = gen.build_tree(scene, 6).set_levels([1, 2, 3, 4, 5, 6], [8, 8, 4, 4, 2, 2])
+    atlas = gen.make_atlas(tree, 32, "f16", 1)
+    mlp = gen.make_mlp(6 * 32 + 6, 3, 1, out_dim=5, out_act="none")
+    w = gen.Workload("F32", tree, atlas, mlp, gen.raycast(scene, gen.make_camera(70, 50, 1)), scene)
     co = OC.from_workload(w)
     q = w.queries
     f, s, t = co.encode(q.x, q.wo)
     rgb = co.query(q.x, q.nrm, q.wo)
     ctx = P.OctaOctree(0).upload_workload(w)
     x, n, wo, _ = _dev(q)
+    with pytest.raises(P.OOError) as e:
+        ctx.oo_query(x, n, wo)
+    assert e.value.status == 2 and "oo_reserve" in str(e.value)
+    ctx.oo_reserve(q.n)
     got = ctx.oo_query(x, n, wo).cpu().numpy()
     assert ctx.oo_get_info()["path_last_query"] == P.PATH_GENERIC
+    assert "OO_PATH_GENERIC" in ctx.oo_last_note()
     assert got.shape == (q.n, 5)
     assert np.abs(got - rgb).max() < 2e-2
     fe, sl, tx = ctx.oo_encode(x, wo, want_debug=True)
     check_indices(sl.cpu().numpy(), tx.cpu().numpy(), s, t)
     check_features(fe.float().cpu().numpy(), f)
+    rgb_d, s_d, t_d = ctx.oo_query_debug(x, n, wo)
+    assert np.array_equal(rgb_d.cpu().numpy(), got)
+    check_indices(s_d.cpu().numpy(), t_d.cpu().numpy(), s, t)
+
+
+@pytest.mark.parametrize("depths,res,F,dtype,H,out_dim,n_extra", [
+    ([1, 2, 3, 4, 5, 6], [8, 8, 4, 4, 2, 2], 8, "f16", 3, 5, 0),            # L = 6, five outputs
+    ([2, 3, 4, 5, 6, 7, 8], [16, 16, 8, 8, 4, 4, 2], 8, "f16", 2, 8, 1),    # L = 7, eight outputs, one extra
+    ([2, 3, 4, 5, 6, 7, 8, 9], [32, 16, 16, 8, 8, 4, 4, 2], 8, "f16", 2, 3, 2),   # L = 8, F = 8: k1 = 80, two-group first layer
+    ([2, 4, 5, 6, 7, 8], [16, 16, 8, 8, 4, 4], 16, "f16", 4, 3, 0),         # L = 6, F = 16: k1 = 112, pipelined + two-group
+    ([2, 4, 5, 6, 7, 8, 9], [16, 16, 8, 8, 4, 4, 2], 16, "f16", 3, 6, 3),   # L = 7, F = 16: k1 = 128 (the widest first layer)
+    ([2, 3, 4, 5, 6, 7, 8, 9], [32, 16, 16, 8, 8, 4, 4, 2], 4, "f32", 4, 3, 7),   # the paper's K = 8, C = 4 fp32 as texel maps
+    ([2, 3, 4, 5, 6], [8, 8, 8, 4, 4], 4, "f32", 2, 4, 0),                  # L = 5 fp32 (odd L: attributes start mid-unit)
+    ([1, 3], [8, 4], 16, "f16", 2, 7, 0)])                                  # two dense levels only
+def test_more_levels_and_outputs_on_the_tmem_path(P, depths, res, F, dtype, H, out_dim, n_extra):
+    """L = 6..8 and out_dim = 5..8 run on the fused tensor-memory kernel (AUTO) instead of dropping to the generic path; every
+    path that has an instance for the shape against the oracle, indices bit-exact through oo_query_debug."""
+    scene = gen.make_scene("three", 3)
+    tree = gen.build_tree(scene, depths[-1]).set_levels(depths, res)
+    atlas = gen.make_atlas(tree, F, dtype, 3)
+    mlp = gen.make_mlp(len(depths) * F + 6 + n_extra, H, 3, out_dim=out_dim)
+    cam = gen.make_camera(120, 77, 3)
+    q = gen.raycast(scene, cam)
+    if n_extra:
+        q.extra = gen.uniform_f32(3, 50 + n_extra, q.n * n_extra, 0.0, 1.0).reshape(q.n, n_extra)
+    w = gen.Workload("wide", tree, atlas, mlp, q, scene, cam)
+    f, s, t = O.encode(w.tree, w.atlas.levels, q.x, q.wo)
+    ref = O.query(w.tree, w.atlas.levels, w.mlp.weights, q.x, q.nrm, q.wo, q.extra, w.mlp.out_act)
+    res_ = _run_all(P, w, f, s, t, ref, expect_fast=None)
+    assert P.PATH_FUSED_TC_TMEM in res_ and P.PATH_UNFUSED in res_ and res_[P.PATH_FUSED_TC_TMEM].shape == (q.n, out_dim)
 
 
 def test_padded_atlas_is_the_octahedral_wrap(P, ):
@@ -190,6 +234,7 @@ def test_padded_atlas_is_the_octahedral_wrap(P, ):
 def test_ragged_sizes(P, n):
     w = gen.config0(n=max(n, 1))
     ctx = P.OctaOctree(0).upload_workload(w)
+    ctx.oo_reserve(n)
     q = w.queries.take(slice(0, n))
     x, nn, wo, _ = _dev(q)
     if n == 0:
@@ -204,6 +249,11 @@ def test_ragged_sizes(P, n):
         assert np.all(got[n:] == -7.0)                 # nothing written past the end
         if n:
             check_rgb(got[:n], ref)
+        # the debug instances write index rows for the n queries and nothing else (the binding pre-fills with -2 / -32768)
+        _, sd, td = ctx.oo_query_debug(x, nn, wo)
+        assert sd.shape == (n, 2) and td.shape == (n, 2, 2)
+        if n:
+            assert int(sd.min()) >= -1 and int(td.min()) >= -1
 
 
 def test_morton_sort_and_permuted_query(P):
@@ -335,7 +385,7 @@ def test_query_host_equals_query(P):
 def test_query_host_pipeline_many_chunks(P):
     """oo_query_host splits the frame into chunks that overlap copy-in, kernel and copy-out: several chunks with a ragged
     last one must give the same bytes as one device-side oo_query, with and without extras, called twice in a row."""
-    w = gen.scene_workload(2, width=640, height=333)          # 213,120 queries -> 4 chunks of 65,536 (last: 16,512)
+    w = gen.scene_workload(2, width=640, height=333)          # 213,120 queries: 2 chunks by default, 4 or 16 on request
     q = w.queries
     ctx = P.OctaOctree(0).upload_workload(w)
     ctx.oo_reserve(q.n)
@@ -343,12 +393,18 @@ def test_query_host_pipeline_many_chunks(P):
     dev = ctx.oo_query(x, n, wo, ex).cpu().numpy()
     pin = lambda a: torch.from_numpy(a).pin_memory()
     hx, hn, hw, he = pin(q.x), pin(q.nrm), pin(q.wo), pin(q.extra)
-    l0 = ctx.oo_get_info()["query_launches"]
-    for _ in range(2):
-        out = torch.full((q.n, 3), float("nan")).pin_memory()
-        host = ctx.oo_query_host(hx, hn, hw, he, rgb=out)
-        assert np.array_equal(host.numpy(), dev)
-    assert ctx.oo_get_info()["query_launches"] - l0 == 2 * 4          # 213,120 = 3 x 65,536 + 16,512
+    for want, chunks in ((0, 2), (4, 4), (16, 16), (1, 1)):
+        ctx.oo_set_host_chunks(want)
+        l0 = ctx.oo_get_info()["query_launches"]
+        for _ in range(2):
+            out = torch.full((q.n, 3), float("nan")).pin_memory()
+            host = ctx.oo_query_host(hx, hn, hw, he, rgb=out)
+            assert np.array_equal(host.numpy(), dev)
+        assert ctx.oo_get_info()["query_launches"] - l0 == 2 * chunks
+    with pytest.raises(P.OOError) as e:
+        ctx.oo_set_host_chunks(17)
+    assert e.value.status == 1
+    ctx.oo_set_host_chunks(0)
     s = torch.cuda.Stream()
     with torch.cuda.stream(s):
         host = ctx.oo_query_host(hx, hn, hw, he)            # the binding passes torch's current stream
@@ -388,3 +444,67 @@ def test_error_codes(P):
     with pytest.raises(P.OOError) as e:
         ctx.oo_sort_queries(x)
     assert e.value.status == 2                                     # oo_reserve not called
+
+
+def test_weights_on_device(P):
+    """oo_mlp_desc.weights_on_device: the same decoder uploaded from DEVICE buffers gives the same bytes."""
+    w = gen.scene_workload(1, width=96, height=64)
+    q = w.queries
+    x, n, wo, _ = _dev(q)
+    ctx = P.OctaOctree(0).upload_workload(w)
+    ref = ctx.oo_query(x, n, wo)
+    ctx.oo_upload_mlp([torch.from_numpy(np.ascontiguousarray(m, np.float16)).cuda() for m in w.mlp.weights], w.mlp.out_act)
+    assert torch.equal(ctx.oo_query(x, n, wo), ref)
+    ctx.oo_upload_mlp([np.zeros_like(m) for m in w.mlp.weights], w.mlp.out_act)      # zero weights: exp(0) = 1
+    assert bool((ctx.oo_query(x, n, wo) == 1.0).all())
+
+
+def test_failed_calls_leave_the_context_usable(P):
+    """Only a lost CUDA context is latched.  An allocation that does not fit (OO_ERR_OOM), missing scratch (OO_ERR_NOT_READY) or
+    a failure on another context do not poison later calls."""
+    w = gen.scene_workload(1, width=64, height=48)
+    q = w.queries
+    x, n, wo, _ = _dev(q)
+    ctx = P.OctaOctree(0).upload_workload(w)
+    ref = ctx.oo_query(x, n, wo)
+    with pytest.raises(P.OOError) as e:
+        ctx.oo_reserve(1 << 40)                                     # ~250 TB of scratch
+    assert e.value.status == 5
+    assert torch.equal(ctx.oo_query(x, n, wo), ref)
+    ctx.oo_reserve(q.n)
+    ctx.oo_set_path(P.PATH_UNFUSED)
+    assert np.abs(ctx.oo_query(x, n, wo).cpu().numpy() - ref.cpu().numpy()).max() < 5e-3
+    ctx.oo_set_path(P.PATH_AUTO)
+    bad = P.OctaOctree(0)
+    with pytest.raises(P.OOError):
+        bad.oo_read_padded_map(0, 0, 8)                             # nothing uploaded on a second context
+    assert torch.equal(ctx.oo_query(x, n, wo), ref)
+
+
+def test_two_contexts_in_one_process(P):
+    """Several contexts may live in one process: two on device 0 with different caches; and, where a second B200 is present, one
+    per device (the >48 KB dynamic shared memory opt-in is per device: every launch site opts in once per device)."""
+    w1 = gen.scene_workload(1, width=80, height=64)
+    w0 = gen.config0()
+    a, b = P.OctaOctree(0).upload_workload(w1), P.OctaOctree(0).upload_workload(w0)
+    co = OC.from_workload(w1)
+    x1, n1, wo1, _ = _dev(w1.queries)
+    x0, n0, wo0, _ = _dev(w0.queries)
+    ra, rb = a.oo_query(x1, n1, wo1), b.oo_query(x0, n0, wo0)
+    check_rgb(ra.cpu().numpy(), co.query(w1.queries.x, w1.queries.nrm, w1.queries.wo))
+    check_rgb(rb.cpu().numpy(), O.query(w0.tree, w0.atlas.levels, w0.mlp.weights, w0.queries.x, w0.queries.nrm, w0.queries.wo))
+    if torch.cuda.device_count() < 2:
+        pytest.skip("one CUDA device: the per-device half of this test needs two")
+    with torch.cuda.device(1):
+        c = P.OctaOctree(1).upload_workload(w1)
+        c.oo_reserve(w1.queries.n)
+        to1 = lambda t: t.to("cuda:1")
+        for path in (P.PATH_FUSED_TC_TMEM, P.PATH_FUSED_TC, P.PATH_FUSED_MMA, P.PATH_UNFUSED):
+            c.oo_set_path(path)
+            a.oo_set_path(path)
+            a.oo_reserve(w1.queries.n)
+            rc = c.oo_query(to1(x1), to1(n1), to1(wo1))
+            torch.cuda.synchronize()
+            assert torch.equal(rc.cpu(), a.oo_query(x1, n1, wo1).cpu())
+        c.oo_set_presort("bin", min_queries=1)
+        assert torch.equal(c.oo_query(to1(x1), to1(n1), to1(wo1)).cpu(), rc.cpu())
