@@ -1,13 +1,18 @@
 #!/usr/bin/env python
 """bench.py — fused encode+MLP throughput of the OctaOctree query on B200 (BASELINE.json metric), one JSON line.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1|2|3] [--path auto|mma|tc|unfused|generic]
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1|2|3|4] [--scaling weak|strong]
+                  [--path auto|mma|tc|tm|unfused|generic]
 
 A "step" is one pass of the whole hot path (a2-a9) over one frame of synthetic primary hits (config 1: 1024x1024).
 `value` = queries/s with the queries already resident in HBM, timed per step with CUDA events on the launching stream,
 L2 flushed between steps; `e2e` = the same through oo_query_host with pinned HOST buffers (H2D + kernel + D2H inside the
-timed region).  N > 1: one process per GPU (torchrun), cache replicated, one frame per rank, no data-path collective
-(weak scaling); timings are the max over ranks.  `--impl reference` times the CPU oracle (oracle/) as it stands.
+timed region).  N > 1: one process per GPU; from a plain shell (`python bench.py --gpus N`, no WORLD_SIZE in the
+environment) the script re-launches itself under `python -m torch.distributed.run --nproc-per-node N`.  The cache is
+replicated on every GPU (read-only); `--scaling weak` (default): every rank renders its OWN frame (camera seed = rank), no
+data-path collective; `--scaling strong`: ONE frame is split into contiguous query slices (dist.shard_range), every rank
+evaluates its slice and the RGB slices are all-gathered over NCCL inside the timed region, so every rank ends the step
+holding the whole frame.  Timings are the max over ranks.  `--impl reference` times the CPU oracle (oracle/) as it stands.
 """
 from __future__ import annotations
 
@@ -28,14 +33,24 @@ UNIT = "Mqueries/s"
 
 
 def workload_for(cfg: int, rank: int = 0):
+    """The BASELINE.json workload of configs[cfg].  rank > 0 (weak scaling): the same scene, cache and decoder with that
+    rank's own frame -- another seeded camera pose (configs 1-3) or another stretch of the incoherent sampler (config 4)."""
     import gen
     if cfg == 4:
         # BASELINE.json configs[4], the incoherent distribution at 2^22 queries: config 3's scene, tree, atlas and MLP; queries =
         # area-weighted surface samples in random order (the batch-size x distribution table is --sweep 4)
         w = gen.scene_workload(3, seed=0, width=64, height=64, incoherent_n=1 << 22)
         w.meta["width"], w.meta["height"], w.meta["incoherent"] = 2048, 2048, True   # width/height only cut the CPU oracle's sample into index ranges
+        if rank:
+            w.queries = gen.incoherent_queries(w.scene, 1 << 22, 0, first=rank << 22)
     else:
         w = gen.scene_workload(cfg, seed=0)
+        if rank:
+            w.camera = gen.make_camera(w.meta["width"], w.meta["height"], rank)
+            ex = w.queries.extra
+            w.queries = gen.raycast(w.scene, w.camera)
+            if ex is not None:
+                w.queries.extra = gen.roughness(w.queries.n, rank)
     L, F = len(w.tree.level_depth), w.atlas.F
     n_extra = 0 if w.queries.extra is None else w.queries.extra.shape[1]
     texel = F * 2
@@ -146,11 +161,153 @@ def run_reference(args):
     val = sample_q.n / mean / 1e6
     out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": mean * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-           "dtype": "f64", "data": "synthetic", "config": dict(desc, sample=sample_desc),
+           "dtype": "f64", "data": "synthetic", "config": desc, "run": {"sample": sample_desc},
            "cpu_baseline": {"value": val, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample_desc},
            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
            "note": "the CPU oracle (oracle/oo_oracle.c, double precision, OpenMP over queries) as it stands; each step = the bounded sample"}
     print(json.dumps(out))
+    return 0
+
+
+PATH_NAMES = {0: "auto", 1: "generic", 2: "unfused", 3: "fused_mma", 4: "fused_tcgen05", 5: "fused_tcgen05_tmem_a", 6: "full_query"}
+
+
+def source_sha() -> str:
+    """Hash of the CUDA sources the library is built from: stamps profiles/traffic.json so that a stale capture is refused."""
+    import hashlib
+    h = hashlib.sha256()
+    d = os.path.join(ROOT, "paper_2606_08469_b200", "csrc")
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh", ".h")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_facts(cfg: int):
+    """Per-launch facts of the dominant kernel from the committed ncu capture (profiles/traffic.json): DRAM bytes and warp
+    instructions.  Valid only for the sources they were captured from: a stamp mismatch returns (None, reason)."""
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    if not os.path.exists(tp):
+        return None, "no profiles/traffic.json"
+    d = json.load(open(tp))
+    e = d.get("cfg%d" % cfg)
+    if not e:
+        return None, "no capture for config %d" % cfg
+    if e.get("source_sha") != source_sha():
+        return None, "stale: captured from other kernel sources (%s, now %s); re-run the ncu pass and bench.py --ingest-ncu" % (e.get("source_sha"), source_sha())
+    return e, None
+
+
+def ingest_ncu(args):
+    """bench.py --ingest-ncu CSV --config K: read an `ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum,
+    smsp__inst_executed.sum,gpu__time_duration.sum --csv --log-file CSV python bench.py --quick --config K ...` launch list and
+    store the LAST launch of the dominant kernel (name contains --ingest-kernel, default 'fused') in profiles/traffic.json,
+    stamped with the hash of the kernel sources."""
+    import csv
+    rows = [r for r in csv.reader(l for l in open(args.ingest_ncu) if l.startswith('"'))]
+    head, rows = rows[0], rows[1:]
+    k_id, k_name, k_metric, k_val = head.index("ID"), head.index("Kernel Name"), head.index("Metric Name"), head.index("Metric Value")
+    launches = {}
+    for r in rows:
+        if args.ingest_kernel in r[k_name]:
+            launches.setdefault(int(r[k_id]), {"kernel": r[k_name].split("(")[0]})[r[k_metric]] = float(r[k_val].replace(",", ""))
+    if not launches:
+        raise SystemExit("no launch of a kernel matching %r in %s" % (args.ingest_kernel, args.ingest_ncu))
+    m = launches[max(launches)]
+    tp = os.path.join(ROOT, "profiles", "traffic.json")
+    d = json.load(open(tp)) if os.path.exists(tp) else {}
+    d.pop("source", None)
+    d["how"] = ("per launch of the dominant kernel, --clock-control none: ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum,"
+                "smsp__inst_executed.sum,gpu__time_duration.sum --csv --log-file X.csv python bench.py --quick --config K --steps 5 --warmup 3; "
+                "python bench.py --ingest-ncu X.csv --config K")
+    d["cfg%d" % args.config] = {"dram_bytes_per_launch": int(m.get("dram__bytes_read.sum", 0) + m.get("dram__bytes_write.sum", 0)),
+                                "warp_instructions_per_launch": int(m.get("smsp__inst_executed.sum", 0)),
+                                "ncu_time_ns": int(m.get("gpu__time_duration.sum", 0)), "kernel": m["kernel"], "source_sha": source_sha()}
+    json.dump(d, open(tp, "w"), indent=1)
+    print(json.dumps(d["cfg%d" % args.config]))
+    return 0
+
+
+def compulsory_bytes(ctx, w, x, nrm, wo, ex):
+    """What one frame MUST read from DRAM if every distinct byte were fetched once: the distinct 32-byte sectors (and distinct
+    texels) of the padded atlas the frame's taps touch, counted from the fused kernel's own indices (oo_query_debug), plus the
+    query stream in and the RGB out.  The gap between this and L*4*texel bytes per query is the reuse neighbouring queries share."""
+    import torch
+    rgb, slot, tex = ctx.oo_query_debug(x, nrm, wo, ex)
+    del rgb
+    tb = w.atlas.F * 2
+    uniq_texels = uniq_sectors = 0
+    for l, R in enumerate(w.tree.level_res):
+        Rp = R + 2
+        s = slot[:, l].long()
+        ok = s >= 0
+        base = s[ok] * (Rp * Rp) + (tex[ok][:, l, 1].long() + 1) * Rp + (tex[ok][:, l, 0].long() + 1)      # padded texel index of tap (i0, j0)
+        taps = torch.cat([base, base + 1, base + Rp, base + Rp + 1])
+        ut = torch.unique(taps)
+        uniq_texels += int(ut.numel())
+        uniq_sectors += int(torch.unique((ut * tb) // 32).numel()) if tb < 32 else int(ut.numel()) * (tb // 32)
+        del s, ok, base, taps, ut
+    n, ne = int(x.shape[0]), 0 if ex is None else int(ex.shape[1])
+    io = n * (36 + 4 * ne + 12)
+    return {"distinct_texel_bytes": uniq_texels * tb, "distinct_sector_bytes": uniq_sectors * 32, "query_io_bytes": io,
+            "total": uniq_sectors * 32 + io, "how": "distinct padded-atlas texels / 32-byte sectors touched by the frame's 4 taps per level (from oo_query_debug's indices) + 36 B in + 12 B out per query"}
+
+
+def relaunch_if_needed(args) -> int:
+    """`python bench.py --gpus N` from a plain shell: start N ranks (one per GPU) of this same command under torch.distributed.run.
+    Returns the children's exit code, or -1 when this process is already a rank (or N == 1) and should carry on."""
+    if args.gpus <= 1 or "WORLD_SIZE" in os.environ:
+        return -1
+    import socket
+    if not args.dry_run_dist:
+        import torch
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            sys.stderr.write("bench.py: --gpus %d but %d CUDA device(s) visible\n" % (args.gpus, have))
+            return 2
+    with socket.socket() as so:
+        so.bind(("127.0.0.1", 0))
+        port = so.getsockname()[1]
+    env = dict(os.environ)
+    env.setdefault("NCCL_DEBUG", "INFO")               # NCCL's init log names every rank and the transport (NVLS / P2P) ...
+    env.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+    env.setdefault("NCCL_DEBUG_FILE", "/dev/stderr")   # ... on stderr: stdout stays the one JSON line
+    env.setdefault("OMP_NUM_THREADS", str(max(1, (os.cpu_count() or 1) // args.gpus)))
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus), "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    return subprocess.call(cmd, env=env)
+
+
+def run_dry_dist(args):
+    """--dry-run-dist: the N > 1 host logic of the product arm with the gloo backend and no GPU -- launcher, rank environment,
+    per-rank frames (weak) or shard_range slices + all_gather_rows (strong), max/sum reductions, one JSON line from rank 0.
+    The per-query work is replaced by a stand-in (rgb = x), so this measures nothing: it is what the CPU tests drive."""
+    import numpy as np
+    import torch
+    import gen
+    from paper_2606_08469_b200 import dist as D
+    rank, local_rank, world = D.env_rank_world()
+    if world > 1:
+        D.init_process_group("gloo")
+    scene = gen.make_scene("three", 0)
+    n_frame = 96 * 64
+    if args.scaling == "strong":
+        q = gen.raycast(scene, gen.make_camera(96, 64, 0))
+        lo, hi = D.shard_range(q.n, rank, world)
+        local = torch.from_numpy(q.x[lo:hi].copy())
+        full = D.all_gather_rows(local, q.n)
+        assert torch.equal(full, torch.from_numpy(q.x)), "all_gather_rows did not rebuild the frame"
+        mine, checksum = hi - lo, float(full.double().sum())
+    else:
+        q = gen.raycast(scene, gen.make_camera(96, 64, rank))
+        mine, checksum = q.n, float(torch.from_numpy(q.x).double().sum())
+    (mx,), (tot, chk) = D.reduce_max_sum([1.0 + rank], [mine, checksum if args.scaling == "weak" else 0.0], torch.device("cpu"))
+    if rank == 0:
+        print(json.dumps({"dry_run": True, "n_gpus": world, "scaling": args.scaling, "queries": int(tot), "frame": n_frame,
+                          "max_ms": mx, "checksum": checksum if args.scaling == "strong" else chk}))
+    if world > 1:
+        torch.distributed.destroy_process_group()
     return 0
 
 
@@ -166,8 +323,11 @@ def run_ours(args):
     dev = torch.device("cuda", local_rank)
     if world > 1:
         D.init_process_group("nccl")
-    w, desc = workload_for(args.config, rank)
+    strong = args.scaling == "strong" and world > 1
+    w, desc = workload_for(args.config, 0 if args.scaling == "strong" else rank)
     q = w.queries
+    n_frame = q.n
+    lo, hi = D.shard_range(q.n, rank, world) if strong else (0, q.n)
     ctx = P.OctaOctree(local_rank).upload_workload(w)
     path = {"auto": P.PATH_AUTO, "mma": P.PATH_FUSED_MMA, "tc": P.PATH_FUSED_TC, "tm": P.PATH_FUSED_TC_TMEM, "unfused": P.PATH_UNFUSED, "generic": P.PATH_GENERIC}[args.path]
     ctx.oo_set_path(path)
@@ -175,11 +335,13 @@ def run_ours(args):
         args.presort = "bin" if args.config == 4 else "none"
     ctx.oo_set_presort(args.presort)
     ctx.oo_reserve(q.n)
-    cu = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    cu = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a[lo:hi])).to(dev)
     x, nrm, wo, ex = cu(q.x), cu(q.nrm), cu(q.wo), cu(q.extra)
-    rgb = torch.empty((q.n, 3), dtype=torch.float32, device=dev)
+    n_mine = hi - lo
+    rgb = torch.empty((n_mine, 3), dtype=torch.float32, device=dev)
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)          # > 126 MB L2
     stream = torch.cuda.current_stream(dev)
+    frame = [None]
 
     def barrier():
         if world > 1:
@@ -199,7 +361,11 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
         return [a.elapsed_time(b) for a, b in evs]
 
-    step = lambda: ctx.oo_query(x, nrm, wo, ex, rgb=rgb)
+    def step():
+        ctx.oo_query(x, nrm, wo, ex, rgb=rgb)
+        if strong:        # the path's one optional exchange: every rank ends the step with the whole frame (NCCL all-gather)
+            frame[0] = D.all_gather_rows(rgb, n_frame)
+
     for _ in range(max(args.warmup, 3)):
         flush.zero_()
         step()
@@ -216,62 +382,143 @@ def run_ours(args):
     if sampler and (t1 - t0) < 0.5 and not args.quick:
         tend = time.time() + 0.5
         while time.time() < tend:
-            step()
+            ctx.oo_query(x, nrm, wo, ex, rgb=rgb)
         torch.cuda.synchronize(dev)
         t1 = time.time()
     clocks = sampler.stop(t0, t1) if sampler else None
     ms_warm = timed(min(args.steps, 50), False, step) if not args.quick else ms
+    checksum_dev = float((frame[0] if strong else rgb).double().sum())
     # e2e: pinned host buffers, H2D + kernels + D2H inside the timed region, through oo_query_host
-    pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a[lo:hi])).pin_memory()
     hx, hn, hw, he = pin(q.x), pin(q.nrm), pin(q.wo), pin(q.extra)
-    hrgb = torch.empty((q.n, 3), dtype=torch.float32).pin_memory()
+    hrgb = torch.empty((n_mine, 3), dtype=torch.float32).pin_memory()
     e2e_steps = max(3, min(args.steps, 20)) if not args.quick else 1
     for _ in range(0 if args.quick else 2):
         ctx.oo_query_host(hx, hn, hw, he, rgb=hrgb)
     barrier()
-    te = time.perf_counter()
+    e2e_times = []
     for _ in range(e2e_steps):
-        ctx.oo_query_host(hx, hn, hw, he, rgb=hrgb)
+        te = time.perf_counter()
+        ctx.oo_query_host(hx, hn, hw, he, rgb=hrgb)          # synchronous: returns when the RGB is in host memory
+        e2e_times.append((time.perf_counter() - te) * 1e3)
     torch.cuda.synchronize(dev)
-    e2e_ms = (time.perf_counter() - te) * 1e3 / e2e_steps
-    checksum = float(hrgb.sum())
+    e2e_ms = sum(e2e_times) / len(e2e_times)
+    checksum = float(hrgb.double().sum())
+    # measured copy rates of this box (one 64 MB pinned copy each way), so that the PCIe floor of e2e is a measured number
+    h2d_gbs = d2h_gbs = None
+    if not args.quick and rank == 0:
+        hb, db = torch.empty(64 << 20, dtype=torch.uint8).pin_memory(), torch.empty(64 << 20, dtype=torch.uint8, device=dev)
+        for direction in (0, 1):
+            best = 1e9
+            for _ in range(5):
+                torch.cuda.synchronize(dev)
+                tc = time.perf_counter()
+                (db.copy_(hb, non_blocking=True) if direction == 0 else hb.copy_(db, non_blocking=True))
+                torch.cuda.synchronize(dev)
+                best = min(best, time.perf_counter() - tc)
+            if direction == 0:
+                h2d_gbs = (64 << 20) / best / 1e9
+            else:
+                d2h_gbs = (64 << 20) / best / 1e9
 
     mean_ms, warm_ms = sum(ms) / len(ms), sum(ms_warm) / len(ms_warm)
-    (mx_ms, mx_warm, mx_e2e), (tot_q,) = D.reduce_max_sum([mean_ms, warm_ms, e2e_ms], [q.n], dev)
+    (mx_ms, mx_warm, mx_e2e), (tot_q, chk_sum) = D.reduce_max_sum([mean_ms, warm_ms, e2e_ms], [n_mine, checksum], dev)
     if rank != 0:
+        if world > 1:
+            torch.distributed.destroy_process_group()
         return 0
     hbm, tf, which = peaks()
     value = tot_q / (mx_ms * 1e-3) / 1e6
-    achieved = desc["bytes_per_query"] * q.n / (mean_ms * 1e-3) / 1e9
-    flop_time = desc["flop_per_query"] * q.n / (tf * 1e12)
-    byte_time = desc["bytes_per_query"] * q.n / (hbm * 1e9)
-    traffic = None
-    tp = os.path.join(ROOT, "profiles", "traffic.json")
-    if os.path.exists(tp):
-        traffic = json.load(open(tp)).get("cfg%d" % args.config, {}).get("dram_bytes_per_launch")
+    ne = 0 if q.extra is None else q.extra.shape[1]
+    alg_bytes = desc["bytes_per_query"] * n_mine                 # rank 0's launch (every rank's is the same size +- 1 query)
+    achieved = alg_bytes / (mean_ms * 1e-3) / 1e9
+    flop_time = desc["flop_per_query"] * n_mine / (tf * 1e12)
+    byte_time = alg_bytes / (hbm * 1e9)
     info = ctx.oo_get_info()
+    facts, stale = (None, "not looked up") if strong else ncu_facts(args.config)
+    roof = {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
+            "traffic": facts["dram_bytes_per_launch"] if facts else None,
+            "peak_source": which, "kernel": "fused encode+MLP (one launch per step)" if args.presort == "none" else
+            "whole step: histogram + scan + bin_scatter + fused encode+MLP on the binned copy + unbin (traffic is the fused launch's)",
+            "definition": "BASELINE.json north_star: ALGORITHMIC bytes (L*4 texels gathered + 36 B in + 12 B out per query) at the measured HBM peak, "
+                          "vs the MLP FLOPs at the dense fp16 peak; the slower of the two is the roofline",
+            "roofline_ms": max(byte_time, flop_time) * 1e3, "flop_time_ms": flop_time * 1e3, "byte_time_ms": byte_time * 1e3,
+            "binds": "bytes" if byte_time >= flop_time else "flops",
+            "frac_warm_l2": alg_bytes / (warm_ms * 1e-3) / 1e9 / hbm}
+    if roof["frac"] > 1.0:
+        roof["frac_note"] = ("above 1: neighbouring queries share texels, so L1/L2 serve bytes the algorithmic count charges to HBM; for this "
+                             "config the algorithmic-byte figure is not a bound -- see dram / compulsory / issue below")
+    if facts:
+        dram = facts["dram_bytes_per_launch"]
+        roof["dram"] = {"bytes_per_launch": dram, "GBps": dram / (mean_ms * 1e-3) / 1e9, "frac_of_peak": dram / (mean_ms * 1e-3) / 1e9 / hbm,
+                        "vs_algorithmic": dram / alg_bytes, "kernel": facts.get("kernel"), "source": "profiles/traffic.json (ncu, stamped %s)" % facts["source_sha"]}
+        wi = facts.get("warp_instructions_per_launch")
+        if wi and clocks and clocks.get("sm_mhz"):
+            # second bound: every warp instruction needs one issue slot; an SM issues 4 per cycle (one per sub-partition)
+            issue_ms = wi / (info["n_sms"] * 4 * clocks["sm_mhz"] * 1e6) * 1e3
+            roof["issue"] = {"warp_instructions_per_launch": wi, "thread_instructions_per_query": wi * 32 / n_mine, "bound_ms": issue_ms,
+                             "frac": issue_ms / mean_ms, "how": "warp instructions / (SMs x 4 issue slots x measured SM clock): the time below which this "
+                             "instruction stream cannot run; frac = share of issue slots used"}
+    else:
+        roof["traffic_note"] = stale
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-        "ms_per_step": mx_ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f16",
-        "data": "synthetic",
-        "config": dict(desc, l2="flushed between steps (256 MB memset)", path={0: "auto", 1: "generic", 2: "unfused", 3: "fused_mma", 4: "fused_tcgen05", 5: "fused_tcgen05_tmem_a"}[info["path_last_query"]],
-                       ms_per_frame_warm_l2=mx_warm, frames_per_rank=1, presort=args.presort, parallelism="replicated cache, one frame per GPU, no collective"),
+        "ms_per_step": mx_ms, "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None, "dtype": "f16",
+        "data": "synthetic", "config": desc,
+        "run": {"l2": "flushed between steps (256 MB memset)", "path": PATH_NAMES[info["path_last_query"]], "ms_per_frame_warm_l2": mx_warm,
+                "presort": args.presort, "queries_per_rank": n_mine, "checksum_device": checksum_dev,
+                "parallelism": ("one GPU" if world == 1 else
+                                "replicated cache; ONE frame split into contiguous query slices, RGB all-gathered over NCCL inside the timed region" if strong else
+                                "replicated cache; every rank its own frame (camera seed = rank); no data-path collective")},
         "clocks": clocks,
-        "e2e": {"value": tot_q / (mx_e2e * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": int((36 + 4 * (0 if q.extra is None else q.extra.shape[1])) * q.n),
-                "d2h_bytes_per_step": int(12 * q.n), "ms_per_step": mx_e2e, "api": "oo_query_host (pinned host buffers)", "checksum": checksum},
+        "e2e": {"value": tot_q / (mx_e2e * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": int((36 + 4 * ne) * n_mine),
+                "d2h_bytes_per_step": int(12 * n_mine), "ms_per_step": mx_e2e, "ms_min": min(e2e_times), "ms_max": max(e2e_times),
+                "api": "oo_query_host (pinned host buffers)", "checksum": chk_sum if not strong else checksum,
+                "h2d_GBps_measured": h2d_gbs, "d2h_GBps_measured": d2h_gbs,
+                "pcie_floor_ms": None if not h2d_gbs else (36 + 4 * ne) * n_mine / (h2d_gbs * 1e9) * 1e3},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm, "traffic": traffic,
-                     "peak_source": which, "kernel": "fused encode+MLP (one launch per step)" if args.presort == "none" else
-                     "whole step: histogram + scan + bin_scatter + fused encode+MLP on the binned copy + unbin (the fused launch is ~3/4 of it; traffic is that launch's)",
-                     "roofline_ms": max(byte_time, flop_time) * 1e3, "flop_time_ms": flop_time * 1e3, "byte_time_ms": byte_time * 1e3,
-                     "frac_warm_l2": desc["bytes_per_query"] * q.n / (warm_ms * 1e-3) / 1e9 / hbm},
+        "roofline": roof,
     }
+    if world == 1 and not args.quick:
+        try:
+            roof["compulsory"] = comp = compulsory_bytes(ctx, w, x, nrm, wo, ex)
+            roof["compulsory"]["byte_time_ms"] = comp["total"] / (hbm * 1e9) * 1e3
+            roof["compulsory"]["frac"] = comp["total"] / (hbm * 1e9) * 1e3 / mean_ms
+            if facts:
+                roof["dram"]["overfetch_vs_compulsory"] = facts["dram_bytes_per_launch"] / comp["total"]
+        except P.OOError as e:
+            roof["compulsory"] = {"unavailable": str(e)}
+        # camera -> RGB without the PCIe copy of the queries: primary visibility on the device + the query (12 B/query D2H only)
+        if w.camera is not None:
+            cam, sc = w.camera, w.scene
+            ctx.oo_upload_scene(sc.spheres, sc.lo, sc.hi)
+            qbuf = tuple(torch.empty((q.n, 3), dtype=torch.float32, device=dev) for _ in range(3))
+            exd = ex
+
+            def cam_to_rgb():
+                ctx.oo_raycast(cam.eye, cam.look, cam.up, cam.vfov_deg, cam.width, cam.height, out=qbuf)
+                ctx.oo_query(qbuf[0], qbuf[1], qbuf[2], exd, rgb=rgb)
+                hrgb.copy_(rgb, non_blocking=True)
+            for _ in range(3):
+                cam_to_rgb()
+            torch.cuda.synchronize(dev)
+            tt = []
+            for _ in range(e2e_steps):
+                tc = time.perf_counter()
+                cam_to_rgb()
+                torch.cuda.synchronize(dev)
+                tt.append((time.perf_counter() - tc) * 1e3)
+            out["e2e_camera_to_rgb"] = {"ms_per_step": sum(tt) / len(tt), "value": q.n / (sum(tt) / len(tt) * 1e-3) / 1e6, "unit": UNIT,
+                                        "h2d_bytes_per_step": 0, "d2h_bytes_per_step": int(12 * q.n),
+                                        "api": "oo_raycast + oo_query + one D2H copy of the RGB: the frame's queries are made on the device (not the headline e2e: its inputs never cross PCIe)"}
     if world == 1 and not args.no_cpu_baseline and not args.quick:
         sample_q, sample_desc = oracle_sample(w, args.ref_sample)
         dt, threads = time_oracle(w, sample_q, repeats=3)
         sample_desc += "; best of 3"
         out["cpu_baseline"] = {"value": sample_q.n / dt / 1e6, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample_desc}
     print(json.dumps(out))
+    if world > 1:
+        torch.distributed.destroy_process_group()
     return 0
 
 
@@ -576,7 +823,19 @@ def main():
     ap.add_argument("--sweep-dist", default="both", choices=["both", "coherent", "incoherent"])
     ap.add_argument("--presort", default=None, choices=["none", "bin"], help="oo_set_presort for the run (default: bin for --config 4, none otherwise)")
     ap.add_argument("--quick", action="store_true", help="timed region only (no warm-L2 / e2e / CPU legs): the command ncu wraps")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"], help="N > 1: every rank its own frame (weak) or one frame split across ranks + RGB all-gather (strong)")
+    ap.add_argument("--dry-run-dist", action="store_true", help="the N > 1 host logic on CPU with gloo (launcher, sharding, gather, reductions): what the CPU tests drive; measures nothing")
+    ap.add_argument("--ingest-ncu", default=None, help="ncu --csv launch list to store in profiles/traffic.json for --config (see ingest_ncu)")
+    ap.add_argument("--ingest-kernel", default="fused", help="substring of the dominant kernel's name for --ingest-ncu")
     args = ap.parse_args()
+    if args.ingest_ncu:
+        return ingest_ncu(args)
+    if args.impl == "ours" and not args.sweep:
+        rc = relaunch_if_needed(args)
+        if rc >= 0:
+            return rc
+        if args.dry_run_dist:
+            return run_dry_dist(args)
     if args.sweep == 8:
         return run_full(args)
     if args.sweep == 5:

@@ -176,6 +176,16 @@ __device__ __forceinline__ void write_row_tail(uint8_t* row, uint32_t feat_dim, 
     if (k1 - feat_dim > 16) dst[2] = make_uint4(0, 0, 0, 0);
 }
 
+// the same when feat_dim = 4 mod 8 (F = 4 fp32 with an odd level count): the tail starts mid-vector; halves one by one
+__device__ __forceinline__ void write_row_tail_odd(uint8_t* row, uint32_t feat_dim, uint32_t k1, const float (&n)[3],
+                                                   const float (&w)[3], const float* __restrict__ extra, uint64_t qi,
+                                                   uint32_t n_extra) {
+    __half* r = (__half*)row;
+    for (uint32_t c = feat_dim; c < k1; ++c) r[c] = __float2half_rn(0.0f);
+    for (int k = 0; k < 3; ++k) { r[feat_dim + k] = __float2half_rn(n[k]); r[feat_dim + 3 + k] = __float2half_rn(w[k]); }
+    for (uint32_t k = 0; k < n_extra; ++k) r[feat_dim + 6 + k] = __float2half_rn(__ldg(extra + qi * n_extra + k));
+}
+
 // rgb of the warp's 32 rows: C fragments -> shared scratch -> one row per lane -> activation -> store at the query's index
 __device__ __forceinline__ void store_rgb(float* s_out /* [32][8] floats, warp private */, const float (&out)[2][4],
                                           float* __restrict__ rgb, uint64_t qi, bool valid, uint32_t out_dim, uint32_t act) {
@@ -229,11 +239,16 @@ __global__ void __launch_bounds__(kMlpThreads, 2) mlp_rows_kernel(const __grid_c
                 const float4 p = __ldg(src + 2 * v), q = __ldg(src + 2 * v + 1);
                 ((uint4*)row)[v] = make_uint4(pack_half2(p.x, p.y), pack_half2(p.z, p.w), pack_half2(q.x, q.y), pack_half2(q.z, q.w));
             }
+            if (fd & 4u) {     // odd number of 4-float levels: one more half vector
+                const float4 p = __ldg(src + 2 * (fd / 8));
+                *(uint2*)(row + (fd & ~7u) * 2) = make_uint2(pack_half2(p.x, p.y), pack_half2(p.z, p.w));
+            }
         } else {
             const uint4* src = (const uint4*)((const __half*)features + qi * fd);
             for (uint32_t v = 0; v < fd / 8; ++v) ((uint4*)row)[v] = __ldg(src + v);
         }
-        write_row_tail(row, fd, M.k1, n, w, Q.extra, qi, Q.n_extra);
+        if (fd & 7u) write_row_tail_odd(row, fd, M.k1, n, w, Q.extra, qi, Q.n_extra);
+        else write_row_tail(row, fd, M.k1, n, w, Q.extra, qi, Q.n_extra);
         __syncwarp();
         float out[2][4];
         warp_mlp(smem_u32(s_a), smem_u32(s_w), M.k1, M.n_hidden, out);
@@ -247,7 +262,7 @@ static uint32_t mlp_smem_bytes(const MlpParams& M, int threads) { return M.image
 int launch_mlp_rows(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const void* features, float* rgb,
                     int n_sms, cudaStream_t stream) {
     if (Q.n == 0) return 0;
-    if (M.feat_dim % 8 != 0) return -1;
+    if (M.feat_dim % 4 != 0 || (M.feat_dim % 8 != 0 && !T.f32)) return -1;
     const uint32_t smem = mlp_smem_bytes(M, kMlpThreads);
     static std::atomic<uint64_t> opted{0};
     if (!opt_in_smem(opted, (const void*)mlp_rows_kernel, 200 * 1024)) return kLaunchCudaError;
@@ -313,11 +328,8 @@ __global__ void __launch_bounds__(kFusedThreads, 2) fused_mma_kernel(const __gri
         }
         if constexpr ((L * F) % 8 == 0) {
             write_row_tail(row, L * F, M.k1, n, w, Q.extra, qi, Q.n_extra);
-        } else {   // L*F = 4 mod 8: the tail starts mid-vector; write halves one by one
-            __half* r = (__half*)row;
-            for (uint32_t c = L * F; c < M.k1; ++c) r[c] = __float2half_rn(0.0f);
-            for (int k = 0; k < 3; ++k) { r[L * F + k] = __float2half_rn(n[k]); r[L * F + 3 + k] = __float2half_rn(w[k]); }
-            for (uint32_t k = 0; k < Q.n_extra; ++k) r[L * F + 6 + k] = __float2half_rn(__ldg(Q.extra + qi * Q.n_extra + k));
+        } else {   // L*F = 4 mod 8
+            write_row_tail_odd(row, L * F, M.k1, n, w, Q.extra, qi, Q.n_extra);
         }
         __syncwarp();
         float out[2][4];
