@@ -202,7 +202,7 @@ def ncu_facts(cfg: int):
 def ingest_ncu(args):
     """bench.py --ingest-ncu CSV --config K: read an `ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum,
     smsp__inst_executed.sum,gpu__time_duration.sum --csv --log-file CSV python bench.py --quick --config K ...` launch list and
-    store the LAST launch of the dominant kernel (name contains --ingest-kernel, default 'fused') in profiles/traffic.json,
+    store the last full-size launch of the dominant kernel (name contains --ingest-kernel, default 'fused') in profiles/traffic.json,
     stamped with the hash of the kernel sources."""
     import csv
     rows = [r for r in csv.reader(l for l in open(args.ingest_ncu) if l.startswith('"'))]
@@ -214,7 +214,10 @@ def ingest_ncu(args):
             launches.setdefault(int(r[k_id]), {"kernel": r[k_name].split("(")[0]})[r[k_metric]] = float(r[k_val].replace(",", ""))
     if not launches:
         raise SystemExit("no launch of a kernel matching %r in %s" % (args.ingest_kernel, args.ingest_ncu))
-    m = launches[max(launches)]
+    # the step's launch, not the smaller ones of the e2e leg's chunks: the last launch among those with the most instructions
+    key = "smsp__inst_executed.sum" if any("smsp__inst_executed.sum" in v for v in launches.values()) else "gpu__time_duration.sum"
+    top = max(v.get(key, 0) for v in launches.values())
+    m = launches[max(i for i, v in launches.items() if v.get(key, 0) >= 0.99 * top)]
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     d = json.load(open(tp)) if os.path.exists(tp) else {}
     d.pop("source", None)
