@@ -334,9 +334,7 @@ def run_ours(args):
     ctx = P.OctaOctree(local_rank).upload_workload(w)
     path = {"auto": P.PATH_AUTO, "mma": P.PATH_FUSED_MMA, "tc": P.PATH_FUSED_TC, "tm": P.PATH_FUSED_TC_TMEM, "unfused": P.PATH_UNFUSED, "generic": P.PATH_GENERIC}[args.path]
     ctx.oo_set_path(path)
-    if args.presort is None:
-        args.presort = "bin" if args.config == 4 else "none"
-    ctx.oo_set_presort(args.presort)
+    ctx.oo_set_presort(args.presort)              # default "auto": what a caller who sets nothing gets
     ctx.oo_reserve(q.n)
     cu = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a[lo:hi])).to(dev)
     x, nrm, wo, ex = cu(q.x), cu(q.nrm), cu(q.wo), cu(q.extra)
@@ -441,7 +439,7 @@ def run_ours(args):
     facts, stale = (None, "not looked up") if strong else ncu_facts(args.config)
     roof = {"bound": "hbm", "achieved": achieved, "peak": hbm, "unit": "GB/s", "frac": achieved / hbm,
             "traffic": facts["dram_bytes_per_launch"] if facts else None,
-            "peak_source": which, "kernel": "fused encode+MLP (one launch per step)" if args.presort == "none" else
+            "peak_source": which, "kernel": "fused encode+MLP (one launch per step)" if not info["presorted_last_query"] else
             "whole step: histogram + scan + bin_scatter + fused encode+MLP on the binned copy + unbin (traffic is the fused launch's)",
             "definition": "BASELINE.json north_star: ALGORITHMIC bytes (L*4 texels gathered + 36 B in + 12 B out per query) at the measured HBM peak, "
                           "vs the MLP FLOPs at the dense fp16 peak; the slower of the two is the roofline",
@@ -469,7 +467,8 @@ def run_ours(args):
         "ms_per_step": mx_ms, "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None, "dtype": "f16",
         "data": "synthetic", "config": desc,
         "run": {"l2": "flushed between steps (256 MB memset)", "path": PATH_NAMES[info["path_last_query"]], "ms_per_frame_warm_l2": mx_warm,
-                "presort": args.presort, "queries_per_rank": n_mine, "checksum_device": checksum_dev,
+                "presort": args.presort, "presorted": bool(info["presorted_last_query"]), "coherence_distinct_cells_per_32_queries": info["coherence_x100"] / 100.0,
+                "queries_per_rank": n_mine, "checksum_device": checksum_dev,
                 "parallelism": ("one GPU" if world == 1 else
                                 "replicated cache; ONE frame split into contiguous query slices, RGB all-gathered over NCCL inside the timed region" if strong else
                                 "replicated cache; every rank its own frame (camera seed = rank); no data-path collective")},
@@ -567,6 +566,7 @@ def run_sweep(args):
         q = w.queries
         ctx = P.OctaOctree(0).upload_workload(w)
         ctx.oo_reserve(q.n)
+        ctx.oo_set_presort("none")                      # this table is about explicit orders
         x, nrm, wo, ex = cu(q.x), cu(q.nrm), cu(q.wo), cu(q.extra)
         rgb = torch.empty((q.n, 3), dtype=torch.float32, device=dev)
         perm = torch.empty(q.n, dtype=torch.int32, device=dev)
@@ -587,6 +587,7 @@ def run_sweep(args):
         bq_fused = L * 4 * F * 2 + 48
         bq_enc = L * 4 * F * 2 + 24 + L * F * 2                           # x, wo in; features out
         ctx = P.OctaOctree(0).upload_workload(w)
+        ctx.oo_set_presort("none")                      # the plain columns are the unsorted call; bin and auto have their own
         n_max = 1 << args.sweep_max_log2
         side = 1 << ((args.sweep_max_log2 + 1) // 2)
         cam = gen.make_camera(side, n_max // side, 0)
@@ -621,9 +622,16 @@ def run_sweep(args):
                 ctx.oo_set_presort("bin", min_queries=1)
                 t_b = timed(lambda: ctx.oo_query(x, nrm, wo, rgb=rgb[:n]), reps)
                 t_be = timed(lambda: ctx.oo_encode(x, wo, features=feat[:n]), reps)
+                # the library's default: OO_PRESORT_AUTO at its default threshold (the warm-ups let it see the batch first)
+                ctx.oo_set_presort("auto")
+                t_a = timed(lambda: ctx.oo_query(x, nrm, wo, rgb=rgb[:n]), reps)
+                auto_binned = bool(ctx.oo_get_info()["presorted_last_query"])
+                t_ae = timed(lambda: ctx.oo_encode(x, wo, features=feat[:n]), reps)
                 ctx.oo_set_presort("none")
                 row.update({"bin_fused_ms": t_b, "bin_fused_roofline_frac": bq_fused * n / (t_b * 1e-3) / 1e9 / hbm,
-                            "bin_encode_ms": t_be, "bin_encode_roofline_frac": bq_enc * n / (t_be * 1e-3) / 1e9 / hbm})
+                            "bin_encode_ms": t_be, "bin_encode_roofline_frac": bq_enc * n / (t_be * 1e-3) / 1e9 / hbm,
+                            "auto_fused_ms": t_a, "auto_fused_roofline_frac": bq_fused * n / (t_a * 1e-3) / 1e9 / hbm, "auto_binned": auto_binned,
+                            "auto_encode_ms": t_ae, "auto_encode_roofline_frac": bq_enc * n / (t_ae * 1e-3) / 1e9 / hbm})
                 rows.append(row)
         out = {"sweep": "BASELINE.json configs[4]: batch size x query distribution on the config-3 tree and MLP",
                "tree_nodes": w.tree.n_nodes, "atlas_bytes": w.atlas.nbytes, "bytes_per_query": {"fused": bq_fused, "encode": bq_enc},
@@ -670,6 +678,7 @@ def run_raycast(args):
         w, desc = workload_for(cfg)
         cam, sc = w.camera, w.scene
         ctx = P.OctaOctree(0).upload_workload(w)
+        ctx.oo_set_presort("none")
         ctx.oo_upload_scene(sc.spheres, sc.lo, sc.hi)
         n = cam.width * cam.height
         out = tuple(torch.empty((n, 3), dtype=torch.float32, device=dev) for _ in range(3))
@@ -718,6 +727,7 @@ def run_full(args):
     q, disp = w.queries, w.meta["disparity"]
     L, F = len(w.tree.level_depth), w.atlas.F
     ctx = P.OctaOctree(0)
+    ctx.oo_set_presort("none")
     ctx.oo_upload_tree(w.tree, w.atlas.levels, w.atlas.dtype, dirmap="vertex")
     x, nrm, wo, ex, dd = cu(q.x), cu(q.nrm), cu(q.wo), cu(q.extra), cu(disp)
     rgb = torch.empty((q.n, 3), dtype=torch.float32, device=dev)
@@ -824,7 +834,7 @@ def main():
     ap.add_argument("--sweep-max-log2", type=int, default=24)
     ap.add_argument("--sweep-min-log2", type=int, default=16)
     ap.add_argument("--sweep-dist", default="both", choices=["both", "coherent", "incoherent"])
-    ap.add_argument("--presort", default=None, choices=["none", "bin"], help="oo_set_presort for the run (default: bin for --config 4, none otherwise)")
+    ap.add_argument("--presort", default="auto", choices=["auto", "none", "bin"], help="oo_set_presort for the run (default: the library's own default, auto)")
     ap.add_argument("--quick", action="store_true", help="timed region only (no warm-L2 / e2e / CPU legs): the command ncu wraps")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"], help="N > 1: every rank its own frame (weak) or one frame split across ranks + RGB all-gather (strong)")
     ap.add_argument("--dry-run-dist", action="store_true", help="the N > 1 host logic on CPU with gloo (launcher, sharding, gather, reductions): what the CPU tests drive; measures nothing")

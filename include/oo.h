@@ -108,7 +108,7 @@ typedef enum {
 } oo_path;
 
 /* Row a1 inside oo_query (BASELINE.json north_star: "an optional Morton pre-sort of queries for gather locality").
- * OO_PRESORT_NONE (default): queries are processed in the caller's order (or in queries.perm's).
+ * OO_PRESORT_NONE: queries are processed in the caller's order (or in queries.perm's).
  * OO_PRESORT_BIN: oo_query first bins the queries by the top 10 bits of their 30-bit Morton key (the octree cell at depth 3
  *   plus one bit: ONE counting pass, 3 launches) MOVING x, n, wo and the extras into library scratch, runs the chosen
  *   kernel path over the binned copy, and a last kernel brings the RGB back to the caller's order.  Results are
@@ -118,8 +118,17 @@ typedef enum {
  *   predicted on the binned copy) when queries.perm is NULL and n >= min_queries of oo_set_presort (default 262144:
  *   below that the extra launches cost more than they save); otherwise the call proceeds in the given order (oo_info.presorted_last_query says
  *   which).  oo_encode on OO_PATH_UNFUSED does the same with x and wo and stores every feature row at its query's index
- *   (oo_info.presorted_last_encode).  Needs oo_reserve(n). */
-typedef enum { OO_PRESORT_NONE = 0, OO_PRESORT_BIN = 1 } oo_presort;
+ *   (oo_info.presorted_last_encode).  Needs oo_reserve(n).
+ * OO_PRESORT_AUTO (default): the library decides per call between the two from the coherence of the recent calls' queries.
+ *   Every kernel that reads the queries in the caller's order samples, in a few of its warps, how many distinct depth-4
+ *   octree cells 32 consecutive queries fall into (1-3 for screen-order primary hits, ~30 for random surface samples) and
+ *   leaves the sample in a small device array that a library-owned side stream copies to the host after the call's kernels;
+ *   the next call reads what has arrived -- nothing waits, the call stays asynchronous, the caller's stream carries one extra
+ *   event record -- and bins when the mean exceeds 12 (and stops below 6).  The decision therefore lags one call: the first
+ *   incoherent batch of a stream runs unsorted.  Without reserved scratch AUTO proceeds unsorted instead of failing.  The
+ *   result bytes never depend on the decision.  oo_info.presort_auto_on / coherence_x100 report it.  Sampled by: the fused
+ *   tensor-memory kernel, the histogram pass of a binned call, oo_encode's specialised kernel, the full-query kernel. */
+typedef enum { OO_PRESORT_NONE = 0, OO_PRESORT_BIN = 1, OO_PRESORT_AUTO = 2 } oo_presort;
 
 /* The octree and its feature atlases ("every non-empty cell stores a learnable octahedral feature map").
  * Node 0 is the root (depth 0, the cube [0,1]^3); a node of depth d is a cell of side 2^-d with half-open extent.
@@ -205,6 +214,8 @@ typedef struct {
     uint32_t full_query;         /* 1 if oo_query runs the full-query kernel under the current tree / mode / decoder
                                     (mode != 0, vertex maps or width 128), i.e. oo_query_debug's outputs are [n][L][J]... */
     uint32_t n_neighbours;       /* J of the current mode: 8 (OO_SPATIAL_TRILINEAR8) or 1 */
+    uint32_t presort_auto_on;    /* OO_PRESORT_AUTO's current decision: 1 = the next batch of >= min_queries queries is binned */
+    uint32_t coherence_x100;     /* 100 x mean number of distinct depth-4 cells per 32 consecutive queries, latest sample */
 } oo_info;
 
 /* Create a context on a CUDA device.  Fails with OO_ERR_CUDA if the device is absent or is not compute capability
@@ -234,7 +245,7 @@ OO_API oo_status oo_reserve(oo_ctx* ctx, uint64_t max_queries);
 OO_API oo_status oo_set_path(oo_ctx* ctx, oo_path path);
 OO_API oo_status oo_get_info(const oo_ctx* ctx, oo_info* out);
 
-/* Switch the in-query pre-sort on or off; see oo_presort.  Batches of fewer than min_queries queries proceed unsorted;
+/* Select the in-query pre-sort policy (default OO_PRESORT_AUTO); see oo_presort.  Batches of fewer than min_queries queries proceed unsorted;
  * 0 selects the library default (262144, about where binning starts to pay on a B200).  OO_ERR_INVALID_ARG for an unknown
  * presort value. */
 OO_API oo_status oo_set_presort(oo_ctx* ctx, oo_presort presort, uint64_t min_queries);

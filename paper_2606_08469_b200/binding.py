@@ -69,7 +69,7 @@ class _Info(C.Structure):
                 ("atlas_bytes", C.c_uint64), ("path_last_query", C.c_uint32), ("path_last_encode", C.c_uint32),
                 ("hop_plan_ok", C.c_uint32), ("n_sms", C.c_uint32),
                 ("presorted_last_query", C.c_uint32), ("presorted_last_encode", C.c_uint32),
-                ("full_query", C.c_uint32), ("n_neighbours", C.c_uint32)]
+                ("full_query", C.c_uint32), ("n_neighbours", C.c_uint32), ("presort_auto_on", C.c_uint32), ("coherence_x100", C.c_uint32)]
 
 
 _lib = None
@@ -232,10 +232,11 @@ class OctaOctree:
     def oo_set_path(self, path: int):
         self._check(self._L.oo_set_path(self._ctx, int(path)))
 
-    def oo_set_presort(self, presort: str = "none", min_queries: int = 0):
-        """"none" (default) or "bin" (oo_query / oo_encode bin the queries by their top Morton bits first; see oo_presort).
+    def oo_set_presort(self, presort: str = "auto", min_queries: int = 0):
+        """"auto" (the library's default: decided from the coherence of the recent calls), "none", or "bin" (oo_query / oo_encode
+        bin the queries by their top Morton bits first; see oo_presort).
         Batches below min_queries proceed unsorted (0 = library default)."""
-        self._check(self._L.oo_set_presort(self._ctx, {"none": 0, "bin": 1}[presort], int(min_queries)))
+        self._check(self._L.oo_set_presort(self._ctx, {"none": 0, "bin": 1, "auto": 2}[presort], int(min_queries)))
 
     def oo_set_mode(self, spatial: str = "nearest", lookup: str = "wo", attrs: str = "n_wo"):
         m = _Mode(SPATIAL[spatial], LOOKUP[lookup], ATTRS[attrs])

@@ -62,8 +62,19 @@ struct oo_ctx {
     uint32_t *d_keys_a = nullptr, *d_keys_b = nullptr, *d_idx_a = nullptr, *d_hist = nullptr;
     float *d_qx = nullptr, *d_qn = nullptr, *d_qw = nullptr, *d_qe = nullptr, *d_rgb = nullptr, *d_qd = nullptr;
     // OO_PRESORT_BIN: the binned copy of the queries and their original indices (allocated by oo_reserve, `reserved` rows)
-    oo_presort presort = OO_PRESORT_NONE;
+    oo_presort presort = OO_PRESORT_AUTO;
     uint64_t bin_min = 1u << 18;           // batches below this proceed unsorted (the extra launches cost more than they save)
+    // OO_PRESORT_AUTO: coherence samples of the recent calls (see kStatSlots).  The kernels write them to d_stat in device
+    // memory; after a sampling call a copy to the pinned host array h_stat is enqueued on a library-owned side stream that
+    // waits for the call's kernels, so the caller's stream carries nothing extra and the host never waits.
+    unsigned long long* h_stat = nullptr;
+    unsigned long long* d_stat = nullptr;
+    cudaStream_t s_stat = nullptr;
+    cudaEvent_t ev_stat = nullptr;
+    bool armed = false;                    // the current call handed d_stat to a kernel
+    uint32_t stat_seq = 0;                 // sequence number of the last sampling call
+    bool auto_on = false;                  // current decision: bin the next large batch
+    float coherence = 0.0f;                // mean distinct depth-4 cells per 32 consecutive queries, latest sample
     float *d_bx = nullptr, *d_bn = nullptr, *d_bw = nullptr, *d_be = nullptr;
     uint32_t *d_binv = nullptr, *d_bidx = nullptr;
     float *d_brgb = nullptr, *d_bdisp = nullptr;
@@ -250,6 +261,19 @@ extern "C" OO_API oo_status oo_create(oo_ctx** out, int cuda_device) {
     c->device = cuda_device;
     c->n_sms = prop.multiProcessorCount;
     c->info.n_sms = (uint32_t)c->n_sms;
+    {   // OO_PRESORT_AUTO: sample array on the device, its pinned host copy, the side stream and event that bring it over
+        DeviceGuard g(cuda_device);
+        const size_t bytes = kStatSlots * sizeof(unsigned long long);
+        if (cudaMalloc((void**)&c->d_stat, bytes) == cudaSuccess && cudaMemset(c->d_stat, 0, bytes) == cudaSuccess &&
+            cudaHostAlloc((void**)&c->h_stat, bytes, cudaHostAllocDefault) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&c->s_stat, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaEventCreateWithFlags(&c->ev_stat, cudaEventDisableTiming) == cudaSuccess) {
+            memset(c->h_stat, 0, bytes);
+        } else {
+            (void)cudaGetLastError();
+            c->presort = OO_PRESORT_NONE;      // AUTO has nothing to decide from
+        }
+    }
     *out = c;
     return OO_OK;
 }
@@ -266,6 +290,13 @@ extern "C" OO_API void oo_destroy(oo_ctx* c) {
         free_dev(c->d_disp_image);
         free_scratch(c);
         free_pipe(c);
+        if (c->s_stat) {
+            cudaStreamSynchronize(c->s_stat);  // a copy into h_stat may still be in flight
+            cudaStreamDestroy(c->s_stat);
+        }
+        if (c->ev_stat) cudaEventDestroy(c->ev_stat);
+        if (c->h_stat) cudaFreeHost(c->h_stat);
+        if (c->d_stat) cudaFree(c->d_stat);
     }
     delete c;
 }
@@ -281,7 +312,8 @@ extern "C" OO_API oo_status oo_set_path(oo_ctx* c, oo_path path) {
 }
 extern "C" OO_API oo_status oo_set_presort(oo_ctx* c, oo_presort presort, uint64_t min_queries) {
     if (!c) return OO_ERR_INVALID_ARG;
-    if (presort != OO_PRESORT_NONE && presort != OO_PRESORT_BIN) return fail(c, OO_ERR_INVALID_ARG, "unknown presort %d", (int)presort);
+    if (presort != OO_PRESORT_NONE && presort != OO_PRESORT_BIN && presort != OO_PRESORT_AUTO) return fail(c, OO_ERR_INVALID_ARG, "unknown presort %d", (int)presort);
+    if (presort == OO_PRESORT_AUTO && !c->ev_stat) return fail(c, OO_ERR_UNSUPPORTED, "OO_PRESORT_AUTO: the sample buffers could not be created on this context");
     c->presort = presort;
     c->bin_min = min_queries ? min_queries : (1u << 18);
     return OO_OK;
@@ -305,6 +337,8 @@ extern "C" OO_API oo_status oo_get_info(const oo_ctx* c, oo_info* out) {
     out->hop_plan_ok = c->plan_ok ? 1u : 0u;
     out->full_query = c->mode.tri8 || c->mode.lookup || c->mode.attrs_paper || (c->have_tree && c->T.vertex) || (c->have_mlp && c->M.width != 64);
     out->n_neighbours = c->mode.tri8 ? 8u : 1u;
+    out->presort_auto_on = c->auto_on ? 1u : 0u;
+    out->coherence_x100 = (uint32_t)(c->coherence * 100.0f + 0.5f);
     return OO_OK;
 }
 
@@ -757,12 +791,55 @@ static oo_status need_bin(oo_ctx* c, uint64_t n) {
 
 // a1' for oo_query: one counting pass on the top Morton bits moves the queries (and a caller-supplied d^) into the binned
 // scratch; *qb then describes the binned copy.  The chosen kernel runs over it into c->d_brgb and unbin restores the order.
-static bool bin_wanted(const oo_ctx* c, const oo_queries* q) {
-    return c->presort == OO_PRESORT_BIN && !q->perm && q->n >= c->bin_min;
+// OO_PRESORT_AUTO: fold the newest coherence sample the kernels have left into the decision.  Slots carry the sequence number of
+// the call that wrote them; the newest call present wins (a call still running contributes the blocks that have finished).
+// Hysteresis: on above 12 distinct cells per 32 queries, off below 6 (screen-order frames measure 1-3, random surface samples ~30).
+static void update_coherence(oo_ctx* c) {
+    if (!c->ev_stat) return;
+    const uint32_t mask = (1u << kStatSeqBits) - 1u;
+    uint32_t best_age = ~0u;
+    uint64_t sum = 0, cnt = 0;
+    for (uint32_t k = 0; k < kStatSlots; ++k) {
+        const unsigned long long v = ((volatile unsigned long long*)c->h_stat)[k];
+        const uint32_t n = (uint32_t)(v >> 32) & ((1u << kStatCntBits) - 1u);
+        if (!n) continue;
+        const uint32_t age = (c->stat_seq - (uint32_t)(v >> 44)) & mask;
+        if (age < best_age) { best_age = age; sum = cnt = 0; }
+        if (age == best_age) { sum += (uint32_t)v; cnt += n; }
+    }
+    if (cnt < 16) return;                     // too few warps sampled to say anything
+    c->coherence = (float)sum / (float)cnt;
+    c->auto_on = c->coherence > (c->auto_on ? 6.0f : 12.0f);
+}
+// Does this call sample?  (Only under AUTO; the kernel that sees the caller's order gets the pointer.)
+static void arm_sampling(oo_ctx* c, QueryParams& Q) {
+    if (c->presort != OO_PRESORT_AUTO || !c->ev_stat || Q.perm) return;
+    c->stat_seq = (c->stat_seq + 1) & ((1u << kStatSeqBits) - 1u);
+    Q.stat = c->d_stat;
+    Q.stat_seq = c->stat_seq;
+    c->armed = true;
+}
+// After the kernels of a sampling call have been enqueued on the caller's stream: the side stream waits for them and copies the
+// sample array to the host.  Nothing is added to the caller's stream but an event record; failures only lose the sample.
+static void collect_samples(oo_ctx* c, cudaStream_t stream) {
+    if (!c->armed) return;
+    c->armed = false;
+    if (cudaEventRecord(c->ev_stat, stream) != cudaSuccess || cudaStreamWaitEvent(c->s_stat, c->ev_stat, 0) != cudaSuccess ||
+        cudaMemcpyAsync(c->h_stat, c->d_stat, kStatSlots * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->s_stat) != cudaSuccess)
+        (void)cudaGetLastError();
+}
+static bool bin_wanted(oo_ctx* c, const oo_queries* q) {
+    if (q->perm || q->n < c->bin_min) return false;
+    if (c->presort == OO_PRESORT_BIN) return true;
+    if (c->presort != OO_PRESORT_AUTO) return false;
+    update_coherence(c);
+    return c->auto_on && q->n <= c->reserved;      // AUTO never fails a call for missing scratch: it proceeds unsorted
 }
 static oo_status bin_for_query(oo_ctx* c, const oo_queries* q, oo_queries* qb, cudaStream_t stream, bool want_idx = false) {
     if (oo_status st = need_bin(c, q->n)) return st;
-    const int k = launch_bin_queries(make_qp(q), c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv,
+    QueryParams Qs = make_qp(q);
+    arm_sampling(c, Qs);                     // binned call: the histogram kernel is the one that sees the caller's order
+    const int k = launch_bin_queries(Qs, c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv,
                                      want_idx ? c->d_bidx : nullptr, q->disparity ? c->d_bdisp : nullptr, stream);
     if (k < 0) return launch_failed(c, k, "bin pass");
     count(c, k);
@@ -813,21 +890,26 @@ extern "C" OO_API oo_status oo_encode(oo_ctx* c, const oo_queries* q, void* d_fe
     QueryParams Q = make_qp(q);
     EncodeOut O{d_features, d_slot, d_texel};
     c->info.presorted_last_encode = 0;
-    if (c->presort == OO_PRESORT_BIN && p == OO_PATH_UNFUSED && !q->perm && q->n >= c->bin_min) {
+    if (p == OO_PATH_UNFUSED && bin_wanted(c, q)) {
         // a1': x and wo move into Morton bins; the encode kernel reads them in order and stores every row at its query's index
         if (oo_status st = need_bin(c, q->n)) return st;
         Q.nrm = nullptr; Q.extra = nullptr; Q.n_extra = 0;
+        arm_sampling(c, Q);
         const int k = launch_bin_queries(Q, c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, c->d_bidx, nullptr, (cudaStream_t)cuda_stream);
         if (k < 0) return launch_failed(c, k, "bin pass");
         count(c, k);
         Q.x = c->d_bx; Q.wo = c->d_bw; Q.out_idx = c->d_bidx;
+        Q.stat = nullptr;
         c->info.presorted_last_encode = 1;
+    } else if (p == OO_PATH_UNFUSED) {
+        arm_sampling(c, Q);
     }
     int n = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Q, O, c->tree_max_depth, (cudaStream_t)cuda_stream)
                                  : launch_encode_fast(c->T, Q, O, c->n_sms, (cudaStream_t)cuda_stream);
     if (n < 0) return launch_failed(c, n, "encode kernel");
     count(c, n);
     c->info.path_last_encode = (uint32_t)p;
+    collect_samples(c, (cudaStream_t)cuda_stream);
     return check_after(c);
 }
 
@@ -945,6 +1027,7 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
         Q = make_qp(&qd);
         Q.dbg_slot = dbg.slot; Q.dbg_texel = dbg.index;
         if (c->info.presorted_last_query && dbg.on()) Q.out_idx = c->d_bidx;
+        if (!c->info.presorted_last_query) arm_sampling(c, Q);
         if (dbg.on())
             n = c->M.width == 64 ? launch_fused_full_w64_dbg(c->T, c->M, Q, c->mode, out, c->n_sms, stream)
                                  : launch_fused_full_w128_dbg(c->T, c->M, Q, c->mode, out, c->n_sms, stream);
@@ -961,6 +1044,7 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
         Q = make_qp(&qd);
         Q.dbg_slot = dbg.slot; Q.dbg_texel = dbg.index;
         if (c->info.presorted_last_query && dbg.on()) Q.out_idx = c->d_bidx;
+        if (!c->info.presorted_last_query) arm_sampling(c, Q);
         // OO_PATH_AUTO walks down the chain until a kernel exists for the shape: activations in tensor memory -> A tile in
         // shared memory -> mma.sync -> features through HBM.  An explicit path runs that kernel or fails.
         const bool walk = c->path == OO_PATH_AUTO;
@@ -1011,6 +1095,7 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
     count(c, n);
     if (c->info.presorted_last_query) count(c, launch_unbin(c->d_brgb, c->d_binv, q->n, c->M.out_dim, d_rgb, c->n_sms, stream));
     c->info.path_last_query = (uint32_t)p;
+    collect_samples(c, stream);
     return check_after(c);
 }
 

@@ -89,6 +89,7 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
 
     uint32_t tile = team * gridDim.x + blockIdx.x;        // the partial last round spreads one tile per SM (see oo_fused_tm.cu)
     if (tile < n_tiles && part == 0) prefetch(tile);
+    bool sample = Q.stat != nullptr;
     for (; tile < n_tiles; tile += tile_stride) {
         const bool valid = (uint64_t)tile * 128 + row < Q.n;
         if (part == 0) asm volatile("cp.async.wait_group 0;" ::: "memory");
@@ -96,6 +97,10 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
         float x[3], w[3], wl[3];
 #pragma unroll
         for (int k = 0; k < 3; ++k) { x[k] = s_q[k * 128]; w[k] = s_q[(6 + k) * 128]; }
+        if (sample) {                        // OO_PRESORT_AUTO: the first tile of every team
+            if (part == 0 && team == 0) stat_sample_warp(Q, blockIdx.x * 4 + (warp & 3u), x[0], x[1], x[2]);
+            sample = false;
+        }
         if (mode.lookup == OO_LOOKUP_WO) {
 #pragma unroll
             for (int a = 0; a < 3; ++a) wl[a] = w[a];

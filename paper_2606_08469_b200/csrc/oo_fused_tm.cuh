@@ -118,6 +118,10 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
 
     mbar_wait(bar_d, 0);                  // descent tables in shared memory
     bool w_ready = false;
+    if (Q.stat && wg == 0 && tile < n_tiles) {   // OO_PRESORT_AUTO: the warps of warpgroup 0 sample their first tile, before the tile loop
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
+        stat_sample_warp(Q, blockIdx.x * 4 + warp, s_q[0], s_q[128], s_q[256]);
+    }
     for (; tile < n_tiles; tile += tile_stride) {
         float x[3], w[3];
         const bool valid = (uint64_t)tile * kRows + row < Q.n;

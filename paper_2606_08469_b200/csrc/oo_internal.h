@@ -62,6 +62,10 @@ struct QueryParams {
     const float* disparity;  // [n] or nullptr (OO_LOOKUP_SHIFTED)
     const uint32_t* out_idx; // encode kernels and the debug instances (OO_PRESORT_BIN): thread t reads query t and stores its
                              // feature / index rows at out_idx[t] (the query's index in the caller's order)
+    // OO_PRESORT_AUTO: where the kernel that sees the queries in the CALLER's order leaves its coherence samples (slots of a
+    // small device array) and the call's sequence number; null = no sampling
+    unsigned long long* stat;
+    uint32_t stat_seq;
     int32_t* dbg_slot;       // oo_query_debug only (read by the DBG instances of the fused kernels): [n][L] (full query [n][L][J])
     int16_t* dbg_texel;      // ... and [n][L][2] (full query [n][L][J][3]); either may be null
 };
@@ -104,6 +108,17 @@ struct EncodeOut {
 };
 
 // ---------------------------------------------------------------------------------------------------------------
+// Coherence statistics (OO_PRESORT_AUTO).  A warp holds 32 consecutive queries of the caller's order; the number of distinct
+// depth-4 cells (16^3) among them is ~1-3 for screen-order primary hits and ~30 for random surface samples.  Sampled warps add
+// write (sequence number of the call, 1, distinct) into a slot of a small device array; a side stream copies the array to pinned
+// host memory after the call's kernels, and the host reads whatever is there when the next call is made: nothing but an event
+// record is added to the caller's stream and nobody waits (every slot is always a whole sample of some recent call).
+constexpr uint32_t kStatSlots = 256;
+constexpr uint32_t kStatSeqBits = 20, kStatCntBits = 12;
+inline unsigned long long stat_pack(uint32_t seq, uint32_t cnt, uint32_t sum) {
+    return ((unsigned long long)(seq & ((1u << kStatSeqBits) - 1u)) << 44) | ((unsigned long long)(cnt & ((1u << kStatCntBits) - 1u)) << 32) | sum;
+}
+
 // cudaFuncAttributeMaxDynamicSharedMemorySize is a PER-DEVICE attribute of a kernel: a context on device 1 created after one
 // on device 0 in the same process needs the opt-in again.  Every launch site therefore owns one bit per device ordinal
 // (`mask`, a function-local static of that site, one per kernel instance) and opts in the first time it launches on the

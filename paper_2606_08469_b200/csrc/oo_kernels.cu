@@ -118,12 +118,17 @@ __global__ void __launch_bounds__(256) encode_fast_kernel(const __grid_constant_
     stage_to_smem(s_dense, T.dense, T.dense_ints * 4);
     __syncthreads();
     constexpr int TB = F * (F32 ? 4 : 2);
+    bool sample = Q.stat != nullptr && threadIdx.x < 32;      // OO_PRESORT_AUTO: warp 0 of every block samples the first queries it takes
     for (uint64_t t = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; t < Q.n; t += (uint64_t)gridDim.x * blockDim.x) {
         const uint64_t qi = Q.perm ? Q.perm[t] : t;
         const uint64_t oi = Q.out_idx ? Q.out_idx[t] : qi;      // where this query's rows go (binned queries: its own index)
         float x[3], w[3];
         load3(Q.x, qi, x);
         load3(Q.wo, qi, w);
+        if (sample) {
+            if ((t | 31u) < Q.n) stat_sample_warp(Q, blockIdx.x, x[0], x[1], x[2]);    // warp-uniform: t | 31 is the warp's last query
+            sample = false;
+        }
         Encoded<L, F, F32> e;
         locate<L, F, F32>(T, s_dense, x, w, e);
 #pragma unroll

@@ -36,10 +36,13 @@ __device__ __forceinline__ uint32_t morton_of(const float* __restrict__ x, uint6
 
 // hist[digit * n_tiles + tile] = number of keys of that digit in the tile; tot[digit] += the same (digit totals of
 // the pass).  FIRST: the keys are made here (from x) and written out, so there is no separate key kernel.
+// stat (OO_PRESORT_AUTO, FIRST only): this is the kernel that sees the queries in the caller's order when a call is binned, so it
+// leaves the coherence sample (distinct depth-4 cells = top 12 key bits among 32 consecutive queries, one warp-sample per warp).
 template <bool FIRST, int THREADS>
 __global__ void __launch_bounds__(THREADS) radix_hist_kernel(const float* __restrict__ x, uint32_t* __restrict__ keys, uint64_t n,
                                                              uint32_t shift, uint32_t n_tiles, uint32_t* __restrict__ hist,
-                                                             uint32_t* __restrict__ tot) {
+                                                             uint32_t* __restrict__ tot, unsigned long long* stat = nullptr,
+                                                             uint32_t stat_seq = 0) {
     // THREADS threads share one 4096-key tile: 256 for the sort's later passes (many tiles in flight anyway), 1024 where the
     // pass runs alone in front of the query and a tile's 16 dependent rounds per thread would be the critical path
     constexpr int ITEMS = kTile / THREADS;
@@ -59,9 +62,21 @@ __global__ void __launch_bounds__(THREADS) radix_hist_kernel(const float* __rest
                 key = keys[i];
             }
             atomicAdd(&cnt[(key >> shift) & (kDigits - 1)], 1u);
+            if constexpr (FIRST) {
+                if (it == 0 && stat && threadIdx.x < 32 && base + 31u < n) {      // warp 0, a whole warp (warp-uniform condition)
+                    const uint32_t peers = __match_any_sync(0xffffffffu, key >> 18);
+                    const bool leader = (uint32_t)(__ffs(peers) - 1) == threadIdx.x;
+                    const uint32_t distinct = __popc(__ballot_sync(0xffffffffu, leader));
+                    // one slot of the device sample array per block (see stat_sample_warp)
+                    if (threadIdx.x == 0)
+                        *(volatile unsigned long long*)(stat + (blockIdx.x % kStatSlots)) =
+                            ((unsigned long long)(stat_seq & ((1u << kStatSeqBits) - 1u)) << 44) | (1ull << 32) | distinct;
+                }
+            }
         }
     }
     __syncthreads();
+
     for (int d = threadIdx.x; d < kDigits; d += THREADS) {
         const uint32_t c = cnt[d];
         hist[(size_t)d * n_tiles + blockIdx.x] = c;
@@ -371,7 +386,7 @@ int launch_bin_queries(const QueryParams& Q, uint32_t* keys, uint32_t* hist, flo
     uint32_t* tot = hist + (size_t)n_tiles * kDigits;
     cudaMemsetAsync(tot, 0, sizeof(uint32_t) * kDigits, stream);
     constexpr uint32_t shift = 30 - kBits;
-    radix_hist_kernel<true, 1024><<<n_tiles, 1024, 0, stream>>>(Q.x, keys, Q.n, shift, n_tiles, hist, tot);
+    radix_hist_kernel<true, 1024><<<n_tiles, 1024, 0, stream>>>(Q.x, keys, Q.n, shift, n_tiles, hist, tot, Q.stat, Q.stat_seq);
     scan_kernel<<<kDigits, kSortThreads, 0, stream>>>(hist, tot, n_tiles);
     const BinPayload B{Q.x, Q.nrm, Q.wo, Q.extra, Q.extra ? Q.n_extra : 0u, sx, sn, sw, se, idx, sdisp ? Q.disparity : nullptr, sdisp};
     bin_scatter_kernel<<<n_tiles, kBinThreads, kBinSmemBytes, stream>>>(keys, Q.n, shift, n_tiles, hist, B, inv);

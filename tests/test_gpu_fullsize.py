@@ -52,6 +52,7 @@ def test_config2_full_frame_all_queries():
     f, s, t = co.encode(q.x, q.wo)
     ctx = P.OctaOctree(0).upload_workload(w)
     ctx.oo_reserve(q.n)
+    ctx.oo_set_presort("none")
     x, n, wo, ex = _dev(q.x), _dev(q.nrm), _dev(q.wo), _dev(q.extra)
     got, s_d, t_d = ctx.oo_query_debug(x, n, wo, ex)
     assert ctx.oo_get_info()["path_last_query"] == P.PATH_FUSED_TC_TMEM
@@ -112,6 +113,7 @@ def test_config3_full_tree_sampled_queries():
     # threshold; the oracle on every 61st query, the two launches against each other on all of them
     qi = gen.incoherent_queries(w.scene, 1 << 22, 0)
     xi, ni, wi = _dev(qi.x), _dev(qi.nrm), _dev(qi.wo)
+    ctx.oo_set_presort("none")
     plain = ctx.oo_query(xi, ni, wi)
     ctx.oo_reserve(qi.n)
     ctx.oo_set_presort("bin")
@@ -175,6 +177,7 @@ def test_config4_2pow24_queries(dist):
     assert q.n == n
     ctx = P.OctaOctree(0).upload_workload(w)
     ctx.oo_reserve(n)
+    ctx.oo_set_presort("none")
     x, nr, wo = _dev(q.x), _dev(q.nrm), _dev(q.wo)
     plain = ctx.oo_query(x, nr, wo)
     assert ctx.oo_get_info()["path_last_query"] == P.PATH_FUSED_TC_TMEM

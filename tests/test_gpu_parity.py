@@ -508,3 +508,51 @@ def test_two_contexts_in_one_process(P):
             assert torch.equal(rc.cpu(), a.oo_query(x1, n1, wo1).cpu())
         c.oo_set_presort("bin", min_queries=1)
         assert torch.equal(c.oo_query(to1(x1), to1(n1), to1(wo1)).cpu(), rc.cpu())
+
+
+def test_presort_auto_follows_the_coherence_of_the_queries(P):
+    """OO_PRESORT_AUTO (the default): kernels leave a coherence sample (distinct depth-4 cells per 32 consecutive queries) in
+    a small device array that a side stream copies to the host, and the next call decides from it.  A screen-order frame measures ~1-3 and stays unsorted; random surface
+    samples measure ~30 and are binned from the second call on; the bytes never depend on the decision."""
+    w = gen.scene_workload(1, width=512, height=512)               # 262,144 queries = the default threshold
+    qc = w.queries
+    qi = gen.incoherent_queries(w.scene, qc.n, 0)
+    ctx = P.OctaOctree(0).upload_workload(w)
+    xc, nc, wc, _ = _dev(qc)
+    xi, ni, wi, _ = _dev(qi)
+    ctx.oo_set_presort("none")
+    ref_c, ref_i = ctx.oo_query(xc, nc, wc), ctx.oo_query(xi, ni, wi)
+    ctx.oo_set_presort("auto")
+    assert torch.equal(ctx.oo_query(xi, ni, wi), ref_i)             # no scratch reserved: AUTO proceeds unsorted, no error
+    assert ctx.oo_get_info()["presorted_last_query"] == 0
+    ctx.oo_reserve(qc.n)
+    ctx.oo_query(xc[:4096], nc[:4096], wc[:4096])                   # a small coherent call (never binned) leaves a coherent sample
+    torch.cuda.synchronize()
+    for _ in range(3):                                              # coherent: never binned
+        assert torch.equal(ctx.oo_query(xc, nc, wc), ref_c)
+        torch.cuda.synchronize()
+        info = ctx.oo_get_info()
+        assert info["presorted_last_query"] == 0
+    ctx.oo_query(xc[:4096], nc[:4096], wc[:4096])                   # (a small call folds the newest sample into the decision too)
+    info = ctx.oo_get_info()
+    assert info["presort_auto_on"] == 0 and 100 <= info["coherence_x100"] < 600, info
+    seen = []
+    for _ in range(4):                                              # incoherent: unsorted once (the decision lags one call), then binned
+        assert torch.equal(ctx.oo_query(xi, ni, wi), ref_i)
+        torch.cuda.synchronize()
+        seen.append(ctx.oo_get_info()["presorted_last_query"])
+    assert seen == [0, 1, 1, 1], seen
+    info = ctx.oo_get_info()
+    assert info["presort_auto_on"] == 1 and info["coherence_x100"] > 2000, info
+    seen = []
+    for _ in range(3):                                              # back to screen order: binned once more (the lag), then not
+        assert torch.equal(ctx.oo_query(xc, nc, wc), ref_c)
+        torch.cuda.synchronize()
+        seen.append(ctx.oo_get_info()["presorted_last_query"])
+    assert seen == [1, 0, 0], seen
+    # oo_encode's specialised kernel and its histogram pass sample too
+    f_ref = ctx.oo_encode(xi, wi)
+    torch.cuda.synchronize()
+    f2 = ctx.oo_encode(xi, wi)
+    torch.cuda.synchronize()
+    assert ctx.oo_get_info()["presorted_last_encode"] == 1 and torch.equal(f2, f_ref)
