@@ -76,7 +76,7 @@ struct oo_ctx {
     bool auto_on = false;                  // current decision: bin the next large batch
     float coherence = 0.0f;                // mean distinct depth-4 cells per 32 consecutive queries, latest sample
     float *d_bx = nullptr, *d_bn = nullptr, *d_bw = nullptr, *d_be = nullptr;
-    uint32_t *d_binv = nullptr, *d_bidx = nullptr;
+    uint32_t *d_binv = nullptr, *d_bidx = nullptr, *d_btot = nullptr;   // d_btot: the bin pass's digit totals (zero between calls)
     float *d_brgb = nullptr, *d_bdisp = nullptr;
 
     // oo_query_host pipeline: copy-in and copy-out streams beside the caller's stream, one event pair per chunk
@@ -160,7 +160,7 @@ void free_scratch(oo_ctx* c) {
     void** ps[] = {(void**)&c->d_keys_a, (void**)&c->d_keys_b, (void**)&c->d_idx_a, (void**)&c->d_hist, (void**)&c->d_qx,
                    (void**)&c->d_qn,     (void**)&c->d_qw,     (void**)&c->d_qe,    (void**)&c->d_rgb, (void**)&c->d_qd};
     for (void** p : ps) free_dev(*p);
-    void** bs[] = {(void**)&c->d_bx, (void**)&c->d_bn, (void**)&c->d_bw, (void**)&c->d_be, (void**)&c->d_binv, (void**)&c->d_bidx, (void**)&c->d_brgb, (void**)&c->d_bdisp};
+    void** bs[] = {(void**)&c->d_bx, (void**)&c->d_bn, (void**)&c->d_bw, (void**)&c->d_be, (void**)&c->d_binv, (void**)&c->d_bidx, (void**)&c->d_brgb, (void**)&c->d_bdisp, (void**)&c->d_btot};
     for (void** p : bs) free_dev(*p);
     c->reserved = 0;
 }
@@ -774,6 +774,8 @@ extern "C" OO_API oo_status oo_reserve(oo_ctx* c, uint64_t n) {
     OO_CUDA(c, cudaMalloc((void**)&c->d_bidx, n * 4));
     OO_CUDA(c, cudaMalloc((void**)&c->d_brgb, n * 4 * 8));
     OO_CUDA(c, cudaMalloc((void**)&c->d_bdisp, n * 4));
+    OO_CUDA(c, cudaMalloc((void**)&c->d_btot, 1024 * 4));
+    OO_CUDA(c, cudaMemset(c->d_btot, 0, 1024 * 4));
     c->reserved = n;
     return OO_OK;
 }
@@ -839,7 +841,7 @@ static oo_status bin_for_query(oo_ctx* c, const oo_queries* q, oo_queries* qb, c
     if (oo_status st = need_bin(c, q->n)) return st;
     QueryParams Qs = make_qp(q);
     arm_sampling(c, Qs);                     // binned call: the histogram kernel is the one that sees the caller's order
-    const int k = launch_bin_queries(Qs, c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv,
+    const int k = launch_bin_queries(Qs, c->d_keys_a, c->d_hist, c->d_btot, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv,
                                      want_idx ? c->d_bidx : nullptr, q->disparity ? c->d_bdisp : nullptr, stream);
     if (k < 0) return launch_failed(c, k, "bin pass");
     count(c, k);
@@ -895,7 +897,7 @@ extern "C" OO_API oo_status oo_encode(oo_ctx* c, const oo_queries* q, void* d_fe
         if (oo_status st = need_bin(c, q->n)) return st;
         Q.nrm = nullptr; Q.extra = nullptr; Q.n_extra = 0;
         arm_sampling(c, Q);
-        const int k = launch_bin_queries(Q, c->d_keys_a, c->d_hist, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, c->d_bidx, nullptr, (cudaStream_t)cuda_stream);
+        const int k = launch_bin_queries(Q, c->d_keys_a, c->d_hist, c->d_btot, c->d_bx, c->d_bn, c->d_bw, c->d_be, c->d_binv, c->d_bidx, nullptr, (cudaStream_t)cuda_stream);
         if (k < 0) return launch_failed(c, k, "bin pass");
         count(c, k);
         Q.x = c->d_bx; Q.wo = c->d_bw; Q.out_idx = c->d_bidx;

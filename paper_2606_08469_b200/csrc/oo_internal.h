@@ -183,7 +183,7 @@ int launch_raycast(const double* d_spheres, uint32_t n_spheres, double lo, doubl
 int launch_morton_sort(const float* x, uint64_t n, uint32_t* keys_a, uint32_t* keys_b, uint32_t* idx_a, uint32_t* perm_out,
                        uint32_t* hist, cudaStream_t stream);
 size_t morton_sort_hist_ints(uint64_t n);
-int launch_bin_queries(const QueryParams& Q, uint32_t* keys, uint32_t* hist, float* sx, float* sn, float* sw, float* se,
+int launch_bin_queries(const QueryParams& Q, uint32_t* keys, uint32_t* hist, uint32_t* bin_tot, float* sx, float* sn, float* sw, float* se,
                        uint32_t* inv, uint32_t* idx, float* sdisp, cudaStream_t stream);
 int launch_unbin(const float* binned, const uint32_t* inv, uint64_t n, uint32_t out_dim, float* out, int n_sms, cudaStream_t stream);
 
