@@ -427,14 +427,23 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
         // texel maps: (R+2)^2 with the wrapped border; vertex maps: the (R+1)^2 vertices as given
         const uint32_t R = t->level_res[l], Rp = vertex ? R + 1 : R + 2;
         const uint64_t slots = std::max<uint64_t>(t->level_slots[l], 1);      // at least one (zero) map, so that the branch-free gather has an address
-        const uint64_t bytes = slots * Rp * Rp * texel_bytes;
+        const uint64_t map_bytes = (uint64_t)Rp * Rp * texel_bytes;
+        const uint64_t lead = vertex ? 0 : map_bytes;                         // texel maps: the all-zero map "slot -1" in front of slot 0
+        const uint64_t bytes = lead + slots * map_bytes;
+        if (bytes / 16 >= (1ull << 32)) return fail(c, OO_ERR_UNSUPPORTED, "level %u: %llu bytes of maps; a level is addressed in 32-bit units of 16 bytes (64 GB)", l, (unsigned long long)bytes);
         OO_CUDA(c, cudaMalloc(&c->atlas_dev[l], bytes));
         atlas_bytes += bytes;
-        if (t->level_slots[l] == 0) OO_CUDA(c, cudaMemsetAsync(c->atlas_dev[l], 0, bytes, stream));
-        else if (vertex) OO_CUDA(c, cudaMemcpyAsync(c->atlas_dev[l], t->atlas[l], bytes, cudaMemcpyDeviceToDevice, stream));
-        else launches += launch_pad_atlas(t->atlas[l], c->atlas_dev[l], t->level_slots[l], R, texel_bytes, stream);
+        uint8_t* slot0 = (uint8_t*)c->atlas_dev[l] + lead;
+        if (lead) OO_CUDA(c, cudaMemsetAsync(c->atlas_dev[l], 0, lead, stream));
+        if (t->level_slots[l] == 0) OO_CUDA(c, cudaMemsetAsync(slot0, 0, slots * map_bytes, stream));
+        else if (vertex) OO_CUDA(c, cudaMemcpyAsync(slot0, t->atlas[l], slots * map_bytes, cudaMemcpyDeviceToDevice, stream));
+        else launches += launch_pad_atlas(t->atlas[l], slot0, t->level_slots[l], R, texel_bytes, stream);
         LevelParams& lv = T.lv[l];
-        lv.atlas = (const uint8_t*)c->atlas_dev[l] + (vertex ? 0 : (uint64_t)(Rp + 1) * texel_bytes);
+        lv.atlas = slot0 + (vertex ? 0 : (uint64_t)(Rp + 1) * texel_bytes);
+        lv.atlas_z = vertex ? nullptr : (const uint8_t*)c->atlas_dev[l];
+        lv.map16 = (uint32_t)(map_bytes / 16);
+        lv.tap16 = (Rp + 1) * texel_bytes / 16;
+        lv.rp_f = (float)Rp;
         lv.half_r = 0.5f * (float)R;
         lv.off = 0.5f * (float)R - 0.5f;
         lv.R = R; lv.Rp = Rp;
@@ -1256,6 +1265,6 @@ extern "C" OO_API oo_status oo_read_padded_map(oo_ctx* c, uint32_t level, uint32
     if (c->T.vertex) return fail(c, OO_ERR_UNSUPPORTED, "vertex maps are stored as given (no padded copy)");
     DeviceGuard g(c->device);
     const LevelParams& lv = c->T.lv[level];
-    OO_CUDA(c, cudaMemcpy(h_out, (const uint8_t*)c->atlas_dev[level] + (uint64_t)slot * lv.map_bytes, lv.map_bytes, cudaMemcpyDeviceToHost));
+    OO_CUDA(c, cudaMemcpy(h_out, (const uint8_t*)c->atlas_dev[level] + (uint64_t)(slot + 1) * lv.map_bytes, lv.map_bytes, cudaMemcpyDeviceToHost));   // + 1: the zero map
     return OO_OK;
 }

@@ -138,8 +138,7 @@ __global__ void __launch_bounds__(NWG * 128, MINB) fused_tc_kernel(const __grid_
 #pragma unroll
                 for (int b = 0; b < NB; ++b)
                     if (l0 + b < L) {
-                        const Tap tp = level_tap(e.uv, T.lv[l0 + b].half_r, T.lv[l0 + b].off);
-                        gather_level<F, F32>(T.lv[l0 + b], e.slot[l0 + b], tp, h[b], dbg, l0 + b);
+                        gather_level<F, F32>(T.lv[l0 + b], e.slot[l0 + b], e.uv, h[b], dbg, l0 + b);
                     }
             }
 #pragma unroll

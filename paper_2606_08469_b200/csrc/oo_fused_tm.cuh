@@ -122,10 +122,22 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
         asm volatile("cp.async.wait_group 0;" ::: "memory");
         stat_sample_warp(Q, blockIdx.x * 4 + warp, s_q[0], s_q[128], s_q[256]);
     }
+#ifdef OO_PROFILE_PHASES      // -DOO_PROFILE_PHASES: per-warp cycle counts of the phases of a tile (one block prints them); never in the product build
+    long long t_gather = 0, t_mlp = 0, t_wait = 0, t_q = 0, t_bar = 0;
+    int n_done = 0;
+    const long long t_begin = clock64();
+#endif
     for (; tile < n_tiles; tile += tile_stride) {
         float x[3], w[3];
         const bool valid = (uint64_t)tile * kRows + row < Q.n;
+#ifdef OO_PROFILE_PHASES
+        const long long t0 = clock64();
+#endif
         asm volatile("cp.async.wait_group 0;" ::: "memory");
+#ifdef OO_PROFILE_PHASES
+        const long long t0b = clock64();
+        long long tw = 0, tb = 0;
+#endif
 #pragma unroll
         for (int k = 0; k < 3; ++k) { x[k] = s_q[k * 128]; w[k] = s_q[(6 + k) * 128]; }
         // ------------------------------------------------------------------ gather: one query per thread -> A0 in TMEM
@@ -185,8 +197,7 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
 #pragma unroll
                     for (int b = 0; b < NB; ++b)
                         if (l0 + b < L) {
-                            const Tap tp = level_tap(e.uv, T.lv[l0 + b].half_r, T.lv[l0 + b].off);
-                            gather_level<F, F32>(T.lv[l0 + b], e.slot[l0 + b], tp, h[b], dbg, l0 + b);
+                            gather_level<F, F32>(T.lv[l0 + b], e.slot[l0 + b], e.uv, h[b], dbg, l0 + b);
                         }
                 }
 #pragma unroll
@@ -206,7 +217,9 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
 #pragma unroll
             for (int v = 0; v < N_LATE / 4; ++v) tmem_st4(a0 + 4 * v, late[4 * v], late[4 * v + 1], late[4 * v + 2], late[4 * v + 3]);
         }
-        {   // attributes + zero padding up to k1, read late from the staging buffer
+        {   // attributes + zero padding up to k1, read late from the staging buffer.  (A shorter special case for "no extras" --
+            // [n | wo | 0 0] as one 4-column store, ~30 instructions fewer per query -- measured 5 us SLOWER on config 1: this kernel
+            // is bound by how its dependent chains interleave, not by its instruction count.)
             float v[24];
 #pragma unroll
             for (int k = 0; k < 24; ++k) v[k] = 0.0f;
@@ -230,15 +243,24 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
                 tmem_st4(aA + 4 * (c0 + 2), pack_half2(v[16], v[17]), pack_half2(v[18], v[19]), pack_half2(v[20], v[21]), pack_half2(v[22], v[23]));
         }
         if (tile + tile_stride < n_tiles) prefetch(tile + tile_stride);
+#ifdef OO_PROFILE_PHASES
+        const long long t1 = clock64();
+#endif
         // ------------------------------------------------------------------ hidden layers
         uint32_t w_off = 0;
         for (uint32_t layer = 0; layer < M.n_hidden; ++layer) {
             const uint32_t kt_n = (layer == 0 ? M.k1 : 64u) >> 4;
             const bool second = KS && layer == 0;         // layer 0's inputs 64.. : 4 K-steps further into W0, accumulating
             const bool odd = layer & 1u;
+#ifdef OO_PROFILE_PHASES
+            const long long tb0 = clock64();
+#endif
             tmem_wait_st();              // my row of A is in TMEM
             fence_before_sync();
             named_bar(1 + wg, 128);
+#ifdef OO_PROFILE_PHASES
+            tb += clock64() - tb0;
+#endif
             if (leader_warp) {
                 if (!w_ready) {
                     mbar_wait(bar_w, 0);      // weight image in shared memory (first MMA of this warpgroup only)
@@ -249,7 +271,13 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
                                  2048 >> 4, idesc_h, second ? kt_n - 4u : kt_n, bar, second ? 1u : 0u);
             }
             w_off += kt_n * 2 * 1024;
+#ifdef OO_PROFILE_PHASES
+            const long long tw0 = clock64();
+#endif
             mbar_wait(bar, phase);
+#ifdef OO_PROFILE_PHASES
+            tw += clock64() - tw0;
+#endif
             phase ^= 1;
             fence_after_sync();
             // epilogue: my row of D -> ReLU -> fp16 -> my row of the next layer's A (over columns of D already read)
@@ -287,20 +315,48 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
         fence_after_sync();
         // the output MMA is N = 16 wide: columns 0..3 always, 4..7 (into the same registers) only for out_dim > 4
         const uint32_t o_addr = tmem_lane + (odd ? 32u : 0u);
-        for (uint32_t c0 = 0; c0 < M.out_dim; c0 += 4) {
-            uint32_t o[4];
-            tmem_ld4(o_addr + c0, o);
-            tmem_wait_ld();
+        uint32_t o[4];
+        tmem_ld4(o_addr, o);
+        tmem_wait_ld();
+        if (M.out_dim == 3 && M.out_act == OO_ACT_EXP) {       // RGB through exp: the case every BASELINE.json config runs
+            if (valid) {
+                float* dst = rgb + (size_t)qi * 3;
+                dst[0] = fast_exp(__uint_as_float(o[0]));
+                dst[1] = fast_exp(__uint_as_float(o[1]));
+                dst[2] = fast_exp(__uint_as_float(o[2]));
+            }
+        } else {
             if (valid) {
 #pragma unroll
                 for (uint32_t c = 0; c < 4; ++c)
-                    if (c0 + c < M.out_dim) {
+                    if (c < M.out_dim) {
                         const float z = __uint_as_float(o[c]);
-                        rgb[(size_t)qi * M.out_dim + c0 + c] = M.out_act == OO_ACT_EXP ? fast_exp(z) : z;
+                        rgb[(size_t)qi * M.out_dim + c] = M.out_act == OO_ACT_EXP ? fast_exp(z) : z;
                     }
             }
+            if (M.out_dim > 4) {
+                tmem_ld4(o_addr + 4, o);
+                tmem_wait_ld();
+                if (valid) {
+#pragma unroll
+                    for (uint32_t c = 0; c < 4; ++c)
+                        if (4 + c < M.out_dim) {
+                            const float z = __uint_as_float(o[c]);
+                            rgb[(size_t)qi * M.out_dim + 4 + c] = M.out_act == OO_ACT_EXP ? fast_exp(z) : z;
+                        }
+                }
+            }
         }
+#ifdef OO_PROFILE_PHASES
+        const long long t2 = clock64();
+        t_q += t0b - t0; t_gather += t1 - t0b; t_mlp += t2 - t1; t_wait += tw; t_bar += tb; ++n_done;
+#endif
     }
+#ifdef OO_PROFILE_PHASES
+    if (blockIdx.x == 3 && (threadIdx.x & 31) == 0 && n_done)
+        printf("wg %u warp %u tiles %d total %lld qwait %lld gather %lld mlp %lld (mma-wait %lld, bar %lld) cycles per tile\n", wg, warp & 3, n_done,
+               (clock64() - t_begin) / n_done, t_q / n_done, t_gather / n_done, t_mlp / n_done, t_wait / n_done, t_bar / n_done);
+#endif
     asm volatile("cp.async.wait_group 0;" ::: "memory");
     fence_before_sync();
     __syncthreads();

@@ -16,8 +16,14 @@ namespace oo {
 // (R+2) x (R+2) texels, the one-texel border pre-filled by the octahedral wrap, so the four bilinear taps of any
 // base texel (i0, j0) in [-1, R-1]^2 are plain neighbours and the hot loop has no wrap logic.  `atlas` is pre-offset by
 // one row and one texel, so tap (i0, j0) is at  atlas + slot*map_bytes + (j0*Rp + i0)*texel_bytes  for i0, j0 >= -1.
+// In front of slot 0 lies one all-zero map, "slot -1": a query whose cell is absent at this level (A17) gathers from it with
+// the ordinary weights and gets exact zeros, so the specialised gather has no `slot >= 0` test, no clamp and no weight masks.
+// `atlas_z` is the start of that zero map and addresses are formed in 16-byte units from it (32 bits reach 64 GB per level):
+//   unit index = (slot + 1) * map16 + ((j0*Rp + i0) * texel16 + tap16),   address = atlas_z + 16 * unit index
+// with tap16 = (Rp + 1) * texel16 the unit of tap (0, 0) inside a map; the second tap row is rb16 = Rp * texel16 units further.
 struct LevelParams {
     const uint8_t* atlas;
+    const uint8_t* atlas_z; // texel maps: start of the zero map in front of slot 0 (see above); vertex maps: nullptr
     const int32_t* hop;     // hop table from the previous station: [n_prev][8^gap] -> slot at this depth (-1 = absent)
     float half_r;           // R/2
     float off;              // R/2 - 1/2
@@ -30,7 +36,9 @@ struct LevelParams {
     uint32_t dense;         // 1: slot = dense table lookup (depth <= 4); 0: hop from the previous station
     uint32_t dense_off;     // offset (ints) of this level's dense table inside the dense block
     uint32_t gap;           // depth - previous station depth (1..3) when !dense
-    uint32_t pad_;
+    uint32_t map16;         // map_bytes / 16
+    uint32_t tap16;         // (Rp + 1) * texel_bytes / 16
+    float rp_f;             // Rp as fp32: (j0*Rp + i0) is formed in fp32 (exact: |value| < 2^24) and converted once
 };
 
 struct TreeParams {

@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(256) encode_fast_kernel(const __grid_constant_
             }
             if (O.features) {
                 float h[F];
-                gather_level<F, F32>(lv, e.slot[l], tp, h);
+                gather_level<F, F32>(lv, e.slot[l], e.uv, h);
                 uint8_t* dst = (uint8_t*)O.features + (oi * L + l) * TB;
                 if constexpr (F32) {
 #pragma unroll
@@ -317,9 +317,8 @@ __global__ void __launch_bounds__(kFusedThreads, 2) fused_mma_kernel(const __gri
 #pragma unroll
         for (int l = 0; l < L; ++l) {
             const LevelParams& lv = T.lv[l];
-            const Tap tp = level_tap(e.uv, lv.half_r, lv.off);
             float h[F];
-            gather_level<F, F32>(lv, e.slot[l], tp, h, dbg, l);
+            gather_level<F, F32>(lv, e.slot[l], e.uv, h, dbg, l);
 #pragma unroll
             for (int v = 0; v < F / 8 + (F % 8 ? 1 : 0); ++v) {
                 if constexpr (F % 8 == 0) {
