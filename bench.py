@@ -362,7 +362,13 @@ def run_ours(args):
         torch.cuda.synchronize(dev)
         return [a.elapsed_time(b) for a, b in evs]
 
+    encode_only = args.phase == "encode"
+    feat = torch.empty((n_mine, len(w.tree.level_depth) * w.atlas.F), dtype=torch.float16, device=dev) if encode_only else None
+
     def step():
+        if encode_only:   # the encoding phase alone (a2-a6): features round-trip HBM; side measurement, the ncu target of north_star's "encoding phase"
+            ctx.oo_encode(x, wo, features=feat)
+            return
         ctx.oo_query(x, nrm, wo, ex, rgb=rgb)
         if strong:        # the path's one optional exchange: every rank ends the step with the whole frame (NCCL all-gather)
             frame[0] = D.all_gather_rows(rgb, n_frame)
@@ -383,11 +389,25 @@ def run_ours(args):
     if sampler and (t1 - t0) < 0.5 and not args.quick:
         tend = time.time() + 0.5
         while time.time() < tend:
-            ctx.oo_query(x, nrm, wo, ex, rgb=rgb)
+            step() if encode_only else ctx.oo_query(x, nrm, wo, ex, rgb=rgb)
         torch.cuda.synchronize(dev)
         t1 = time.time()
     clocks = sampler.stop(t0, t1) if sampler else None
     ms_warm = timed(min(args.steps, 50), False, step) if not args.quick else ms
+    if encode_only:
+        mean_ms, warm_ms = sum(ms) / len(ms), sum(ms_warm) / len(ms_warm)
+        hbm, tf, which = peaks()
+        L, F = len(w.tree.level_depth), w.atlas.F
+        bq = desc["gather_bytes_per_query"] + 24 + L * F * 2        # x, wo in; fp16 feature row out
+        info = ctx.oo_get_info()
+        print(json.dumps({"metric": "encode-only query throughput (a2-a6, features to HBM)", "value": n_mine / (mean_ms * 1e-3) / 1e6, "unit": UNIT,
+                          "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": mean_ms, "ms_per_step_warm_l2": warm_ms,
+                          "config": desc, "run": {"presort": args.presort, "presorted": bool(info["presorted_last_encode"]), "l2": "flushed between steps",
+                                                  "path": PATH_NAMES[info["path_last_encode"]]},
+                          "clocks": clocks, "gpu_launches": int(launches), "dtype": "f16", "data": "synthetic",
+                          "roofline": {"bound": "hbm", "achieved": bq * n_mine / (mean_ms * 1e-3) / 1e9, "peak": hbm, "unit": "GB/s",
+                                       "frac": bq * n_mine / (mean_ms * 1e-3) / 1e9 / hbm, "bytes_per_query": bq, "peak_source": which}}))
+        return 0
     checksum_dev = float((frame[0] if strong else rgb).double().sum())
     # e2e: pinned host buffers, H2D + kernels + D2H inside the timed region, through oo_query_host
     pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a[lo:hi])).pin_memory()
@@ -600,8 +620,13 @@ def run_sweep(args):
         feat = torch.empty((n_max, L * F), dtype=torch.float16, device=dev)
         rgb = torch.empty((n_max, 3), dtype=torch.float32, device=dev)
         perm = torch.empty(n_max, dtype=torch.int32, device=dev)
+        floor = {}
         for dname, q in dists.items():
             X, Nn, W = cu(q.x), cu(q.nrm), cu(q.wo)
+            # the latency floor of a call: ONE 128-query tile (launch + prologue + one descent/gather chain + the decoder's MMA
+            # round trips, cold L2); no batch, however small, finishes sooner, so small batches are judged against it
+            floor[dname] = {"fused_one_tile_ms": timed(lambda: ctx.oo_query(X[:128], Nn[:128], W[:128], rgb=rgb[:128]), 20),
+                            "encode_one_tile_ms": timed(lambda: ctx.oo_encode(X[:128], W[:128], features=feat[:128]), 20)}
             for lg in range(args.sweep_min_log2, args.sweep_max_log2 + 1):
                 n = 1 << lg
                 x, nrm, wo = X[:n], Nn[:n], W[:n]
@@ -635,7 +660,7 @@ def run_sweep(args):
                 rows.append(row)
         out = {"sweep": "BASELINE.json configs[4]: batch size x query distribution on the config-3 tree and MLP",
                "tree_nodes": w.tree.n_nodes, "atlas_bytes": w.atlas.nbytes, "bytes_per_query": {"fused": bq_fused, "encode": bq_enc},
-               "rows": rows}
+               "latency_floor": floor, "rows": rows}
     out.update({"unit": UNIT, "l2": "flushed between launches (256 MB memset)", "timing": "median of CUDA-event times",
                 "peak_gbs": hbm, "peak_source": which, "data": "synthetic"})
     print(json.dumps(out))
@@ -836,6 +861,7 @@ def main():
     ap.add_argument("--sweep-dist", default="both", choices=["both", "coherent", "incoherent"])
     ap.add_argument("--presort", default="auto", choices=["auto", "none", "bin"], help="oo_set_presort for the run (default: the library's own default, auto)")
     ap.add_argument("--quick", action="store_true", help="timed region only (no warm-L2 / e2e / CPU legs): the command ncu wraps")
+    ap.add_argument("--phase", default="fused", choices=["fused", "encode"], help="fused = the whole hot path (the headline); encode = oo_encode alone (a2-a6), a side measurement and the ncu target for the encoding phase")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"], help="N > 1: every rank its own frame (weak) or one frame split across ranks + RGB all-gather (strong)")
     ap.add_argument("--dry-run-dist", action="store_true", help="the N > 1 host logic on CPU with gloo (launcher, sharding, gather, reductions): what the CPU tests drive; measures nothing")
     ap.add_argument("--ingest-ncu", default=None, help="ncu --csv launch list to store in profiles/traffic.json for --config (see ingest_ncu)")

@@ -283,15 +283,17 @@ def tie_vertex_map_borders(a: np.ndarray) -> np.ndarray:
     return a
 
 
-def make_vertex_atlas(tree: Tree, F: int, dtype: str, seed: int, std: float = 0.1) -> Atlas:
+def make_vertex_atlas(tree: Tree, F: int, dtype: str, seed: int, std: float = 0.1, tie: bool = True) -> Atlas:
     """Vertex-stored maps (PAPER.md "features are stored at map vertices", vertex resolution n_l + 1 with n_l =
     tree.level_res[l] intervals per axis): per used level [slots][n+1][n+1][F], same value distributions as make_atlas,
-    boundary vertices tied (tie_vertex_map_borders)."""
+    boundary vertices tied (tie_vertex_map_borders) unless tie=False (a cache whose owner stored the coinciding vertices
+    independently: what the library's upload has to repair)."""
     out = []
     for l, (R, S) in enumerate(zip(tree.level_res, tree.level_slots)):
         n = S * (R + 1) * (R + 1) * F
         a = normal_f16(seed, STREAM_ATLAS + l, n, std) if dtype == "f16" else uniform_f32(seed, STREAM_ATLAS + l, n, -1.0, 1.0)
-        out.append(tie_vertex_map_borders(a.reshape(S, R + 1, R + 1, F)))
+        a = a.reshape(S, R + 1, R + 1, F)
+        out.append(tie_vertex_map_borders(a) if tie else a)
     return Atlas(F, dtype, out)
 
 

@@ -78,8 +78,12 @@ typedef enum { OO_SPATIAL_NEAREST = 0, OO_SPATIAL_TRILINEAR8 = 1 } oo_spatial;
  * grid with R intervals per axis; the lookup finds the grid cell (ci, cj) = min(floor((u+1)/2*R), R-1), splits it along
  * the anti-diagonal where u_x*u_y > 0 (cell in a same-sign quadrant) and along the main diagonal otherwise, so that the
  * hypotenuses run parallel to the octahedron's face edges, and takes the barycentric combination of the containing
- * triangle's three vertices.  Boundary vertices that coincide on the sphere are stored separately; the library reads
- * them as given (tying them is the owner's concern). */
+ * triangle's three vertices.  Boundary vertices that coincide on the sphere ("the edge vertices are shared along adjacent
+ * faces", Fig. 3 caption / P:125) are stored separately in the caller's arrays: (0, c) and (0, R-c), (R, c) and (R, R-c),
+ * (r, 0) and (R-r, 0), (r, R) and (R-r, R) are one vertex each, the four corners are all the -z pole.  oo_upload_tree TIES
+ * them in the library's copy: each pair takes the value of the member with the smaller index along its side, the corners
+ * that of vertex (0, 0), so the interpolant is continuous across the seam whatever was stored (a cache whose owner shares
+ * them already is unchanged).  oo_info.tied_vertices counts the stored vertices the last upload rewrote. */
 typedef enum { OO_DIRMAP_TEXEL = 0, OO_DIRMAP_VERTEX = 1 } oo_dirmap;
 /* f3, P:135 and Eq. 8-9: the direction that indexes the maps.  WO: wo itself.  MIRROR: w_r = 2(n.wo)n - wo.
  * SHIFTED: per cell j with centre c_j, w~_j = (x - c_j)*d^ + w_r (Eq. 9 before normalisation; Eq. 4 is scale invariant),
@@ -214,6 +218,8 @@ typedef struct {
     uint32_t full_query;         /* 1 if oo_query runs the full-query kernel under the current tree / mode / decoder
                                     (mode != 0, vertex maps or width 128), i.e. oo_query_debug's outputs are [n][L][J]... */
     uint32_t n_neighbours;       /* J of the current mode: 8 (OO_SPATIAL_TRILINEAR8) or 1 */
+    uint64_t tied_vertices;      /* OO_DIRMAP_VERTEX: boundary vertices the last oo_upload_tree rewrote when it tied the seam (0 for
+                                    a cache stored with shared edge vertices, and for texel maps) */
     uint32_t presort_auto_on;    /* OO_PRESORT_AUTO's current decision: 1 = the next batch of >= min_queries queries is binned */
     uint32_t coherence_x100;     /* 100 x mean number of distinct depth-4 cells per 32 consecutive queries, latest sample */
 } oo_info;
@@ -290,8 +296,8 @@ OO_API oo_status oo_query(oo_ctx* ctx, const oo_queries* q, float* d_rgb, void* 
 OO_API oo_status oo_query_debug(oo_ctx* ctx, const oo_queries* q, float* d_rgb, int32_t* d_slot, int16_t* d_index,
                          void* cuda_stream);
 
-/* Number of chunks oo_query_host splits a batch into: 1..16, or 0 (default) = chosen from the batch size (one chunk
- * below 131,072 queries, else about 262,144 queries per chunk, 2..8 chunks). */
+/* Number of (equal) chunks oo_query_host splits a batch into: 1..16, or 0 (default) = chosen from the batch size (one
+ * chunk below 131,072 queries, else about 262,144 queries per chunk, 2..8 chunks). */
 OO_API oo_status oo_set_host_chunks(oo_ctx* ctx, uint32_t n_chunks);
 
 /* The whole path from HOST buffers, as a chunked three-stage pipeline: the queries are split into chunks of whole

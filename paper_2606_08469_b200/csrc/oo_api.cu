@@ -423,6 +423,11 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
     c->atlas_dev.assign(L, nullptr);
     uint64_t atlas_bytes = 0;
     int launches = 0;
+    unsigned long long* d_changed = nullptr;      // vertex maps: number of boundary vertices the tying rewrote
+    if (vertex) {
+        OO_CUDA(c, cudaMalloc((void**)&d_changed, sizeof(unsigned long long)));
+        OO_CUDA(c, cudaMemsetAsync(d_changed, 0, sizeof(unsigned long long), stream));
+    }
     for (uint32_t l = 0; l < L; ++l) {
         // texel maps: (R+2)^2 with the wrapped border; vertex maps: the (R+1)^2 vertices as given
         const uint32_t R = t->level_res[l], Rp = vertex ? R + 1 : R + 2;
@@ -436,8 +441,10 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
         uint8_t* slot0 = (uint8_t*)c->atlas_dev[l] + lead;
         if (lead) OO_CUDA(c, cudaMemsetAsync(c->atlas_dev[l], 0, lead, stream));
         if (t->level_slots[l] == 0) OO_CUDA(c, cudaMemsetAsync(slot0, 0, slots * map_bytes, stream));
-        else if (vertex) OO_CUDA(c, cudaMemcpyAsync(slot0, t->atlas[l], slots * map_bytes, cudaMemcpyDeviceToDevice, stream));
-        else launches += launch_pad_atlas(t->atlas[l], slot0, t->level_slots[l], R, texel_bytes, stream);
+        else if (vertex) {
+            OO_CUDA(c, cudaMemcpyAsync(slot0, t->atlas[l], slots * map_bytes, cudaMemcpyDeviceToDevice, stream));
+            launches += launch_tie_vertex_borders(slot0, t->level_slots[l], R, texel_bytes, d_changed, stream);      // f2: P:125
+        } else launches += launch_pad_atlas(t->atlas[l], slot0, t->level_slots[l], R, texel_bytes, stream);
         LevelParams& lv = T.lv[l];
         lv.atlas = slot0 + (vertex ? 0 : (uint64_t)(Rp + 1) * texel_bytes);
         lv.atlas_z = vertex ? nullptr : (const uint8_t*)c->atlas_dev[l];
@@ -566,6 +573,15 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
     }
     c->info.node_table_bytes = table_bytes;
     c->info.launches += (uint64_t)launches;
+    c->info.tied_vertices = 0;
+    if (d_changed) {
+        unsigned long long h = 0;
+        const cudaError_t e = cudaMemcpyAsync(&h, d_changed, sizeof h, cudaMemcpyDeviceToHost, stream);
+        const cudaError_t e2 = e == cudaSuccess ? cudaStreamSynchronize(stream) : e;
+        cudaFree(d_changed);
+        OO_CUDA(c, e2);
+        c->info.tied_vertices = h;
+    }
     OO_CUDA(c, cudaStreamSynchronize(stream));
     OO_CUDA(c, cudaGetLastError());
     c->T = T;
@@ -1156,16 +1172,27 @@ extern "C" OO_API oo_status oo_query_host(oo_ctx* c, const oo_queries* q, float*
     }
     // Chunked three-stage pipeline: copy-in of chunk i+1 (s_h2d) overlaps the kernel of chunk i (caller's stream) and the
     // copy-out of chunk i-1 (s_d2h); PCIe is full duplex, so a frame costs about its copy-in time instead of the sum of the three.
-    // Chunks are whole multiples of 128-query tiles.  The exposed tail is the LAST chunk's kernel + copy-out and the exposed head
-    // the FIRST chunk's copy-in, so the chunk count follows the batch size (oo_set_host_chunks overrides): about 256 Ki queries per
-    // chunk, at least 2 and at most 8 chunks from 128 Ki queries on, one chunk below that.
-    // Measured on B200 (config 1, pinned buffers): 1 chunk 1.07-1.10 ms, 2: 0.99, 4: 0.98, 8: 1.01-1.03, 16: 1.15 ms.
+    // Chunks are whole multiples of 128-query tiles, all of one size.  The chunk count follows the batch size (oo_set_host_chunks
+    // overrides): one chunk below 128 Ki queries, else about 256 Ki queries per chunk, at least 2 and at most 8 chunks.
+    // Measured on B200 (config 1 = 2^20 queries, pinned buffers): 1 chunk 1.07-1.10 ms, 2: 0.99, 4: 0.93-0.98, 8: 1.01-1.03, 16: 1.15 ms;
+    // five chunks with a half-length first and last one (to shorten the exposed head and tail) 1.09 ms: every chunk costs three
+    // host-to-device copies whose fixed cost outweighs what a shorter head saves.  The floor is the 37.7 MB copy-in at the
+    // measured 54.8 GB/s = 0.69 ms.
     const uint64_t n = q->n;
     int want = c->host_chunks;
     if (want <= 0) want = n < (1u << 17) ? 1 : (int)std::min<uint64_t>(8, std::max<uint64_t>(2, n >> 18));
-    uint64_t chunk = (n + want - 1) / want;
-    chunk = (chunk + 127) & ~127ull;
-    const int n_chunks = (int)((n + chunk - 1) / chunk);
+    uint64_t bounds[oo_ctx::kMaxChunks + 1];
+    int n_chunks = 0;
+    {
+        uint64_t unit = (n + want - 1) / want;
+        unit = (unit + 127) & ~127ull;
+        bounds[0] = 0;
+        for (int i = 0; i < want && bounds[n_chunks] < n; ++i) {
+            bounds[n_chunks + 1] = std::min(n, bounds[n_chunks] + unit);
+            ++n_chunks;
+        }
+        bounds[n_chunks] = n;
+    }
     const uint32_t od = c->M.out_dim;
     // any failure below leaves copies from / to the caller's host buffers in flight on the library's streams: drain all three
     // before returning, so that the caller may free or reuse its buffers whatever the status
@@ -1186,7 +1213,7 @@ extern "C" OO_API oo_status oo_query_host(oo_ctx* c, const oo_queries* q, float*
     OO_PIPE(cudaStreamWaitEvent(c->s_h2d, c->ev_start, 0));
     OO_PIPE(cudaStreamWaitEvent(c->s_d2h, c->ev_start, 0));
     for (int i = 0; i < n_chunks; ++i) {
-        const uint64_t o = (uint64_t)i * chunk, m = std::min(chunk, n - o);
+        const uint64_t o = bounds[i], m = bounds[i + 1] - o;
         OO_PIPE(cudaMemcpyAsync(c->d_qx + o * 3, q->x + o * 3, m * 12, cudaMemcpyHostToDevice, c->s_h2d));
         OO_PIPE(cudaMemcpyAsync(c->d_qn + o * 3, q->nrm + o * 3, m * 12, cudaMemcpyHostToDevice, c->s_h2d));
         OO_PIPE(cudaMemcpyAsync(c->d_qw + o * 3, q->wo + o * 3, m * 12, cudaMemcpyHostToDevice, c->s_h2d));

@@ -145,6 +145,7 @@ inline bool opt_in_smem(std::atomic<uint64_t>& mask, const void* kernel, int byt
 // Launchers (oo_kernels.cu / oo_sort.cu).  Each returns the number of kernels it launched, -1 if the requested
 // specialisation does not exist, or kLaunchCudaError if a CUDA call made on the way failed.  All launches go to `stream`.
 int launch_pad_atlas(const void* src, void* dst, uint64_t slots, uint32_t R, uint32_t texel_bytes, cudaStream_t stream);
+int launch_tie_vertex_borders(void* maps, uint64_t slots, uint32_t R, uint32_t texel_bytes, unsigned long long* changed, cudaStream_t stream);
 int launch_encode_generic(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, uint32_t tree_max_depth,
                           cudaStream_t stream);
 int launch_encode_fast(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, int n_sms, cudaStream_t stream);

@@ -38,6 +38,52 @@ int launch_pad_atlas(const void* src, void* dst, uint64_t slots, uint32_t R, uin
 }
 
 // =====================================================================================================================
+// Upload-time tying of vertex-stored maps (f2, P:125 / Fig. 3 caption: "the edge vertices are shared along adjacent faces").
+// On the unfolded octahedron the outer edge of the (R+1) x (R+1) vertex grid is the four lower-hemisphere face edges met
+// twice, mirrored about each side's midpoint, and the four corners are all the -z pole: stored vertices (0, c) and (0, R-c),
+// (R, c) and (R, R-c), (r, 0) and (R-r, 0), (r, R) and (R-r, R) are one vertex each.  The library's copy gives every such
+// pair the value of the member with the smaller index along its side (the corners that of vertex (0, 0)), so that the
+// barycentric interpolant is continuous across the seam whatever the owner stored; *changed counts the vertices rewritten.
+// One thread per boundary vertex of one map.
+// =====================================================================================================================
+__global__ void tie_vertex_borders_kernel(uint4* __restrict__ maps, uint64_t slots, uint32_t R, uint32_t vec_per_texel,
+                                          unsigned long long* __restrict__ changed) {
+    const uint32_t n = R, Rp = R + 1;
+    const uint64_t total = slots * 4ull * n;
+    for (uint64_t t = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; t < total; t += (uint64_t)gridDim.x * blockDim.x) {
+        const uint64_t slot = t / (4ull * n);
+        const uint32_t b = (uint32_t)(t - slot * 4ull * n), e = b / n, i = b - e * n;
+        // the 4n boundary vertices, each once: side 0 (0, i), side 1 (i, n), side 2 (n, n - i), side 3 (n - i, 0), i = 0..n-1
+        const uint32_t r = e == 0 ? 0u : e == 1 ? i : e == 2 ? n : n - i;
+        const uint32_t c = e == 0 ? i : e == 1 ? n : e == 2 ? n - i : 0u;
+        uint32_t sr = r, sc = c;
+        const bool corner = (r == 0 || r == n) && (c == 0 || c == n);
+        if (corner) { sr = 0; sc = 0; }
+        else if ((r == 0 || r == n) && 2 * c > n) sc = n - c;
+        else if ((c == 0 || c == n) && 2 * r > n) sr = n - r;
+        if (sr == r && sc == c) continue;
+        uint4* dst = maps + ((slot * Rp + r) * Rp + c) * vec_per_texel;
+        const uint4* src = maps + ((slot * Rp + sr) * Rp + sc) * vec_per_texel;
+        bool diff = false;
+        for (uint32_t v = 0; v < vec_per_texel; ++v) {
+            const uint4 a = src[v], o = dst[v];
+            diff |= (a.x != o.x) | (a.y != o.y) | (a.z != o.z) | (a.w != o.w);
+            dst[v] = a;
+        }
+        if (diff) atomicAdd(changed, 1ull);
+    }
+}
+
+int launch_tie_vertex_borders(void* maps, uint64_t slots, uint32_t R, uint32_t texel_bytes, unsigned long long* changed, cudaStream_t stream) {
+    if (slots == 0) return 0;
+    const uint64_t total = slots * 4ull * R;
+    const uint64_t blocks = (total + 255) / 256;
+    const unsigned grid = (unsigned)(blocks < 148ull * 32 ? blocks : 148ull * 32);
+    tie_vertex_borders_kernel<<<grid, 256, 0, stream>>>((uint4*)maps, slots, R, texel_bytes / 16, changed);
+    return 1;
+}
+
+// =====================================================================================================================
 // Generic encode: any tree, any (F, dtype) with 16/32/64-byte texels.  Plain child-table descent per level.
 // One thread per query.  Slow by design; it is the fallback and a cross-check of the specialised kernels.
 // =====================================================================================================================

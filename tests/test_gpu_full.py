@@ -232,6 +232,37 @@ def test_all_neighbours_empty_gives_the_attribute_only_answer(P):
     _check(P, t2, atlas, "f32", mlp, q, mode, d)
 
 
+def test_vertex_map_seam_is_tied_at_upload(P):
+    """f2, P:125 ("the edge vertices are shared along adjacent faces"): a cache that stores the coinciding boundary vertices
+    independently is repaired by oo_upload_tree -- the library's copy equals the tied maps, so the query matches the oracle run
+    on the tied maps (and differs from the oracle on the untied ones); an already tied cache is left as it is."""
+    w = gen.scene_workload(1, width=96, height=64, max_depth=6)
+    q = w.queries
+    q.wo[:64] = np.array([[0.3, -0.2, -1.0], [-0.7, 0.1, -0.05], [0.0, 0.0, -1.0], [1.0, 1.0, -1e-3]], np.float32).repeat(16, 0)   # around the seam
+    mode = FO.Mode(spatial="trilinear8", dirmap="vertex")
+    mlp = gen.make_mlp(24 + 6, 2, 0)
+    untied = gen.make_vertex_atlas(w.tree, 8, "f16", 0, tie=False).levels
+    tied = [gen.tie_vertex_map_borders(a.copy()) for a in untied]
+    assert any(not np.array_equal(a, b) for a, b in zip(untied, tied))
+    ref = FO.query_full(w.tree, tied, mlp.weights, q.x, q.nrm, q.wo, None, mlp.out_act, mode, None)
+    ref_untied = FO.query_full(w.tree, untied, mlp.weights, q.x, q.nrm, q.wo, None, mlp.out_act, mode, None)
+    assert np.abs(ref - ref_untied).max() > 1e-2                     # the seam matters for these directions
+    ctx = P.OctaOctree(0)
+    ctx.oo_upload_tree(w.tree, untied, "f16", dirmap="vertex")
+    n_boundary = sum(S * 4 * R for S, R in zip(w.tree.level_slots, w.tree.level_res))
+    changed = ctx.oo_get_info()["tied_vertices"]
+    assert 0 < changed <= n_boundary // 2 + 3 * sum(w.tree.level_slots), (changed, n_boundary)
+    ctx.oo_upload_mlp(mlp.weights, mlp.out_act)
+    ctx.oo_set_mode(mode.spatial, mode.lookup, mode.attrs)
+    got = ctx.oo_query(_cu(q.x), _cu(q.nrm), _cu(q.wo)).cpu().numpy()
+    check_rgb(got, ref)
+    ctx.oo_upload_tree(w.tree, tied, "f16", dirmap="vertex")
+    assert ctx.oo_get_info()["tied_vertices"] == 0
+    assert np.array_equal(ctx.oo_query(_cu(q.x), _cu(q.nrm), _cu(q.wo)).cpu().numpy(), got)
+    ctx.oo_upload_tree(w.tree, w.atlas.levels, "f16")                # texel maps: nothing to tie
+    assert ctx.oo_get_info()["tied_vertices"] == 0
+
+
 def test_full_query_argument_errors(P):
     w = gen.config0(n=64)
     ctx = P.OctaOctree(0).upload_workload(w)

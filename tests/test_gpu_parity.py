@@ -385,7 +385,7 @@ def test_query_host_equals_query(P):
 def test_query_host_pipeline_many_chunks(P):
     """oo_query_host splits the frame into chunks that overlap copy-in, kernel and copy-out: several chunks with a ragged
     last one must give the same bytes as one device-side oo_query, with and without extras, called twice in a row."""
-    w = gen.scene_workload(2, width=640, height=333)          # 213,120 queries: 2 chunks by default, 4 or 16 on request
+    w = gen.scene_workload(2, width=640, height=333)          # 213,120 queries: 2 chunks by default, 1..16 on request
     q = w.queries
     ctx = P.OctaOctree(0).upload_workload(w)
     ctx.oo_reserve(q.n)
@@ -393,7 +393,7 @@ def test_query_host_pipeline_many_chunks(P):
     dev = ctx.oo_query(x, n, wo, ex).cpu().numpy()
     pin = lambda a: torch.from_numpy(a).pin_memory()
     hx, hn, hw, he = pin(q.x), pin(q.nrm), pin(q.wo), pin(q.extra)
-    for want, chunks in ((0, 2), (4, 4), (16, 16), (1, 1)):
+    for want, chunks in ((0, 2), (4, 4), (16, 16), (3, 3), (1, 1)):
         ctx.oo_set_host_chunks(want)
         l0 = ctx.oo_get_info()["query_launches"]
         for _ in range(2):
