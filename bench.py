@@ -425,6 +425,18 @@ def run_ours(args):
     torch.cuda.synchronize(dev)
     e2e_ms = sum(e2e_times) / len(e2e_times)
     checksum = float(hrgb.double().sum())
+    e2e_zero_copy = bool(ctx.oo_get_info()["host_zero_copy_last"])
+    pipeline_ms = None
+    if e2e_zero_copy and not args.quick:           # for comparison: the same call through the chunked copy pipeline
+        ctx.oo_set_host_zero_copy(False)
+        ctx.oo_query_host(hx, hn, hw, he, rgb=hrgb)
+        tt = []
+        for _ in range(5):
+            te = time.perf_counter()
+            ctx.oo_query_host(hx, hn, hw, he, rgb=hrgb)
+            tt.append((time.perf_counter() - te) * 1e3)
+        pipeline_ms = sum(tt) / len(tt)
+        ctx.oo_set_host_zero_copy(True)
     # measured copy rates of this box (one 64 MB pinned copy each way), so that the PCIe floor of e2e is a measured number
     h2d_gbs = d2h_gbs = None
     if not args.quick and rank == 0:
@@ -495,7 +507,9 @@ def run_ours(args):
         "clocks": clocks,
         "e2e": {"value": tot_q / (mx_e2e * 1e-3) / 1e6, "unit": UNIT, "h2d_bytes_per_step": int((36 + 4 * ne) * n_mine),
                 "d2h_bytes_per_step": int(12 * n_mine), "ms_per_step": mx_e2e, "ms_min": min(e2e_times), "ms_max": max(e2e_times),
-                "api": "oo_query_host (pinned host buffers)", "checksum": chk_sum if not strong else checksum,
+                "api": "oo_query_host (pinned host buffers)" + (": one launch reads the queries from host memory in place and writes the RGB back (zero-copy)" if e2e_zero_copy
+                                                                  else ": chunked copy-in / kernel / copy-out pipeline"),
+                "copy_pipeline_ms": pipeline_ms, "checksum": chk_sum if not strong else checksum,
                 "h2d_GBps_measured": h2d_gbs, "d2h_GBps_measured": d2h_gbs,
                 "pcie_floor_ms": None if not h2d_gbs else (36 + 4 * ne) * n_mine / (h2d_gbs * 1e9) * 1e3},
         "gpu_launches": int(launches),

@@ -220,6 +220,7 @@ typedef struct {
     uint32_t n_neighbours;       /* J of the current mode: 8 (OO_SPATIAL_TRILINEAR8) or 1 */
     uint64_t tied_vertices;      /* OO_DIRMAP_VERTEX: boundary vertices the last oo_upload_tree rewrote when it tied the seam (0 for
                                     a cache stored with shared edge vertices, and for texel maps) */
+    uint32_t host_zero_copy_last; /* 1 if the last oo_query_host read its (pinned) host buffers in place, 0 if it ran the copy pipeline */
     uint32_t presort_auto_on;    /* OO_PRESORT_AUTO's current decision: 1 = the next batch of >= min_queries queries is binned */
     uint32_t coherence_x100;     /* 100 x mean number of distinct depth-4 cells per 32 consecutive queries, latest sample */
 } oo_info;
@@ -300,7 +301,15 @@ OO_API oo_status oo_query_debug(oo_ctx* ctx, const oo_queries* q, float* d_rgb, 
  * chunk below 131,072 queries, else about 262,144 queries per chunk, 2..8 chunks). */
 OO_API oo_status oo_set_host_chunks(oo_ctx* ctx, uint32_t n_chunks);
 
-/* The whole path from HOST buffers, as a chunked three-stage pipeline: the queries are split into chunks of whole
+/* oo_query_host reads PINNED host buffers in place (see there) when enable != 0 (default); 0 forces the chunked copy pipeline. */
+OO_API oo_status oo_set_host_zero_copy(oo_ctx* ctx, uint32_t enable);
+
+/* The whole path from HOST buffers.  Fast path (default, oo_set_host_zero_copy): when q->x, q->nrm, q->wo, q->extra,
+ * q->disparity and h_rgb are all pinned (page-locked) host memory that the device can address, and the batch is not going to
+ * be binned (oo_presort), ONE launch of the fused kernel reads the queries straight from host memory over PCIe -- the next
+ * tile's queries are prefetched behind the current tile, so the reads stream -- and writes the RGB straight back: no staging
+ * copy, no chunks (oo_info.host_zero_copy_last = 1).  Needs no oo_reserve.  Otherwise (pageable memory, binned batches, or the
+ * fast path switched off) a chunked three-stage pipeline: the queries are split into chunks of whole
  * 128-query tiles (see oo_set_host_chunks); chunk i+1 is copied to the device on a library-owned copy-in
  * stream while oo_query runs chunk i on the caller's stream and chunk i-1's RGB returns to h_rgb (HOST [n][out_dim]) on
  * a library-owned copy-out stream.  Work starts after everything already enqueued on the caller's stream; the call

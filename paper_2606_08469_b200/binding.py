@@ -20,7 +20,7 @@ _STATUS = {0: "OO_OK", 1: "OO_ERR_INVALID_ARG", 2: "OO_ERR_NOT_READY", 3: "OO_ER
 EXPORTED_SYMBOLS = ["oo_create", "oo_destroy", "oo_last_error", "oo_upload_tree", "oo_upload_mlp", "oo_reserve", "oo_set_path",
                     "oo_get_info", "oo_sort_queries", "oo_encode", "oo_query", "oo_query_host", "oo_read_padded_map", "oo_set_mode",
                     "oo_encode_full", "oo_upload_scene", "oo_raycast", "oo_upload_disparity", "oo_predict_disparity", "oo_set_presort",
-                    "oo_query_debug", "oo_set_host_chunks", "oo_last_note"]
+                    "oo_query_debug", "oo_set_host_chunks", "oo_last_note", "oo_set_host_zero_copy"]
 
 
 class OOError(RuntimeError):
@@ -69,7 +69,7 @@ class _Info(C.Structure):
                 ("atlas_bytes", C.c_uint64), ("path_last_query", C.c_uint32), ("path_last_encode", C.c_uint32),
                 ("hop_plan_ok", C.c_uint32), ("n_sms", C.c_uint32),
                 ("presorted_last_query", C.c_uint32), ("presorted_last_encode", C.c_uint32),
-                ("full_query", C.c_uint32), ("n_neighbours", C.c_uint32), ("tied_vertices", C.c_uint64), ("presort_auto_on", C.c_uint32),
+                ("full_query", C.c_uint32), ("n_neighbours", C.c_uint32), ("tied_vertices", C.c_uint64), ("host_zero_copy_last", C.c_uint32), ("presort_auto_on", C.c_uint32),
                 ("coherence_x100", C.c_uint32)]
 
 
@@ -98,6 +98,7 @@ def load_library():
     L.oo_last_note.restype = C.c_char_p
     L.oo_query_debug.argtypes = [vp, C.POINTER(_Queries), vp, vp, vp, vp]
     L.oo_set_host_chunks.argtypes = [vp, u32]
+    L.oo_set_host_zero_copy.argtypes = [vp, u32]
     L.oo_upload_tree.argtypes = [vp, C.POINTER(_TreeDesc), vp]
     L.oo_upload_mlp.argtypes = [vp, C.POINTER(_MlpDesc), vp]
     L.oo_reserve.argtypes = [vp, u64]
@@ -327,6 +328,9 @@ class OctaOctree:
 
     def oo_set_host_chunks(self, n_chunks: int = 0):
         self._check(self._L.oo_set_host_chunks(self._ctx, int(n_chunks)))
+
+    def oo_set_host_zero_copy(self, enable: bool = True):
+        self._check(self._L.oo_set_host_zero_copy(self._ctx, 1 if enable else 0))
 
     def oo_last_note(self) -> str:
         return self._L.oo_last_note(self._ctx).decode()

@@ -376,10 +376,23 @@ def test_query_host_equals_query(P):
     x, n, wo, ex = _dev(q)
     dev = ctx.oo_query(x, n, wo, ex).cpu().numpy()
     pin = lambda a: torch.from_numpy(a).pin_memory()
-    host = ctx.oo_query_host(pin(q.x), pin(q.nrm), pin(q.wo), pin(q.extra))
+    l0 = ctx.oo_get_info()["query_launches"]
+    host = ctx.oo_query_host(pin(q.x), pin(q.nrm), pin(q.wo), pin(q.extra))          # all pinned: one launch reads them in place
+    info = ctx.oo_get_info()
+    assert info["host_zero_copy_last"] == 1 and info["query_launches"] - l0 == 1
     assert np.array_equal(host.numpy(), dev)
-    host2 = ctx.oo_query_host(q.x, q.nrm, q.wo, q.extra, rgb=np.empty((q.n, 3), np.float32))   # pageable numpy
+    host2 = ctx.oo_query_host(q.x, q.nrm, q.wo, q.extra, rgb=np.empty((q.n, 3), np.float32))   # pageable numpy: the copy pipeline
+    assert ctx.oo_get_info()["host_zero_copy_last"] == 0
     assert np.array_equal(host2, dev)
+    ctx.oo_set_host_zero_copy(False)
+    host3 = ctx.oo_query_host(pin(q.x), pin(q.nrm), pin(q.wo), pin(q.extra))
+    assert ctx.oo_get_info()["host_zero_copy_last"] == 0 and np.array_equal(host3.numpy(), dev)
+    # the zero-copy path needs no scratch; the pipeline does
+    ctx2 = P.OctaOctree(0).upload_workload(w)
+    assert np.array_equal(ctx2.oo_query_host(pin(q.x), pin(q.nrm), pin(q.wo), pin(q.extra)).numpy(), dev)
+    with pytest.raises(P.OOError) as e:
+        ctx2.oo_query_host(q.x, q.nrm, q.wo, q.extra, rgb=np.empty((q.n, 3), np.float32))
+    assert e.value.status == 2
 
 
 def test_query_host_pipeline_many_chunks(P):
@@ -393,6 +406,7 @@ def test_query_host_pipeline_many_chunks(P):
     dev = ctx.oo_query(x, n, wo, ex).cpu().numpy()
     pin = lambda a: torch.from_numpy(a).pin_memory()
     hx, hn, hw, he = pin(q.x), pin(q.nrm), pin(q.wo), pin(q.extra)
+    ctx.oo_set_host_zero_copy(False)                          # this test is about the copy pipeline
     for want, chunks in ((0, 2), (4, 4), (16, 16), (3, 3), (1, 1)):
         ctx.oo_set_host_chunks(want)
         l0 = ctx.oo_get_info()["query_launches"]
