@@ -856,6 +856,9 @@ static void collect_samples(oo_ctx* c, cudaStream_t stream) {
         cudaMemcpyAsync(c->h_stat, c->d_stat, kStatSlots * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->s_stat) != cudaSuccess)
         (void)cudaGetLastError();
 }
+// Will this batch's taps miss the caches?  Binned queries do by construction (they are incoherent or they would not have been binned);
+// otherwise the latest coherence sample decides (none taken yet: no).  Chooses between the two encode kernels.
+static bool cache_cold(const oo_ctx* c, bool binned) { return binned || c->coherence > 12.0f; }
 static bool bin_wanted(oo_ctx* c, const oo_queries* q) {
     if (q->perm || q->n < c->bin_min) return false;
     if (c->presort == OO_PRESORT_BIN) return true;
@@ -933,7 +936,7 @@ extern "C" OO_API oo_status oo_encode(oo_ctx* c, const oo_queries* q, void* d_fe
         arm_sampling(c, Q);
     }
     int n = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Q, O, c->tree_max_depth, (cudaStream_t)cuda_stream)
-                                 : launch_encode_fast(c->T, Q, O, c->n_sms, (cudaStream_t)cuda_stream);
+                                 : launch_encode_fast(c->T, Q, O, c->n_sms, (cudaStream_t)cuda_stream, cache_cold(c, c->info.presorted_last_encode != 0));
     if (n < 0) return launch_failed(c, n, "encode kernel");
     count(c, n);
     c->info.path_last_encode = (uint32_t)p;
@@ -1097,14 +1100,14 @@ static oo_status query_device(oo_ctx* c, const oo_queries* q, float* d_rgb, cuda
             if (c->info.presorted_last_query) Qe.out_idx = nullptr;     // features stay in processing order for the MLP kernel ...
             EncodeOut O{c->d_feat, nullptr, nullptr};
             if (dbg.on() && !c->info.presorted_last_query) { O.slot = dbg.slot; O.texel = dbg.index; }
-            n = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Qe, O, c->tree_max_depth, stream) : launch_encode_fast(c->T, Qe, O, c->n_sms, stream);
+            n = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Qe, O, c->tree_max_depth, stream) : launch_encode_fast(c->T, Qe, O, c->n_sms, stream, cache_cold(c, c->info.presorted_last_query != 0));
             if (n < 0) return launch_failed(c, n, "encode kernel");
             count(c, n);
             if (dbg.on() && c->info.presorted_last_query) {             // ... so binned debug rows take a second, index-only pass
                 QueryParams Qi = Q;
                 Qi.out_idx = c->d_bidx;
                 EncodeOut Oi{nullptr, dbg.slot, dbg.index};
-                const int k = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Qi, Oi, c->tree_max_depth, stream) : launch_encode_fast(c->T, Qi, Oi, c->n_sms, stream);
+                const int k = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Qi, Oi, c->tree_max_depth, stream) : launch_encode_fast(c->T, Qi, Oi, c->n_sms, stream, true);
                 if (k < 0) return launch_failed(c, k, "encode kernel");
                 count(c, k);
             }

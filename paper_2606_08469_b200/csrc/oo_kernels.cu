@@ -205,6 +205,55 @@ __global__ void __launch_bounds__(256) encode_fast_kernel(const __grid_constant_
     }
 }
 
+// The same encode for batches whose taps miss the caches (binned or incoherent queries): the fused kernel's pipelined descent
+// (gather_pipelined: the hop chain overlaps the gathers, two or three levels of taps in flight per query) instead of one level
+// at a time.  It costs registers, i.e. occupancy, which is what the kernel above lives on when the taps hit L1/L2 -- so the
+// launcher picks per call: this one when the batch was binned or measured incoherent, the one above for coherent frames.
+// Same taps, weights and accumulation order: bit-identical rows.
+template <int L, int F, bool F32, bool IDX>
+__global__ void __launch_bounds__(256) encode_pipe_kernel(const __grid_constant__ TreeParams T,
+                                                          const __grid_constant__ QueryParams Q,
+                                                          const __grid_constant__ EncodeOut O) {
+    extern __shared__ __align__(16) uint8_t smem[];
+    int32_t* s_dense = (int32_t*)smem;
+    stage_to_smem(s_dense, T.dense, T.dense_ints * 4);
+    __syncthreads();
+    constexpr int TB = F * (F32 ? 4 : 2);
+    bool sample = Q.stat != nullptr && threadIdx.x < 32;
+    for (uint64_t t = blockIdx.x * (uint64_t)blockDim.x + threadIdx.x; t < Q.n; t += (uint64_t)gridDim.x * blockDim.x) {
+        const uint64_t qi = Q.perm ? Q.perm[t] : t;
+        const uint64_t oi = Q.out_idx ? Q.out_idx[t] : qi;
+        float x[3], w[3];
+        load3(Q.x, qi, x);
+        load3(Q.wo, qi, w);
+        if (sample) {
+            if ((t | 31u) < Q.n) stat_sample_warp(Q, blockIdx.x, x[0], x[1], x[2]);
+            sample = false;
+        }
+        typename DbgSel<IDX>::type dbg;          // IDX: the slot / base-texel rows are wanted too
+        if constexpr (IDX) {
+            dbg.slot = O.slot ? O.slot + oi * L : nullptr;
+            dbg.texel = O.texel ? O.texel + oi * L * 2 : nullptr;
+        }
+        uint8_t* row = (uint8_t*)O.features + oi * L * TB;
+        auto store = [&](int l, const float (&h)[F]) {
+            if (!O.features) return;
+            uint8_t* dst = row + l * TB;
+            if constexpr (F32) {
+#pragma unroll
+                for (int v = 0; v < F / 4; ++v)
+                    ((float4*)dst)[v] = make_float4(h[4 * v], h[4 * v + 1], h[4 * v + 2], h[4 * v + 3]);
+            } else {
+#pragma unroll
+                for (int v = 0; v < F / 8; ++v)
+                    ((uint4*)dst)[v] = make_uint4(pack_half2(h[8 * v], h[8 * v + 1]), pack_half2(h[8 * v + 2], h[8 * v + 3]),
+                                                  pack_half2(h[8 * v + 4], h[8 * v + 5]), pack_half2(h[8 * v + 6], h[8 * v + 7]));
+            }
+        };
+        gather_pipelined<L, F, F32>(T, s_dense, x, w, store, dbg);
+    }
+}
+
 // =====================================================================================================================
 // MLP input row: [h (L*F) | n | wo | extra | 0-pad] as fp16 in shared memory, row stride (k1 + 8) halves.
 // The tail (attributes + padding) is written 16 bytes at a time starting at column feat_dim (a multiple of 8).
@@ -411,11 +460,27 @@ bool fast_shape_supported(uint32_t L, uint32_t F, bool f32) {
     return false;
 }
 
-int launch_encode_fast(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, int n_sms, cudaStream_t stream) {
+// the shapes of the pipelined descent (pipe_applies: fp16 trees, two dense levels, then hops)
+#define OO_ENC_PIPE_SHAPES(X)                                                                          \
+    X(3, 8, false) X(4, 8, false) X(5, 8, false) X(6, 8, false) X(7, 8, false) X(8, 8, false)          \
+    X(3, 16, false) X(4, 16, false) X(5, 16, false) X(6, 16, false) X(7, 16, false) X(8, 16, false)
+
+// cache_cold: the batch was binned, or measured incoherent (OO_PRESORT_AUTO's samples): its taps miss L1/L2
+int launch_encode_fast(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, int n_sms, cudaStream_t stream, bool cache_cold) {
     if (Q.n == 0) return 0;
     const uint32_t smem = T.dense_ints * 4;
     const uint64_t blocks = (Q.n + 255) / 256;
     const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms * 8 ? blocks : (uint64_t)n_sms * 8);
+    if (cache_cold && pipe_applies(T)) {
+#define X(l, f, t)                                                                          \
+    if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                 \
+        if (O.slot || O.texel) encode_pipe_kernel<l, f, t, true><<<grid, 256, smem, stream>>>(T, Q, O);   \
+        else encode_pipe_kernel<l, f, t, false><<<grid, 256, smem, stream>>>(T, Q, O);      \
+        return 1;                                                                           \
+    }
+        OO_ENC_PIPE_SHAPES(X)
+#undef X
+    }
 #define X(l, f, t)                                                                          \
     if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                 \
         encode_fast_kernel<l, f, t><<<grid, 256, smem, stream>>>(T, Q, O);                  \
