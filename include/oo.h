@@ -223,6 +223,8 @@ typedef struct {
     uint32_t host_zero_copy_last; /* 1 if the last oo_query_host read its (pinned) host buffers in place, 0 if it ran the copy pipeline */
     uint32_t presort_auto_on;    /* OO_PRESORT_AUTO's current decision: 1 = the next batch of >= min_queries queries is binned */
     uint32_t coherence_x100;     /* 100 x mean number of distinct depth-4 cells per 32 consecutive queries, latest sample */
+    uint32_t encode_pipelined_last; /* 1 if the last oo_encode ran the pipelined-descent kernel (the batch was binned, or the latest coherence
+                                    sample says its taps miss the caches), 0 if it ran the occupancy kernel (coherent frames); same bytes either way */
 } oo_info;
 
 /* Create a context on a CUDA device.  Fails with OO_ERR_CUDA if the device is absent or is not compute capability

@@ -70,7 +70,7 @@ class _Info(C.Structure):
                 ("hop_plan_ok", C.c_uint32), ("n_sms", C.c_uint32),
                 ("presorted_last_query", C.c_uint32), ("presorted_last_encode", C.c_uint32),
                 ("full_query", C.c_uint32), ("n_neighbours", C.c_uint32), ("tied_vertices", C.c_uint64), ("host_zero_copy_last", C.c_uint32), ("presort_auto_on", C.c_uint32),
-                ("coherence_x100", C.c_uint32)]
+                ("coherence_x100", C.c_uint32), ("encode_pipelined_last", C.c_uint32)]
 
 
 _lib = None

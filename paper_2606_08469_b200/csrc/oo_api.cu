@@ -857,8 +857,13 @@ static void collect_samples(oo_ctx* c, cudaStream_t stream) {
         (void)cudaGetLastError();
 }
 // Will this batch's taps miss the caches?  Binned queries do by construction (they are incoherent or they would not have been binned);
-// otherwise the latest coherence sample decides (none taken yet: no).  Chooses between the two encode kernels.
-static bool cache_cold(const oo_ctx* c, bool binned) { return binned || c->coherence > 12.0f; }
+// otherwise, under OO_PRESORT_AUTO (the only mode that samples), the latest coherence sample decides.  Chooses between the two encode kernels.
+static bool cache_cold(oo_ctx* c, bool binned) {
+    if (binned) return true;
+    if (c->presort != OO_PRESORT_AUTO) return false;
+    update_coherence(c);                   // (batches below the binning threshold have not been through bin_wanted's update)
+    return c->coherence > 12.0f;
+}
 static bool bin_wanted(oo_ctx* c, const oo_queries* q) {
     if (q->perm || q->n < c->bin_min) return false;
     if (c->presort == OO_PRESORT_BIN) return true;
@@ -935,11 +940,13 @@ extern "C" OO_API oo_status oo_encode(oo_ctx* c, const oo_queries* q, void* d_fe
     } else if (p == OO_PATH_UNFUSED) {
         arm_sampling(c, Q);
     }
+    bool pipelined = false;
     int n = p == OO_PATH_GENERIC ? launch_encode_generic(c->T, Q, O, c->tree_max_depth, (cudaStream_t)cuda_stream)
-                                 : launch_encode_fast(c->T, Q, O, c->n_sms, (cudaStream_t)cuda_stream, cache_cold(c, c->info.presorted_last_encode != 0));
+                                 : launch_encode_fast(c->T, Q, O, c->n_sms, (cudaStream_t)cuda_stream, cache_cold(c, c->info.presorted_last_encode != 0), &pipelined);
     if (n < 0) return launch_failed(c, n, "encode kernel");
     count(c, n);
     c->info.path_last_encode = (uint32_t)p;
+    c->info.encode_pipelined_last = pipelined ? 1u : 0u;
     collect_samples(c, (cudaStream_t)cuda_stream);
     return check_after(c);
 }

@@ -149,7 +149,8 @@ int launch_tie_vertex_borders(void* maps, uint64_t slots, uint32_t R, uint32_t t
 int launch_encode_generic(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, uint32_t tree_max_depth,
                           cudaStream_t stream);
 // cache_cold: binned or measured-incoherent batch -> the pipelined-descent variant where the tree has one (oo_kernels.cu)
-int launch_encode_fast(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, int n_sms, cudaStream_t stream, bool cache_cold = false);
+int launch_encode_fast(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, int n_sms, cudaStream_t stream, bool cache_cold = false,
+                       bool* pipelined = nullptr);
 int launch_mlp_rows(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const void* features, float* rgb,
                     int n_sms, cudaStream_t stream);
 // dbg = true selects the instances with the index sink compiled in (oo_query_debug; QueryParams::dbg_slot / dbg_texel)

@@ -466,7 +466,8 @@ bool fast_shape_supported(uint32_t L, uint32_t F, bool f32) {
     X(3, 16, false) X(4, 16, false) X(5, 16, false) X(6, 16, false) X(7, 16, false) X(8, 16, false)
 
 // cache_cold: the batch was binned, or measured incoherent (OO_PRESORT_AUTO's samples): its taps miss L1/L2
-int launch_encode_fast(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, int n_sms, cudaStream_t stream, bool cache_cold) {
+int launch_encode_fast(const TreeParams& T, const QueryParams& Q, const EncodeOut& O, int n_sms, cudaStream_t stream, bool cache_cold, bool* pipelined) {
+    if (pipelined) *pipelined = false;
     if (Q.n == 0) return 0;
     const uint32_t smem = T.dense_ints * 4;
     const uint64_t blocks = (Q.n + 255) / 256;
@@ -476,6 +477,7 @@ int launch_encode_fast(const TreeParams& T, const QueryParams& Q, const EncodeOu
     if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                 \
         if (O.slot || O.texel) encode_pipe_kernel<l, f, t, true><<<grid, 256, smem, stream>>>(T, Q, O);   \
         else encode_pipe_kernel<l, f, t, false><<<grid, 256, smem, stream>>>(T, Q, O);      \
+        if (pipelined) *pipelined = true;                                                   \
         return 1;                                                                           \
     }
         OO_ENC_PIPE_SHAPES(X)

@@ -569,4 +569,25 @@ def test_presort_auto_follows_the_coherence_of_the_queries(P):
     torch.cuda.synchronize()
     f2 = ctx.oo_encode(xi, wi)
     torch.cuda.synchronize()
-    assert ctx.oo_get_info()["presorted_last_encode"] == 1 and torch.equal(f2, f_ref)
+    info = ctx.oo_get_info()
+    assert info["presorted_last_encode"] == 1 and info["encode_pipelined_last"] == 1 and torch.equal(f2, f_ref)
+    # oo_encode picks its kernel per call: binned or measured-incoherent batches run the fused kernel's pipelined descent, coherent frames
+    # the occupancy kernel; below the binning threshold an incoherent batch goes unsorted through the pipelined one.  Same bytes always.
+    ctx.oo_set_presort("none")
+    fc = ctx.oo_encode(xc, wc, want_debug=True)
+    ctx.oo_set_presort("auto", min_queries=1 << 30)                  # AUTO keeps sampling but never bins
+    for x_, w_, pipelined in ((xc, wc, 1), (xc, wc, 0), (xi, wi, 0), (xi, wi, 1), (xi, wi, 1), (xc, wc, 1), (xc, wc, 0)):   # the decision lags one call
+        f = ctx.oo_encode(x_, w_, want_debug=True)
+        torch.cuda.synchronize()
+        info = ctx.oo_get_info()
+        assert info["presorted_last_encode"] == 0 and info["encode_pipelined_last"] == pipelined, (info, pipelined)
+        ref = fc if x_ is xc else None
+        if ref is not None:
+            assert all(torch.equal(a, b) for a, b in zip(f, ref))
+    ctx.oo_set_presort("none")                                       # no samples are taken: only binned batches count as cache-cold
+    fi_fast = ctx.oo_encode(xi, wi, want_debug=True)
+    assert ctx.oo_get_info()["encode_pipelined_last"] == 0
+    ctx.oo_set_presort("bin", min_queries=1)
+    fi_pipe = ctx.oo_encode(xi, wi, want_debug=True)
+    assert ctx.oo_get_info()["encode_pipelined_last"] == 1
+    assert all(torch.equal(a, b) for a, b in zip(fi_pipe, fi_fast))  # features, slots and base texels, bit for bit
