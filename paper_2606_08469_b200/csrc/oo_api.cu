@@ -434,7 +434,7 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
         const uint32_t R = t->level_res[l], Rp = vertex ? R + 1 : R + 2;
         const uint64_t slots = std::max<uint64_t>(t->level_slots[l], 1);      // at least one (zero) map, so that the branch-free gather has an address
         const uint64_t map_bytes = (uint64_t)Rp * Rp * texel_bytes;
-        const uint64_t lead = vertex ? 0 : map_bytes;                         // texel maps: the all-zero map "slot -1" in front of slot 0
+        const uint64_t lead = map_bytes;                                      // the all-zero map "slot -1" in front of slot 0
         const uint64_t bytes = lead + slots * map_bytes;
         if (bytes / 16 >= (1ull << 32)) return fail(c, OO_ERR_UNSUPPORTED, "level %u: %llu bytes of maps; a level is addressed in 32-bit units of 16 bytes (64 GB)", l, (unsigned long long)bytes);
         OO_CUDA(c, cudaMalloc(&c->atlas_dev[l], bytes));
@@ -543,6 +543,8 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
             size_t rows = std::max<size_t>(by_depth[prev_depth].size(), 1);
             const int pl = level_of_depth[prev_depth];
             if (pl >= 0) rows = std::max<size_t>(t->level_slots[pl], 1);
+            if (((uint64_t)rows << (3 * gdep)) >= (1ull << 32))      // the kernels index a hop table with 32 bits
+                return fail(c, OO_ERR_UNSUPPORTED, "level %u: a hop table of %llu entries (>= 2^32, 16 GB)", l, (unsigned long long)rows << (3 * gdep));
             hop_host.emplace_back(rows << (3 * gdep), -1);
             std::vector<int32_t>& tab = hop_host.back();
             const uint32_t m = (1u << gdep) - 1;

@@ -48,31 +48,28 @@ __device__ __forceinline__ DirTaps dir_taps(const LevelParams& lv, int TB, OctaU
         d.w[0] = wx0 * wy0; d.w[1] = t.fx * wy0; d.w[2] = wx0 * t.fy; d.w[3] = t.fx * t.fy;
         d.ci = t.i0; d.cj = t.j0; d.up = 0;
     } else {
-        // g = u*(R/2) + R/2 (one rounding: the product is exact), cell = clamp(floor(g), 0, R-1), (a, b) = g - cell
+        // g = u*(R/2) + R/2 (one rounding: the product is exact), cell = min(floor(g), R-1) (g lies in [0, R]: |u| <= 1), (a, b) = g - cell
         const float gx = __fmaf_rn(uv.ux, lv.half_r, lv.half_r), gy = __fmaf_rn(uv.uy, lv.half_r, lv.half_r);
         const int Rm1 = (int)lv.R - 1;
-        const int ci = max(min((int)floorf(gx), Rm1), 0), cj = max(min((int)floorf(gy), Rm1), 0);
+        const int ci = min(__float2int_rd(gx), Rm1), cj = min(__float2int_rd(gy), Rm1);
         const float a = __fsub_rn(gx, (float)ci), b = __fsub_rn(gy, (float)cj);
         const int half = (int)(lv.R >> 1);
         const bool same = (ci >= half) == (cj >= half);
-        const bool up = same ? (__fadd_rn(a, b) >= 1.0f) : (b > a);
+        const bool up = same ? (__fadd_rn(a, b) >= 1.0f) : (b > a);          // the index decisions, in the contract's form
+        // Weights and taps: a cell split along its anti-diagonal (same-sign quadrant) is a cell split along its main diagonal mirrored in
+        // x -- a' = 1 - a, columns swapped -- so one rule serves both: vertices (0,0)' and (1,1)' always, (0,1)' above the diagonal
+        // and (1,0)' below it, with weights 1 - max(a', b), min(a', b), |b - a'|.
+        const float am = same ? 1.0f - a : a;
+        const int x0 = same ? TB : 0, x1 = TB - x0;
         const int row = (int)lv.row_bytes;
         const int c00 = (cj * (int)lv.Rp + ci) * TB;
-        // anti-diagonal split (same-sign quadrant): taps (1,0) (0,1) and (0,0) [lower] or (1,1) [upper]
-        // main-diagonal split                    : taps (0,0) (1,1) and (1,0) [lower, a >= b] or (0,1) [upper]
-        d.off[0] = c00 + (same ? TB : 0);
-        d.off[1] = c00 + (same ? row : row + TB);
-        d.off[2] = c00 + (same ? (up ? row + TB : 0) : (up ? row : TB));
+        d.off[0] = c00 + x0;
+        d.off[1] = c00 + row + x1;
+        d.off[2] = up ? c00 + row + x0 : c00 + x1;
         d.off[3] = d.off[2];
-        if (same) {
-            d.w[0] = up ? 1.0f - b : a;
-            d.w[1] = up ? 1.0f - a : b;
-            d.w[2] = up ? (a + b) - 1.0f : (1.0f - a) - b;
-        } else {
-            d.w[0] = up ? 1.0f - b : 1.0f - a;
-            d.w[1] = up ? a : b;
-            d.w[2] = up ? b - a : a - b;
-        }
+        d.w[0] = 1.0f - (up ? b : am);
+        d.w[1] = up ? am : b;
+        d.w[2] = fabsf(b - am);
         d.w[3] = 0.0f;
         d.ci = ci; d.cj = cj; d.up = up ? 1 : 0;
     }
@@ -160,7 +157,7 @@ __device__ __forceinline__ void block_slots(const LevelParams& lv, const int32_t
         else prev = st.node[0];
         const uint32_t idx = ix[0][ox] | ix[1][oy] | ix[2][oz];
         int v = -1;
-        if (prev >= 0) v = __ldg(lv.hop + (((size_t)prev << (3 * g)) + idx));
+        if (prev >= 0) v = __ldg(lv.hop + (((uint32_t)prev << (3 * g)) + idx));
         slot[j] = v;
     }
 #pragma unroll
@@ -246,12 +243,12 @@ __device__ __forceinline__ void full_level(const LevelParams& lv, const int32_t*
             } else {
                 d = dq;
             }
-            const bool ok = slot[j] >= 0;
-            const uint8_t* p = lv.atlas + (uint64_t)(ok ? (uint32_t)slot[j] : 0u) * lv.map_bytes;
+            // an absent neighbour (slot -1) reads the all-zero map in front of slot 0 (and carries weight 0): no test, no predicate
+            const uint8_t* p = lv.atlas + (int64_t)slot[j] * (int64_t)lv.map_bytes;
 #pragma unroll
             for (int k = 0; k < NT; ++k)
 #pragma unroll
-                for (int q = 0; q < NV; ++q) v[b][k][q] = ok ? ldg16(p + d.off[k] + 16 * q) : make_uint4(0, 0, 0, 0);
+                for (int q = 0; q < NV; ++q) v[b][k][q] = ldg16(p + d.off[k] + 16 * q);
             tw[b].w00 = wj[j] * d.w[0]; tw[b].w10 = wj[j] * d.w[1]; tw[b].w01 = wj[j] * d.w[2]; tw[b].w11 = wj[j] * d.w[3];
             if constexpr (!F32) {
                 tw[b].p0 = pack_half2(tw[b].w00, tw[b].w10);
