@@ -214,10 +214,14 @@ def ingest_ncu(args):
             launches.setdefault(int(r[k_id]), {"kernel": r[k_name].split("(")[0]})[r[k_metric]] = float(r[k_val].replace(",", ""))
     if not launches:
         raise SystemExit("no launch of a kernel matching %r in %s" % (args.ingest_kernel, args.ingest_ncu))
-    # the step's launch, not the smaller ones of the e2e leg's chunks: the last launch among those with the most instructions
+    # the step's launch: among the launches with the most instructions (not the smaller ones of the e2e leg's chunks) the last one that
+    # ran from device memory (the e2e leg's zero-copy launch executes the same instructions but reads its queries over PCIe and takes
+    # many times longer)
     key = "smsp__inst_executed.sum" if any("smsp__inst_executed.sum" in v for v in launches.values()) else "gpu__time_duration.sum"
     top = max(v.get(key, 0) for v in launches.values())
-    m = launches[max(i for i, v in launches.items() if v.get(key, 0) >= 0.99 * top)]
+    full = {i: v for i, v in launches.items() if v.get(key, 0) >= 0.99 * top}
+    fastest = min(v.get("gpu__time_duration.sum", 0) for v in full.values())
+    m = full[max(i for i, v in full.items() if v.get("gpu__time_duration.sum", 0) <= 1.5 * fastest)]
     tp = os.path.join(ROOT, "profiles", "traffic.json")
     d = json.load(open(tp)) if os.path.exists(tp) else {}
     d.pop("source", None)

@@ -31,6 +31,9 @@
  *     ...: every later call then fails at once with OO_ERR_CUDA).  A non-fatal CUDA error that some other code left
  *     pending on the calling thread is cleared by the next oo_ call that launches (it is not this library's to report).
  *   - One context per device; several contexts, on the same or on different devices, may live in one process.
+ *   - A context is not thread-safe, and its hot calls share context-owned scratch (the binned copy of the queries, staging, feature
+ *     rows, coherence samples): calls on ONE context must be ordered on one stream (or by events between streams).  Work that is to
+ *     overlap on several streams takes one context per stream.
  *   - Not checked per query (result undefined, never a crash): non-finite inputs, wo = 0.  x outside [0,1]^3 is
  *     clamped componentwise (A16).
  *   - There is no CPU fallback: without a usable CUDA device oo_create fails.
