@@ -115,6 +115,42 @@ def test_absent_cells_and_out_of_cube_positions(P):
     _run_all(P, w, f, s, t, rgb)
 
 
+def test_direction_magnitudes_and_tiny_components(P):
+    """The index contract at the ends of the range (A22: wo is not normalised).  Eq. 4 divides by the L1 norm, and the kernels share one
+    refined reciprocal between its two divisions (div2_rn) where the operands lie in [2^-60, 2^60], the compiler's IEEE division elsewhere:
+    directions scaled by 2^-75 .. 2^75 (and by factors that are not powers of two), with one or two components 20 or more orders of
+    magnitude below the largest, must give the oracle's slots and base texels bit for bit on every path, and its features."""
+    w = gen.scene_workload(1, width=64, height=64)
+    q = gen.random_queries(8192, 11)
+    rng = np.random.default_rng(5)
+    n = q.n
+    scale = np.ldexp(1.0, rng.integers(-75, 76, n)) * np.where(rng.random(n) < 0.5, 1.0, rng.uniform(1.0, 2.0, n))
+    wo = q.wo.astype(np.float64)
+    tiny = rng.random((n, 3)) < 0.25
+    tiny[np.arange(n), np.argmax(np.abs(wo), axis=1)] = False          # the largest component stays
+    wo = np.where(tiny, wo * np.ldexp(1.0, -rng.integers(66, 100, (n, 3))), wo)
+    q.wo = (wo * scale[:, None]).astype(np.float32)
+    assert np.isfinite(q.wo).all() and (np.abs(q.wo).max(axis=1) > 0).all()
+    w.queries = q
+    co = OC.from_workload(w)
+    f_ref, s_ref, t_ref = co.encode(q.x, q.wo)
+    ctx = P.OctaOctree(0).upload_workload(w)
+    ctx.oo_reserve(n)
+    x, nr, wo_d, ex = _dev(q)
+    for path in _paths(P, ctx):
+        ctx.oo_set_path(path)
+        _, s_d, t_d = ctx.oo_query_debug(x, nr, wo_d, ex)             # the RGB is meaningless here (the decoder sees the raw wo): indices only
+        torch.cuda.synchronize()
+        check_indices(s_d.cpu().numpy(), t_d.cpu().numpy(), s_ref, t_ref)
+    for path in (P.PATH_GENERIC, P.PATH_UNFUSED):
+        ctx.oo_set_path(path)
+        f, s, t = ctx.oo_encode(x, wo_d, want_debug=True)
+        torch.cuda.synchronize()
+        check_indices(s.cpu().numpy(), t.cpu().numpy(), s_ref, t_ref)
+        check_features(f.float().cpu().numpy(), f_ref)
+    ctx.close()
+
+
 def test_non_canonical_levels_fall_back_to_generic(P):
     """Used depths {1, 8}: 8 is more than 3 levels below the top station (depth 4), so there is no hop plan; AUTO must
     run the generic kernels and still match."""
