@@ -46,14 +46,22 @@ __device__ __forceinline__ void relu_pack32(const uint32_t (&r)[32], uint32_t (&
 // padding) is gathered and packed while that MMA is in flight, stored over the same columns once it has completed, and
 // accumulated by the second group.  A tile then needs 96 TMEM columns like the narrow configs instead of 64 + k1/2, so five
 // warpgroups fit where four did (config 3: k1 = 96, 112 columns), at the price of one more MMA round trip per tile.
-template <int L, int F, bool F32, int NWG, bool PIPE = false, bool KS = false, bool DBG = false>
+// H, K1, NX (0, 0, -1 = read from the parameter structs): the decoder's hidden-layer count, the padded width of its first layer and the
+// number of extra scalars as compile-time constants, with out_dim = 3 through exp implied.  The instances of the BASELINE.json configs
+// are compiled this way: the layer loop unrolls, the K-step predicates of the MMA issue, the attribute-row conditionals and most
+// parameter loads fold away (config 1: 901 -> ~780 thread instructions per query).  Same arithmetic, same order: bit-identical.
+template <int L, int F, bool F32, int NWG, bool PIPE = false, bool KS = false, bool DBG = false, int H = 0, int K1 = 0, int NX = -1>
 __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_constant__ TreeParams T,
                                                                const __grid_constant__ MlpParams M,
                                                                const __grid_constant__ QueryParams Q,
                                                                float* __restrict__ rgb, uint32_t n_tiles, uint32_t wg_cols) {
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t dense_bytes = (T.dense_ints * 4 + 127) & ~127u;
-    const uint32_t q_words = 10 + Q.n_extra;                         // x3 n3 wo3 index extras, each [128] words
+    constexpr bool SPEC = H != 0;                                     // (then out_dim = 3 through exp: checked by the launcher)
+    const uint32_t n_extra = NX >= 0 ? (uint32_t)NX : Q.n_extra;
+    const uint32_t n_hidden = H ? (uint32_t)H : M.n_hidden;
+    const uint32_t k1 = K1 ? (uint32_t)K1 : M.k1;
+    const uint32_t q_words = 10 + n_extra;                           // x3 n3 wo3 index extras, each [128] words
     const uint32_t q_bytes = q_words * kRows * 4;
     int32_t* s_dense = (int32_t*)smem;
     uint8_t* s_w = smem + dense_bytes;
@@ -92,7 +100,8 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             cp_async4(q_addr + (3 + k) * 512, pn + k);
             cp_async4(q_addr + (6 + k) * 512, pw + k);
         }
-        for (uint32_t k = 0; k < Q.n_extra; ++k) cp_async4(q_addr + (10 + k) * 512, Q.extra + (size_t)qi * Q.n_extra + k);
+#pragma unroll(NX > 0 ? NX : 1)
+        for (uint32_t k = 0; k < n_extra; ++k) cp_async4(q_addr + (10 + k) * 512, Q.extra + (size_t)qi * n_extra + k);
         s_q[9 * 128] = __uint_as_float(qi);
         asm volatile("cp.async.commit_group;" ::: "memory");
     };
@@ -114,7 +123,10 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
     const uint32_t w_addr = smem_u32(s_w), bar = smem_u32(&s_bar[wg]);
     const bool rgb_vec = !Q.perm && !Q.out_idx && ((uintptr_t)rgb & 15u) == 0;   // rows in order and the output 16-byte aligned: vector stores
     uint32_t phase = 0;
-    const bool leader_warp = row < 32;
+    // The warp that issues a warpgroup's MMAs executes ~45 % more instructions per tile than the other three (descriptor arithmetic on the
+    // uniform datapath, elect, commit) and every tile waits for it: the five issuing warps sit on different scheduler partitions
+    // (warp index mod 4) instead of all on partition 0 (ncu before: issue slots 75 % busy there, 51 % on the other three).
+    const bool leader_warp = (row >> 5) == (wg & 3u);
     constexpr uint32_t idesc_h = instr_desc(128, 64), idesc_o = instr_desc(128, 16);
     const uint32_t tile_stride = gridDim.x * NWG;
 
@@ -230,10 +242,10 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             for (int k = 0; k < 3; ++k) { v[lead + k] = s_q[(3 + k) * 128]; v[lead + 3 + k] = w[k]; }
 #pragma unroll
             for (int k = 0; k < OO_MAX_EXTRA; ++k)
-                if ((uint32_t)k < Q.n_extra) v[lead + 6 + k] = s_q[(10 + k) * 128];
+                if ((uint32_t)k < n_extra) v[lead + 6 + k] = s_q[(10 + k) * 128];
             qi = __float_as_uint(s_q[9 * 128]);
             constexpr int c0 = (L * F) / 8;              // first 8-half unit (4 columns) holding attributes
-            const uint32_t c_end = M.k1 / 8;
+            const uint32_t c_end = k1 / 8;
             if constexpr (lead == 0) {
                 tmem_st4(aA + 4 * c0, pack_half2(v[0], v[1]), pack_half2(v[2], v[3]), pack_half2(v[4], v[5]), pack_half2(v[6], v[7]));
             } else {
@@ -250,8 +262,9 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
 #endif
         // ------------------------------------------------------------------ hidden layers
         uint32_t w_off = 0;
-        for (uint32_t layer = 0; layer < M.n_hidden; ++layer) {
-            const uint32_t kt_n = (layer == 0 ? M.k1 : 64u) >> 4;
+#pragma unroll(H ? H : 1)
+        for (uint32_t layer = 0; layer < n_hidden; ++layer) {
+            const uint32_t kt_n = (layer == 0 ? k1 : 64u) >> 4;
             const bool second = KS && layer == 0;         // layer 0's inputs 64.. : 4 K-steps further into W0, accumulating
             const bool odd = layer & 1u;
 #ifdef OO_PROFILE_PHASES
@@ -304,7 +317,7 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             }
         }
         // ------------------------------------------------------------------ output layer (N = 16, K = 64)
-        const bool odd = M.n_hidden & 1u;
+        const bool odd = n_hidden & 1u;
         tmem_wait_st();
         fence_before_sync();
         named_bar(1 + wg, 128);
@@ -320,7 +333,7 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
         uint32_t o[4];
         tmem_ld4(o_addr, o);
         tmem_wait_ld();
-        if (M.out_dim == 3 && M.out_act == OO_ACT_EXP) {       // RGB through exp: the case every BASELINE.json config runs
+        if (SPEC || (M.out_dim == 3 && M.out_act == OO_ACT_EXP)) {       // RGB through exp: the case every BASELINE.json config runs
             const float r0 = fast_exp(__uint_as_float(o[0])), r1 = fast_exp(__uint_as_float(o[1])), r2 = fast_exp(__uint_as_float(o[2]));
             // A warp's 32 rows are 384 contiguous bytes of the output when the queries are processed in order: they go through a
             // warp-private strip of shared memory and leave as 24 sixteen-byte stores (whole 32-byte sectors: what makes writing the RGB
@@ -392,6 +405,20 @@ static bool ks_applies(const TreeParams& T, const MlpParams& M) {
 }
 #define OO_TM_KS_SHAPES(X) X(4, 16, false) X(5, 16, false) X(6, 16, false) X(7, 16, false) X(8, 8, false)
 
+// one instance with the decoder's shape compiled in (see H, K1, NX above)
+template <int L, int F, int NWG, bool KS, bool DBG, int H, int K1, int NX>
+static int launch_tm_spec(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, uint32_t wg_cols, cudaStream_t stream) {
+    const uint64_t n_tiles = (Q.n + kRows - 1) / kRows;
+    const unsigned grid = (unsigned)(n_tiles < (uint64_t)n_sms ? n_tiles : (uint64_t)n_sms);
+    const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + NWG * (10 + Q.n_extra) * kRows * 4 + NWG * 4 * 96 * 4 + 128;
+    if (smem > 227 * 1024) return -1;
+    static std::atomic<uint64_t> opted{0};
+    auto kern = fused_tm_kernel<L, F, false, NWG, true, KS, DBG, H, K1, NX>;
+    if (!opt_in_smem(opted, (const void*)kern, 227 * 1024)) return kLaunchCudaError;
+    kern<<<grid, NWG * 128, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles, wg_cols);
+    return 1;
+}
+
 template <int NWG, bool PIPE, bool KS, bool DBG>
 static int launch_tm_variant(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, uint32_t wg_cols,
                              cudaStream_t stream) {
@@ -428,6 +455,12 @@ static int launch_fused_tm_impl(const TreeParams& T, const MlpParams& M, const Q
     // unsorted incoherent 2^22 queries 1.53 -> 1.32 ms.  Binned queries: mixed with four warpgroups (-2 % at 2^22, +8 % at 2^24),
     // a gain at every size once KS runs five (2^22 0.657 -> 0.632 ms, 2^24 2.40 -> 2.22 ms), so PIPE is used wherever it applies.
     const bool pipe = pipe_applies(T);
+    // the BASELINE.json configs: decoder shape compiled in (configs 1, 2: 38/39 -> 3 x 64 -> 3 exp on L = 4, F = 8; configs 3, 4: 86 -> 4 x 64 -> 3 exp on L = 5, F = 16)
+    if (pipe && M.out_dim == 3 && M.out_act == OO_ACT_EXP && !T.f32) {
+        if (T.n_levels == 4 && T.F == 8 && M.n_hidden == 3 && M.k1 == 48 && Q.n_extra == 0) return launch_tm_spec<4, 8, 5, false, DBG, 3, 48, 0>(T, M, Q, rgb, n_sms, 96, stream);
+        if (T.n_levels == 4 && T.F == 8 && M.n_hidden == 3 && M.k1 == 48 && Q.n_extra == 1) return launch_tm_spec<4, 8, 5, false, DBG, 3, 48, 1>(T, M, Q, rgb, n_sms, 96, stream);
+        if (T.n_levels == 5 && T.F == 16 && M.n_hidden == 4 && M.k1 == 96 && Q.n_extra == 0) return launch_tm_spec<5, 16, 5, true, DBG, 4, 96, 0>(T, M, Q, rgb, n_sms, 96, stream);
+    }
     if (ks_applies(T, M)) {      // 96 columns per tile: five warpgroups
         const int n = pipe ? launch_tm_variant<5, true, true, DBG>(T, M, Q, rgb, n_sms, 96, stream)
                            : launch_tm_variant<5, false, true, DBG>(T, M, Q, rgb, n_sms, 96, stream);
