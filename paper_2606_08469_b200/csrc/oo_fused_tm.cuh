@@ -182,16 +182,21 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             }
             if constexpr (KS) {
                 if ((l + 1) * F == 64) {      // inputs 0..63 of all 128 rows are in TMEM: first MMA group of layer 0
-                    tmem_wait_st();
-                    fence_before_sync();
-                    named_bar(1 + wg, 128);
-                    if (leader_warp) {
+                    uint32_t g_d = tmem_wg, g_a = tmem_wg + 64u;
+                    uint64_t g_b = smem_desc(w_addr, 1024, 128);
+                    if (leader_warp) {           // operand addresses and the weights' arrival ahead of the barrier (see the hidden layers)
+                        asm volatile("" : "+r"(g_d), "+r"(g_a), "+l"(g_b));
                         if (!w_ready) {
                             mbar_wait(bar_w, 0);
                             w_ready = true;
                         }
+                    }
+                    tmem_wait_st();
+                    fence_before_sync();
+                    named_bar(1 + wg, 128);
+                    if (leader_warp) {
                         fence_after_sync();
-                        umma_group_ts<4>(tmem_wg, tmem_wg + 64u, smem_desc(w_addr, 1024, 128), 2048 >> 4, idesc_h, 4u, bar);
+                        umma_group_ts<4>(g_d, g_a, g_b, 2048 >> 4, idesc_h, 4u, bar);
                     }
                 }
             }
@@ -270,6 +275,18 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
 #ifdef OO_PROFILE_PHASES
             const long long tb0 = clock64();
 #endif
+            // The issuing warp forms this layer's operand addresses BEFORE it waits for the other warps' rows (the empty volatile asm pins
+            // the values ahead of the barrier): between the barrier and the first tcgen05.mma only the issue itself is left.  Every
+            // instruction of that warp there is on the tile's critical path and takes ~9 cycles with five warps sharing a scheduler.
+            uint32_t mma_d = tmem_wg + (odd ? 32u : 0u), mma_a = tmem_wg + (odd ? 0u : 64u);
+            uint64_t mma_b = smem_desc(w_addr + w_off + (second ? 4u * 2048u : 0u), 1024, 128);
+            if (leader_warp) {
+                asm volatile("" : "+r"(mma_d), "+r"(mma_a), "+l"(mma_b));
+                if (layer == 0 && !w_ready) {
+                    mbar_wait(bar_w, 0);      // weight image in shared memory (first MMA of this warpgroup only)
+                    w_ready = true;
+                }
+            }
             tmem_wait_st();              // my row of A is in TMEM
             fence_before_sync();
             named_bar(1 + wg, 128);
@@ -277,13 +294,8 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             tb += clock64() - tb0;
 #endif
             if (leader_warp) {
-                if (!w_ready) {
-                    mbar_wait(bar_w, 0);      // weight image in shared memory (first MMA of this warpgroup only)
-                    w_ready = true;
-                }
                 fence_after_sync();
-                umma_group_ts<8>(tmem_wg + (odd ? 32u : 0u), tmem_wg + (odd ? 0u : 64u), smem_desc(w_addr + w_off + (second ? 4u * 2048u : 0u), 1024, 128),
-                                 2048 >> 4, idesc_h, second ? kt_n - 4u : kt_n, bar, second ? 1u : 0u);
+                umma_group_ts<8>(mma_d, mma_a, mma_b, 2048 >> 4, idesc_h, second ? kt_n - 4u : kt_n, bar, second ? 1u : 0u);
             }
             w_off += kt_n * 2 * 1024;
 #ifdef OO_PROFILE_PHASES
@@ -318,12 +330,15 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
         }
         // ------------------------------------------------------------------ output layer (N = 16, K = 64)
         const bool odd = n_hidden & 1u;
+        uint32_t out_d = tmem_wg + (odd ? 32u : 0u), out_a = tmem_wg + (odd ? 0u : 64u);
+        uint64_t out_b = smem_desc(w_addr + w_off, 256, 128);
+        if (leader_warp) asm volatile("" : "+r"(out_d), "+r"(out_a), "+l"(out_b));       // formed ahead of the barrier, as above
         tmem_wait_st();
         fence_before_sync();
         named_bar(1 + wg, 128);
         if (leader_warp) {
             fence_after_sync();
-            umma_group_ts<4>(tmem_wg + (odd ? 32u : 0u), tmem_wg + (odd ? 0u : 64u), smem_desc(w_addr + w_off, 256, 128), 512 >> 4, idesc_o, 4u, bar);
+            umma_group_ts<4>(out_d, out_a, out_b, 512 >> 4, idesc_o, 4u, bar);
         }
         mbar_wait(bar, phase);
         phase ^= 1;
