@@ -261,7 +261,6 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             if (c0 + 2 < c_end)
                 tmem_st4(aA + 4 * (c0 + 2), pack_half2(v[16], v[17]), pack_half2(v[18], v[19]), pack_half2(v[20], v[21]), pack_half2(v[22], v[23]));
         }
-        if (tile + tile_stride < n_tiles) prefetch(tile + tile_stride);
 #ifdef OO_PROFILE_PHASES
         const long long t1 = clock64();
 #endif
@@ -297,6 +296,9 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
                 fence_after_sync();
                 umma_group_ts<8>(mma_d, mma_a, mma_b, 2048 >> 4, idesc_h, second ? kt_n - 4u : kt_n, bar, second ? 1u : 0u);
             }
+            // the next tile's queries are requested inside layer 0's MMA window (the staging buffer was read above): ~35 instructions
+            // per thread that would otherwise sit between the gather and the first MMA of every tile
+            if (layer == 0 && tile + tile_stride < n_tiles) prefetch(tile + tile_stride);
             w_off += kt_n * 2 * 1024;
 #ifdef OO_PROFILE_PHASES
             const long long tw0 = clock64();
