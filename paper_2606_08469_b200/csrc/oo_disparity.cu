@@ -157,13 +157,16 @@ __global__ void __launch_bounds__(kNWG * 128, 1) disparity_kernel(const __grid_c
         for (uint32_t layer = 0; layer < M.n_hidden; ++layer) {
             const uint32_t kt_n = (layer == 0 ? M.k1 : 64u) >> 4;
             const bool odd = layer & 1u;
+            // operand addresses formed by the issuing warp ahead of the barrier (see oo_fused_tm.cuh)
+            uint32_t mma_d = tmem_wg + (odd ? 32u : 0u), mma_a = tmem_wg + (odd ? 0u : 64u);
+            uint64_t mma_b = smem_desc(w_addr + w_off, 1024, 128);
+            if (leader_warp) asm volatile("" : "+r"(mma_d), "+r"(mma_a), "+l"(mma_b));
             tmem_wait_st();
             fence_before_sync();
             named_bar(1 + wg, 128);
             if (leader_warp) {
                 fence_after_sync();
-                umma_group_ts<4>(tmem_wg + (odd ? 32u : 0u), tmem_wg + (odd ? 0u : 64u), smem_desc(w_addr + w_off, 1024, 128), 2048 >> 4,
-                                 idesc_h, kt_n, bar);
+                umma_group_ts<4>(mma_d, mma_a, mma_b, 2048 >> 4, idesc_h, kt_n, bar);
             }
             w_off += kt_n * 2 * 1024;
             mbar_wait(bar, phase);
@@ -192,12 +195,15 @@ __global__ void __launch_bounds__(kNWG * 128, 1) disparity_kernel(const __grid_c
         }
         // ------------------------------------------------------------------ output layer (N = 16 rows of which one is real)
         const bool odd = M.n_hidden & 1u;
+        uint32_t out_d = tmem_wg + (odd ? 32u : 0u), out_a = tmem_wg + (odd ? 0u : 64u);
+        uint64_t out_b = smem_desc(w_addr + w_off, 256, 128);
+        if (leader_warp) asm volatile("" : "+r"(out_d), "+r"(out_a), "+l"(out_b));
         tmem_wait_st();
         fence_before_sync();
         named_bar(1 + wg, 128);
         if (leader_warp) {
             fence_after_sync();
-            umma_group_ts<4>(tmem_wg + (odd ? 32u : 0u), tmem_wg + (odd ? 0u : 64u), smem_desc(w_addr + w_off, 256, 128), 512 >> 4, idesc_o, 4u, bar);
+            umma_group_ts<4>(out_d, out_a, out_b, 512 >> 4, idesc_o, 4u, bar);
         }
         mbar_wait(bar, phase);
         phase ^= 1;

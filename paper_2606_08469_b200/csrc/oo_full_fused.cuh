@@ -170,13 +170,17 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
         for (uint32_t layer = 0; layer < M.n_hidden; ++layer) {
             const uint32_t kt_n = (layer == 0 ? M.k1 : (uint32_t)W) >> 4;
             const bool odd = layer & 1u;
+            // the issuing warp forms the layer's operand addresses ahead of the barrier (see oo_fused_tm.cuh): between the barrier and the
+            // first tcgen05.mma only the issue itself is left on the tile's critical path
+            uint32_t mma_d = tmem_team + (odd ? (uint32_t)(W / 2) : 0u), mma_a = tmem_team + (odd ? 0u : (uint32_t)W);
+            uint64_t mma_b = smem_desc(w_addr + w_off, 16 * W, 128);
+            if (leader_warp) asm volatile("" : "+r"(mma_d), "+r"(mma_a), "+l"(mma_b));
             tmem_wait_st();              // my part of A is in TMEM
             fence_before_sync();
             named_bar(1 + team, TEAM_THREADS);
             if (leader_warp) {
                 fence_after_sync();
-                umma_group_ts<8>(tmem_team + (odd ? (uint32_t)(W / 2) : 0u), tmem_team + (odd ? 0u : (uint32_t)W),
-                                 smem_desc(w_addr + w_off, 16 * W, 128), (32 * W) >> 4, idesc_h, kt_n, bar);
+                umma_group_ts<8>(mma_d, mma_a, mma_b, (32 * W) >> 4, idesc_h, kt_n, bar);
             }
             if (layer == 0 && part == 0 && tile + tile_stride < n_tiles) prefetch(tile + tile_stride);   // staging is free now
             w_off += kt_n * 32 * W;
@@ -222,13 +226,15 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
         }
         // ------------------------------------------------------------------ output layer (N = 16, K = W)
         const bool odd = M.n_hidden & 1u;
+        uint32_t out_d = tmem_team + (odd ? (uint32_t)(W / 2) : 0u), out_a = tmem_team + (odd ? 0u : (uint32_t)W);
+        uint64_t out_b = smem_desc(w_addr + w_off, 256, 128);
+        if (leader_warp) asm volatile("" : "+r"(out_d), "+r"(out_a), "+l"(out_b));
         tmem_wait_st();
         fence_before_sync();
         named_bar(1 + team, TEAM_THREADS);
         if (leader_warp) {
             fence_after_sync();
-            umma_group_ts<W / 16>(tmem_team + (odd ? (uint32_t)(W / 2) : 0u), tmem_team + (odd ? 0u : (uint32_t)W),
-                                  smem_desc(w_addr + w_off, 256, 128), 512 >> 4, idesc_o, (uint32_t)(W / 16), bar);
+            umma_group_ts<W / 16>(out_d, out_a, out_b, 512 >> 4, idesc_o, (uint32_t)(W / 16), bar);
         }
         mbar_wait(bar, phase);
         phase ^= 1;
