@@ -50,13 +50,19 @@ __device__ __forceinline__ void relu_pack32(const uint32_t (&r)[32], uint32_t (&
 // number of extra scalars as compile-time constants, with out_dim = 3 through exp implied.  The instances of the BASELINE.json configs
 // are compiled this way: the layer loop unrolls, the K-step predicates of the MMA issue, the attribute-row conditionals and most
 // parameter loads fold away (config 1: 901 -> ~780 thread instructions per query).  Same arithmetic, same order: bit-identical.
-template <int L, int F, bool F32, int NWG, bool PIPE = false, bool KS = false, bool DBG = false, int H = 0, int K1 = 0, int NX = -1>
+// NSLOT < NWG (k1 <= 64 or KS, i.e. 32 A columns): the accumulators are SHARED.  Every warpgroup owns an A region of 32 columns (its tile's
+// activations) and the fp32 accumulator D (64 columns) lives in one of NSLOT slots taken from a free mask in shared memory right before the
+// tile's first MMA and given back when its four warps have read the output:  A of warpgroup wg at [32 wg, +32), D slot s at
+// [32 NWG + 64 s, +64); 6 x 32 + 5 x 64 = 512 columns.  A tile needs a D slot only for the decoder half of its life, so six tiles share five.
+// The epilogue reads its whole row of D into registers and then writes the next layer's A over the A region (the MMA that read it has completed).
+template <int L, int F, bool F32, int NWG, bool PIPE = false, bool KS = false, bool DBG = false, int H = 0, int K1 = 0, int NX = -1, int NSLOT = NWG>
 __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_constant__ TreeParams T,
                                                                const __grid_constant__ MlpParams M,
                                                                const __grid_constant__ QueryParams Q,
                                                                float* __restrict__ rgb, uint32_t n_tiles, uint32_t wg_cols) {
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t dense_bytes = (T.dense_ints * 4 + 127) & ~127u;
+    constexpr bool DYN = NSLOT < NWG;                                 // accumulator slots are handed around
     constexpr bool SPEC = H != 0;                                     // (then out_dim = 3 through exp: checked by the launcher)
     const uint32_t n_extra = NX >= 0 ? (uint32_t)NX : Q.n_extra;
     const uint32_t n_hidden = H ? (uint32_t)H : M.n_hidden;
@@ -69,6 +75,9 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
     float* s_out = (float*)(s_stage + NWG * q_bytes);            // [NWG * 4 warps][32 rows * 3]: a warp's RGB rows before their 16-byte stores
     uint64_t* s_bar = (uint64_t*)(s_out + NWG * 4 * 96);         // one per warpgroup, then tables, then weights
     uint32_t* s_tmem = (uint32_t*)(s_bar + NWG + 2);
+    uint32_t* s_free = s_tmem + 1;                               // DYN: bit s set = D slot s is free
+    uint32_t* s_slot = s_free + 1;                               // [NWG] the slot a warpgroup's tile holds, for its other warps
+    uint32_t* s_rel = s_slot + NWG;                              // [NWG] warps of the warpgroup that are done with the slot
 
     const uint32_t wg = threadIdx.x >> 7, row = threadIdx.x & 127, warp = threadIdx.x >> 5;
     // Prologue: the descent tables and the weight image arrive by two bulk asynchronous copies that thread 0 issues before
@@ -79,6 +88,9 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int k = 0; k < NWG + 2; ++k) mbar_init(smem_u32(&s_bar[k]), 1);
+        *s_free = (1u << NSLOT) - 1u;
+#pragma unroll
+        for (int k = 0; k < NWG; ++k) s_rel[k] = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
         mbar_expect_tx(bar_d, T.dense_ints * 4);
         bulk_g2s(smem_u32(s_dense), T.dense, T.dense_ints * 4, bar_d);
@@ -118,8 +130,13 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
     fence_before_sync();
     __syncthreads();
     fence_after_sync();
-    const uint32_t tmem_wg = *s_tmem + wg * wg_cols;                 // this warpgroup's columns
-    const uint32_t tmem_lane = tmem_wg + ((row & ~31u) << 16);       // ... and this warp's 32 lanes
+    const uint32_t tmem_wg = *s_tmem + wg * wg_cols;                 // this warpgroup's columns (DYN: wg_cols = 32, its A region)
+    const uint32_t lane_off = (row & ~31u) << 16;                    // ... and this warp's 32 lanes
+    const uint32_t tmem_d0 = *s_tmem + NWG * wg_cols;                // DYN: D slot 0
+    uint32_t tmem_d = tmem_d0;                                       // DYN: the D slot of the current tile
+    // columns of the A operand / the accumulator of a layer of the given parity (warp-uniform, no lane offset)
+    auto col_a = [&](bool odd) -> uint32_t { return DYN ? tmem_wg : tmem_wg + (odd ? 0u : 64u); };
+    auto col_d = [&](bool odd) -> uint32_t { return DYN ? tmem_d : tmem_wg + (odd ? 32u : 0u); };
     const uint32_t w_addr = smem_u32(s_w), bar = smem_u32(&s_bar[wg]);
     const bool rgb_vec = !Q.perm && !Q.out_idx && ((uintptr_t)rgb & 15u) == 0;   // rows in order and the output 16-byte aligned: vector stores
     uint32_t phase = 0;
@@ -127,6 +144,25 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
     // uniform datapath, elect, commit) and every tile waits for it: the five issuing warps sit on different scheduler partitions
     // (warp index mod 4) instead of all on partition 0 (ncu before: issue slots 75 % busy there, 51 % on the other three).
     const bool leader_warp = (row >> 5) == (wg & 3u);
+    // DYN: lane 0 of the issuing warp takes a free D slot (spinning while all are busy: a holder never waits on anyone), tells its own warp
+    // by shuffle and the other three through shared memory (they read it after the barrier that precedes the tile's first MMA)
+    auto acquire_slot = [&]() {
+        uint32_t got = 0;
+        if ((threadIdx.x & 31u) == 0) {
+            got = 0xffffffffu;
+            while (got == 0xffffffffu) {
+                const uint32_t m = *(volatile uint32_t*)s_free;
+                if (m) {
+                    const uint32_t b = (uint32_t)__ffs((int)m) - 1u;
+                    if (atomicAnd(s_free, ~(1u << b)) & (1u << b)) got = b;
+                } else {
+                    __nanosleep(20);
+                }
+            }
+            *(volatile uint32_t*)&s_slot[wg] = got;
+        }
+        tmem_d = tmem_d0 + 64u * __shfl_sync(0xffffffffu, got, 0);
+    };
     constexpr uint32_t idesc_h = instr_desc(128, 64), idesc_o = instr_desc(128, 16);
     const uint32_t tile_stride = gridDim.x * NWG;
 
@@ -155,7 +191,7 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
 #pragma unroll
         for (int k = 0; k < 3; ++k) { x[k] = s_q[k * 128]; w[k] = s_q[(6 + k) * 128]; }
         // ------------------------------------------------------------------ gather: one query per thread -> A0 in TMEM
-        const uint32_t a0 = tmem_lane + 64;                          // layer 0 is even: A at [64, 64 + k1/2)
+        const uint32_t a0 = col_a(false) + lane_off;                 // my row of layer 0's A
         uint64_t dbg_row = 0;
         if constexpr (DBG) {             // where this query's index rows go: its own index (binned queries: out_idx's)
             const uint64_t t = (uint64_t)tile * kRows + row;
@@ -182,7 +218,10 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             }
             if constexpr (KS) {
                 if ((l + 1) * F == 64) {      // inputs 0..63 of all 128 rows are in TMEM: first MMA group of layer 0
-                    uint32_t g_d = tmem_wg, g_a = tmem_wg + 64u;
+                    if constexpr (DYN) {
+                        if (leader_warp) acquire_slot();
+                    }
+                    uint32_t g_d = col_d(false), g_a = col_a(false);
                     uint64_t g_b = smem_desc(w_addr, 1024, 128);
                     if (leader_warp) {           // operand addresses and the weights' arrival ahead of the barrier (see the hidden layers)
                         asm volatile("" : "+r"(g_d), "+r"(g_a), "+l"(g_b));
@@ -194,6 +233,9 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
                     tmem_wait_st();
                     fence_before_sync();
                     named_bar(1 + wg, 128);
+                    if constexpr (DYN) {
+                        if (!leader_warp) tmem_d = tmem_d0 + 64u * *(volatile uint32_t*)&s_slot[wg];
+                    }
                     if (leader_warp) {
                         fence_after_sync();
                         umma_group_ts<4>(g_d, g_a, g_b, 2048 >> 4, idesc_h, 4u, bar);
@@ -277,7 +319,10 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             // The issuing warp forms this layer's operand addresses BEFORE it waits for the other warps' rows (the empty volatile asm pins
             // the values ahead of the barrier): between the barrier and the first tcgen05.mma only the issue itself is left.  Every
             // instruction of that warp there is on the tile's critical path and takes ~9 cycles with five warps sharing a scheduler.
-            uint32_t mma_d = tmem_wg + (odd ? 32u : 0u), mma_a = tmem_wg + (odd ? 0u : 64u);
+            if constexpr (DYN && !KS) {
+                if (layer == 0 && leader_warp) acquire_slot();
+            }
+            uint32_t mma_d = col_d(odd), mma_a = col_a(odd);
             uint64_t mma_b = smem_desc(w_addr + w_off + (second ? 4u * 2048u : 0u), 1024, 128);
             if (leader_warp) {
                 asm volatile("" : "+r"(mma_d), "+r"(mma_a), "+l"(mma_b));
@@ -292,6 +337,9 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
 #ifdef OO_PROFILE_PHASES
             tb += clock64() - tb0;
 #endif
+            if constexpr (DYN && !KS) {
+                if (layer == 0 && !leader_warp) tmem_d = tmem_d0 + 64u * *(volatile uint32_t*)&s_slot[wg];
+            }
             if (leader_warp) {
                 fence_after_sync();
                 umma_group_ts<8>(mma_d, mma_a, mma_b, 2048 >> 4, idesc_h, second ? kt_n - 4u : kt_n, bar, second ? 1u : 0u);
@@ -312,27 +360,18 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
             // epilogue: my row of D -> ReLU -> fp16 -> my row of the next layer's A (over columns of D already read)
             // both halves of D are requested before the single wait::ld, so the second TMEM read hides behind the first
             uint32_t r0[32], r1[32], p[16];
-            if (!odd) {
-                tmem_ld32(tmem_lane, r0);
-                tmem_ld32(tmem_lane + 32, r1);
-                tmem_wait_ld();
-                relu_pack32(r0, p);
-                tmem_st16(tmem_lane, p);
-                relu_pack32(r1, p);
-                tmem_st16(tmem_lane + 16, p);
-            } else {
-                tmem_ld32(tmem_lane + 64, r0);
-                tmem_ld32(tmem_lane + 32, r1);
-                tmem_wait_ld();
-                relu_pack32(r0, p);
-                tmem_st16(tmem_lane + 80, p);
-                relu_pack32(r1, p);
-                tmem_st16(tmem_lane + 64, p);
-            }
+            const uint32_t d_lane = col_d(odd) + lane_off, a_next = col_a(!odd) + lane_off;
+            tmem_ld32(d_lane, r0);                  // outputs 0..31
+            tmem_ld32(d_lane + 32, r1);             // outputs 32..63
+            tmem_wait_ld();                         // the whole row is in registers: the next A may overlap D's columns
+            relu_pack32(r0, p);
+            tmem_st16(a_next, p);
+            relu_pack32(r1, p);
+            tmem_st16(a_next + 16, p);
         }
         // ------------------------------------------------------------------ output layer (N = 16, K = 64)
         const bool odd = n_hidden & 1u;
-        uint32_t out_d = tmem_wg + (odd ? 32u : 0u), out_a = tmem_wg + (odd ? 0u : 64u);
+        uint32_t out_d = col_d(odd), out_a = col_a(odd);
         uint64_t out_b = smem_desc(w_addr + w_off, 256, 128);
         if (leader_warp) asm volatile("" : "+r"(out_d), "+r"(out_a), "+l"(out_b));       // formed ahead of the barrier, as above
         tmem_wait_st();
@@ -346,10 +385,16 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
         phase ^= 1;
         fence_after_sync();
         // the output MMA is N = 16 wide: columns 0..3 always, 4..7 (into the same registers) only for out_dim > 4
-        const uint32_t o_addr = tmem_lane + (odd ? 32u : 0u);
-        uint32_t o[4];
+        const uint32_t o_addr = col_d(odd) + lane_off;
+        uint32_t o[4], o_hi[4];
         tmem_ld4(o_addr, o);
+        if (!SPEC && M.out_dim > 4) tmem_ld4(o_addr + 4, o_hi);
         tmem_wait_ld();
+        if constexpr (DYN) {          // this warp is done with the D slot; the last of the four warps gives it back
+            fence_before_sync();
+            __syncwarp();
+            if ((threadIdx.x & 31u) == 0 && (atomicAdd(&s_rel[wg], 1u) & 3u) == 3u) atomicOr(s_free, 1u << ((tmem_d - tmem_d0) >> 6));
+        }
         if (SPEC || (M.out_dim == 3 && M.out_act == OO_ACT_EXP)) {       // RGB through exp: the case every BASELINE.json config runs
             const float r0 = fast_exp(__uint_as_float(o[0])), r1 = fast_exp(__uint_as_float(o[1])), r2 = fast_exp(__uint_as_float(o[2]));
             // A warp's 32 rows are 384 contiguous bytes of the output when the queries are processed in order: they go through a
@@ -377,13 +422,11 @@ __global__ void __launch_bounds__(NWG * 128, 1) fused_tm_kernel(const __grid_con
                     }
             }
             if (M.out_dim > 4) {
-                tmem_ld4(o_addr + 4, o);
-                tmem_wait_ld();
                 if (valid) {
 #pragma unroll
                     for (uint32_t c = 0; c < 4; ++c)
                         if (4 + c < M.out_dim) {
-                            const float z = __uint_as_float(o[c]);
+                            const float z = __uint_as_float(o_hi[c]);
                             rgb[(size_t)qi * M.out_dim + 4 + c] = M.out_act == OO_ACT_EXP ? fast_exp(z) : z;
                         }
                 }
@@ -423,14 +466,14 @@ static bool ks_applies(const TreeParams& T, const MlpParams& M) {
 #define OO_TM_KS_SHAPES(X) X(4, 16, false) X(5, 16, false) X(6, 16, false) X(7, 16, false) X(8, 8, false)
 
 // one instance with the decoder's shape compiled in (see H, K1, NX above)
-template <int L, int F, int NWG, bool KS, bool DBG, int H, int K1, int NX>
+template <int L, int F, int NWG, bool KS, bool DBG, int H, int K1, int NX, int NSLOT = NWG>
 static int launch_tm_spec(const TreeParams& T, const MlpParams& M, const QueryParams& Q, float* rgb, int n_sms, uint32_t wg_cols, cudaStream_t stream) {
     const uint64_t n_tiles = (Q.n + kRows - 1) / kRows;
     const unsigned grid = (unsigned)(n_tiles < (uint64_t)n_sms ? n_tiles : (uint64_t)n_sms);
-    const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + NWG * (10 + Q.n_extra) * kRows * 4 + NWG * 4 * 96 * 4 + 128;
+    const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + NWG * (10 + Q.n_extra) * kRows * 4 + NWG * 4 * 96 * 4 + 256;
     if (smem > 227 * 1024) return -1;
     static std::atomic<uint64_t> opted{0};
-    auto kern = fused_tm_kernel<L, F, false, NWG, true, KS, DBG, H, K1, NX>;
+    auto kern = fused_tm_kernel<L, F, false, NWG, true, KS, DBG, H, K1, NX, NSLOT>;
     if (!opt_in_smem(opted, (const void*)kern, 227 * 1024)) return kLaunchCudaError;
     kern<<<grid, NWG * 128, smem, stream>>>(T, M, Q, rgb, (uint32_t)n_tiles, wg_cols);
     return 1;
@@ -443,7 +486,7 @@ static int launch_tm_variant(const TreeParams& T, const MlpParams& M, const Quer
     // one block per SM as soon as there is a tile for each: a small batch spreads over all SMs (a warpgroup alone on its SM
     // finishes a tile faster than four sharing one) instead of filling every warpgroup of the first n_tiles / NWG SMs
     const unsigned grid = (unsigned)(n_tiles < (uint64_t)n_sms ? n_tiles : (uint64_t)n_sms);
-    const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + NWG * (10 + Q.n_extra) * kRows * 4 + NWG * 4 * 96 * 4 + 128;
+    const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + NWG * (10 + Q.n_extra) * kRows * 4 + NWG * 4 * 96 * 4 + 256;
     if (smem > 227 * 1024) return -1;
 #define X(l, f, t)                                                                                                     \
     if (T.n_levels == l && T.F == f && (T.f32 != 0) == t) {                                                            \
@@ -474,9 +517,19 @@ static int launch_fused_tm_impl(const TreeParams& T, const MlpParams& M, const Q
     const bool pipe = pipe_applies(T);
     // the BASELINE.json configs: decoder shape compiled in (configs 1, 2: 38/39 -> 3 x 64 -> 3 exp on L = 4, F = 8; configs 3, 4: 86 -> 4 x 64 -> 3 exp on L = 5, F = 16)
     if (pipe && M.out_dim == 3 && M.out_act == OO_ACT_EXP && !T.f32) {
-        if (T.n_levels == 4 && T.F == 8 && M.n_hidden == 3 && M.k1 == 48 && Q.n_extra == 0) return launch_tm_spec<4, 8, 5, false, DBG, 3, 48, 0>(T, M, Q, rgb, n_sms, 96, stream);
-        if (T.n_levels == 4 && T.F == 8 && M.n_hidden == 3 && M.k1 == 48 && Q.n_extra == 1) return launch_tm_spec<4, 8, 5, false, DBG, 3, 48, 1>(T, M, Q, rgb, n_sms, 96, stream);
-        if (T.n_levels == 5 && T.F == 16 && M.n_hidden == 4 && M.k1 == 96 && Q.n_extra == 0) return launch_tm_spec<5, 16, 5, true, DBG, 4, 96, 0>(T, M, Q, rgb, n_sms, 96, stream);
+        // warpgroups x accumulator slots (see NSLOT).  Measured on B200: config 1 5x5 / 6x5 / 7x4 = 48.9 / 52.3 / 45.8 us (72 registers and no spills
+        // at 7x4), config 3 244.6 / 236.9 / 291.7 us (7x4 spills there).  Below ~2^19 queries the shared slots lose 1-2 us (all warpgroups reach their
+        // first MMA together and queue for the slots; there is no steady state to amortise it), so small batches keep one slot per warpgroup.
+        const bool shared_slots = (Q.n + kRows - 1) / kRows >= 4096;
+        if (T.n_levels == 4 && T.F == 8 && M.n_hidden == 3 && M.k1 == 48 && Q.n_extra == 0)
+            return shared_slots ? launch_tm_spec<4, 8, 7, false, DBG, 3, 48, 0, 4>(T, M, Q, rgb, n_sms, 32, stream)
+                                : launch_tm_spec<4, 8, 5, false, DBG, 3, 48, 0>(T, M, Q, rgb, n_sms, 96, stream);
+        if (T.n_levels == 4 && T.F == 8 && M.n_hidden == 3 && M.k1 == 48 && Q.n_extra == 1)
+            return shared_slots ? launch_tm_spec<4, 8, 7, false, DBG, 3, 48, 1, 4>(T, M, Q, rgb, n_sms, 32, stream)
+                                : launch_tm_spec<4, 8, 5, false, DBG, 3, 48, 1>(T, M, Q, rgb, n_sms, 96, stream);
+        if (T.n_levels == 5 && T.F == 16 && M.n_hidden == 4 && M.k1 == 96 && Q.n_extra == 0)
+            return shared_slots ? launch_tm_spec<5, 16, 6, true, DBG, 4, 96, 0, 5>(T, M, Q, rgb, n_sms, 32, stream)
+                                : launch_tm_spec<5, 16, 5, true, DBG, 4, 96, 0>(T, M, Q, rgb, n_sms, 96, stream);
     }
     if (ks_applies(T, M)) {      // 96 columns per tile: five warpgroups
         const int n = pipe ? launch_tm_variant<5, true, true, DBG>(T, M, Q, rgb, n_sms, 96, stream)
