@@ -19,7 +19,11 @@
 
 namespace oo {
 
-template <int F, bool F32, bool VERTEX, bool TRI8, bool SHIFTED, int W, int KS, int NTEAM, bool DBG>
+// NSLOT < NTEAM: the accumulators are shared as in fused_tm_kernel (oo_fused_tm.cuh).  A team owns an A region of team_cols = max(W/2, k1/2)
+// columns; D (W columns) lives in one of NSLOT slots taken before the tile's first MMA and given back when its output has been read:
+// A of team t at [t * team_cols, +team_cols), D slot s at [NTEAM * team_cols + W * s, +W).  The full query spends three quarters of a tile
+// in its gather, so four one-part teams share two slots (4 x 64 + 2 x 128 = 512 columns) and no thread walks a descent it does not gather from.
+template <int F, bool F32, bool VERTEX, bool TRI8, bool SHIFTED, int W, int KS, int NTEAM, bool DBG, int NSLOT = NTEAM>
 __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
     fused_full_kernel(const __grid_constant__ TreeParams T, const __grid_constant__ MlpParams M,
                       const __grid_constant__ QueryParams Q, const __grid_constant__ FullMode mode, float* __restrict__ rgb,
@@ -37,6 +41,10 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
     uint8_t* s_stage = s_w + ((M.image_tc_bytes + 127) & ~127u);
     uint64_t* s_bar = (uint64_t*)(s_stage + NTEAM * q_bytes);
     uint32_t* s_tmem = (uint32_t*)(s_bar + NTEAM);
+    constexpr bool DYN = NSLOT < NTEAM;
+    uint32_t* s_free = s_tmem + 1;                               // DYN: bit s set = D slot s is free
+    uint32_t* s_slot = s_free + 1;                               // [NTEAM] the slot a team's tile holds
+    uint32_t* s_rel = s_slot + NTEAM;                            // [NTEAM] warps of part 0 that are done with the slot
 
     const uint32_t team = threadIdx.x / TEAM_THREADS, part = (threadIdx.x >> 7) % KS, row = threadIdx.x & 127,
                    warp = threadIdx.x >> 5;
@@ -48,7 +56,11 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
         d = (uint4*)s_w;
         for (uint32_t i = threadIdx.x; i < M.image_tc_bytes / 16; i += blockDim.x) d[i] = __ldg(s + i);
     }
-    if (threadIdx.x < NTEAM) mbar_init(smem_u32(&s_bar[threadIdx.x]), 1);
+    if (threadIdx.x < NTEAM) {
+        mbar_init(smem_u32(&s_bar[threadIdx.x]), 1);
+        s_rel[threadIdx.x] = 0;
+    }
+    if (threadIdx.x == 0) *s_free = (1u << NSLOT) - 1u;
     if (threadIdx.x == 0) asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     if (warp == 0) {
         tmem_alloc(smem_u32(s_tmem), 512);
@@ -59,7 +71,12 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
     __syncthreads();
     fence_after_sync();
     const uint32_t tmem_team = *s_tmem + team * team_cols;
-    const uint32_t tmem_lane = tmem_team + ((row & ~31u) << 16);
+    const uint32_t lane_off = (row & ~31u) << 16;
+    const uint32_t tmem_d0 = *s_tmem + NTEAM * team_cols;            // DYN: D slot 0
+    uint32_t tmem_d = tmem_d0;                                       // DYN: the D slot of the current tile
+    // columns of the A operand / the accumulator of a layer of the given parity (warp-uniform)
+    auto col_a = [&](bool odd) -> uint32_t { return DYN ? tmem_team : tmem_team + (odd ? 0u : (uint32_t)W); };
+    auto col_d = [&](bool odd) -> uint32_t { return DYN ? tmem_d : tmem_team + (odd ? (uint32_t)(W / 2) : 0u); };
     float* s_q = (float*)(s_stage + team * q_bytes) + row;            // word k of my row: s_q[k * 128]
     const uint32_t w_addr = smem_u32(s_w), bar = smem_u32(&s_bar[team]), q_addr = smem_u32(s_q);
     uint32_t phase = 0;
@@ -112,7 +129,7 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
         OctaUV uv{0.0f, 0.0f};
         if constexpr (!SHIFTED) uv = octa_project(wl[0], wl[1], wl[2]);
         // ------------------------------------------------------------------ gather -> A0 in TMEM (layer 0 is even)
-        const uint32_t a0 = tmem_lane + W;
+        const uint32_t a0 = col_a(false) + lane_off;
         {
             Station<NJ> st;
             station_init<NJ>(T, s_dense, x, st);
@@ -172,12 +189,34 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
             const bool odd = layer & 1u;
             // the issuing warp forms the layer's operand addresses ahead of the barrier (see oo_fused_tm.cuh): between the barrier and the
             // first tcgen05.mma only the issue itself is left on the tile's critical path
-            uint32_t mma_d = tmem_team + (odd ? (uint32_t)(W / 2) : 0u), mma_a = tmem_team + (odd ? 0u : (uint32_t)W);
+            if constexpr (DYN) {
+                if (layer == 0 && leader_warp) {      // lane 0 takes a free D slot (see fused_tm_kernel) and tells its warp and the team
+                    uint32_t got = 0;
+                    if ((threadIdx.x & 31u) == 0) {
+                        got = 0xffffffffu;
+                        while (got == 0xffffffffu) {
+                            const uint32_t m = *(volatile uint32_t*)s_free;
+                            if (m) {
+                                const uint32_t b = (uint32_t)__ffs((int)m) - 1u;
+                                if (atomicAnd(s_free, ~(1u << b)) & (1u << b)) got = b;
+                            } else {
+                                __nanosleep(20);
+                            }
+                        }
+                        *(volatile uint32_t*)&s_slot[team] = got;
+                    }
+                    tmem_d = tmem_d0 + (uint32_t)W * __shfl_sync(0xffffffffu, got, 0);
+                }
+            }
+            uint32_t mma_d = col_d(odd), mma_a = col_a(odd);
             uint64_t mma_b = smem_desc(w_addr + w_off, 16 * W, 128);
             if (leader_warp) asm volatile("" : "+r"(mma_d), "+r"(mma_a), "+l"(mma_b));
             tmem_wait_st();              // my part of A is in TMEM
             fence_before_sync();
             named_bar(1 + team, TEAM_THREADS);
+            if constexpr (DYN) {
+                if (layer == 0 && !leader_warp) tmem_d = tmem_d0 + (uint32_t)W * *(volatile uint32_t*)&s_slot[team];
+            }
             if (leader_warp) {
                 fence_after_sync();
                 umma_group_ts<8>(mma_d, mma_a, mma_b, (32 * W) >> 4, idesc_h, kt_n, bar);
@@ -188,8 +227,8 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
             phase ^= 1;
             fence_after_sync();
             // epilogue: my row of D -> ReLU -> fp16 -> my row of the next layer's A (over columns of D already read)
-            const uint32_t d_base = tmem_lane + (odd ? (uint32_t)(W / 2) : 0u);
-            const uint32_t a_base = tmem_lane + (odd ? (uint32_t)W : 0u);
+            const uint32_t d_base = col_d(odd) + lane_off;
+            const uint32_t a_base = col_a(!odd) + lane_off;
             if constexpr (KS == 1) {
 #pragma unroll
                 for (int i = 0; i < NCHUNK; ++i) {
@@ -226,7 +265,7 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
         }
         // ------------------------------------------------------------------ output layer (N = 16, K = W)
         const bool odd = M.n_hidden & 1u;
-        uint32_t out_d = tmem_team + (odd ? (uint32_t)(W / 2) : 0u), out_a = tmem_team + (odd ? 0u : (uint32_t)W);
+        uint32_t out_d = col_d(odd), out_a = col_a(odd);
         uint64_t out_b = smem_desc(w_addr + w_off, 256, 128);
         if (leader_warp) asm volatile("" : "+r"(out_d), "+r"(out_a), "+l"(out_b));
         tmem_wait_st();
@@ -241,8 +280,13 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
         fence_after_sync();
         if (part == 0) {
             uint32_t o[4];
-            tmem_ld4(tmem_lane + (odd ? (uint32_t)(W / 2) : 0u), o);
+            tmem_ld4(col_d(odd) + lane_off, o);
             tmem_wait_ld();
+            if constexpr (DYN) {      // part 0's four warps are the last readers of the slot
+                fence_before_sync();
+                __syncwarp();
+                if ((threadIdx.x & 31u) == 0 && (atomicAdd(&s_rel[team], 1u) & 3u) == 3u) atomicOr(s_free, 1u << ((tmem_d - tmem_d0) / (uint32_t)W));
+            }
             if (valid) {
 #pragma unroll
                 for (uint32_t c = 0; c < 4; ++c)
@@ -262,15 +306,15 @@ __global__ void __launch_bounds__(NTEAM* KS * 128, 1)
 }
 
 // ---------------------------------------------------------------------------------------------------------------------
-template <int F, bool F32, bool VERTEX, bool TRI8, bool SHIFTED, int W, int KS, int NTEAM, bool DBG>
+template <int F, bool F32, bool VERTEX, bool TRI8, bool SHIFTED, int W, int KS, int NTEAM, bool DBG, int NSLOT = NTEAM>
 static int launch_full_inst(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const FullModeH& mode, float* rgb,
                             int n_sms, uint32_t team_cols, cudaStream_t stream) {
     const uint64_t n_tiles = (Q.n + 127) / 128;
     const uint64_t blocks = (n_tiles + NTEAM - 1) / NTEAM;
     const unsigned grid = (unsigned)(blocks < (uint64_t)n_sms ? blocks : (uint64_t)n_sms);
-    const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + NTEAM * (11 + Q.n_extra) * 128 * 4 + 128;
+    const uint32_t smem = ((T.dense_ints * 4 + 127) & ~127u) + ((M.image_tc_bytes + 127) & ~127u) + NTEAM * (11 + Q.n_extra) * 128 * 4 + 256;
     if (smem > 227 * 1024) return -1;
-    auto kern = fused_full_kernel<F, F32, VERTEX, TRI8, SHIFTED, W, KS, NTEAM, DBG>;
+    auto kern = fused_full_kernel<F, F32, VERTEX, TRI8, SHIFTED, W, KS, NTEAM, DBG, NSLOT>;
     static std::atomic<uint64_t> opted{0};
     if (!opt_in_smem(opted, (const void*)kern, 227 * 1024)) return kLaunchCudaError;
     kern<<<grid, NTEAM * KS * 128, smem, stream>>>(T, M, Q, mode, rgb, (uint32_t)n_tiles, team_cols);
@@ -282,13 +326,13 @@ static int launch_full_inst(const TreeParams& T, const MlpParams& M, const Query
     X(f, t, true, false, false) X(f, t, true, false, true) X(f, t, true, true, false) X(f, t, true, true, true)
 
 // dispatch over (F, dtype, vertex, tri8, shifted) for a fixed (W, KS, NTEAM)
-template <int W, int KS, int NTEAM, bool DBG>
+template <int W, int KS, int NTEAM, bool DBG, int NSLOT = NTEAM>
 static int launch_full_w(const TreeParams& T, const MlpParams& M, const QueryParams& Q, const FullModeH& mode, float* rgb,
                          int n_sms, uint32_t team_cols, cudaStream_t stream) {
     const bool vertex = T.vertex != 0, tri8 = mode.tri8 != 0, shifted = mode.lookup == OO_LOOKUP_SHIFTED;
 #define X(f, t, v, s8, sh)                                                                                 \
     if (T.F == f && (T.f32 != 0) == t && vertex == v && tri8 == s8 && shifted == sh)                       \
-        return launch_full_inst<f, t, v, s8, sh, W, KS, NTEAM, DBG>(T, M, Q, mode, rgb, n_sms, team_cols, stream);
+        return launch_full_inst<f, t, v, s8, sh, W, KS, NTEAM, DBG, NSLOT>(T, M, Q, mode, rgb, n_sms, team_cols, stream);
     OO_FULL_MODES(X, 4, true)
     OO_FULL_MODES(X, 8, false)
     OO_FULL_MODES(X, 16, false)
