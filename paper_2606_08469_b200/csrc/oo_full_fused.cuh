@@ -3,7 +3,8 @@
 //
 // Same skeleton as oo_fused_tm.cu (A operand of every layer in TMEM, weights in shared memory, accumulator in TMEM, the
 // epilogue writes the next A over accumulator columns already read), generalised in two directions:
-//   * W = 128: D is 128 columns and A 64, so a tile needs 192 TMEM columns and only TWO tiles fit an SM.  To keep the
+//   * W = 128: D is 128 columns and A 64, so a tile with an accumulator of its own needs 192 TMEM columns and only TWO fit an SM.
+//     Either the accumulators are shared (NSLOT < NTEAM, below: the product form, four one-part teams over two slots), or, to keep the
 //     gather phase populated, a tile is worked by a TEAM of KS x 128 threads: part p of the team gathers the levels
 //     l = p (mod KS) of the same 128 queries (levels are independent channels, Eq. 11) and writes them to its rows of A
 //     (a warp may touch TMEM lanes 32*(warp%4)..+32, so part p's warp 4p+i shares lanes with warp i); the epilogue's
