@@ -41,6 +41,7 @@
 #ifndef OO_H_
 #define OO_H_
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -269,6 +270,29 @@ OO_API oo_status oo_set_mode(oo_ctx* ctx, const oo_mode* mode);
  * clamp(floor(x*1024), 0, 1023) (bit b of q_x -> key bit 3b, q_y -> 3b+1, q_z -> 3b+2), ties in original order
  * (stable).  d_perm_out: DEVICE [n].  Needs oo_reserve(n). */
 OO_API oo_status oo_sort_queries(oo_ctx* ctx, const oo_queries* q, uint32_t* d_perm_out, void* cuda_stream);
+
+/* Row a1 for callers that cannot allocate device memory.  Same result as oo_sort_queries (same kernels, same unique stable
+ * permutation), but it needs no context, no oo_reserve and no cudaMalloc, cudaFree or allocating library routine, on any call:
+ * its scratch is an array built into the library image.  It is meant for code that runs after an application has frozen its
+ * memory budget, inside a host program that owns the device heap, or on a latency-critical thread where an allocation's
+ * device-wide synchronisation is not acceptable.
+ *   d_x         DEVICE [n][3] packed fp32 positions, read-only; d_perm_out DEVICE [n] uint32.  Both belong to the calling
+ *               thread's CURRENT CUDA device, which is the device the call runs on.
+ *   n           at most OO_SORT_STATIC_MAX_QUERIES; more returns OO_ERR_UNSUPPORTED and launches nothing (use oo_sort_queries).
+ *   cuda_stream a cudaStream_t of that device (NULL = legacy default stream); kernels are enqueued, the call does not wait.
+ *   err_msg     optional HOST buffer of err_cap bytes that receives a NUL-terminated description when the status is not
+ *               OO_OK (emptied on success); NULL / 0 = status code only.
+ * Cost: each GPU on which the call is made holds the scratch, 13,643,776 bytes, from its first call until the process exits.
+ * First call on a device: it looks up the array's device address (cudaGetSymbolAddress) before it launches, which also makes
+ * the CUDA runtime load that part of the library onto the device.  Make that first call (n = 0 is enough, and launches nothing)
+ * during start-up, before any stream capture begins on that device; later calls only clear 12 KB and launch 9 kernels.
+ * All calls a process makes on one device share the one array, and it keeps the previous call's contents (the call clears the
+ * part that must start at zero itself).  Two such calls whose kernels can overlap on the GPU - issued to different streams
+ * with no event between them, for instance from two host threads - race on the array and both permutations are garbage:
+ * order the calls on one stream or with events.  (Another process has its own copy of the array.) */
+#define OO_SORT_STATIC_MAX_QUERIES 1048576u   /* one 1024 x 1024 frame */
+OO_API oo_status oo_sort_queries_static(const float* d_x, uint64_t n, uint32_t* d_perm_out, void* cuda_stream, char* err_msg,
+                                        size_t err_cap);
 
 /* Steps 1-3 only.  d_features: DEVICE [n][L*F] in the tree's dtype (fp32 accumulate, one rounding on store).
  * Optional debug outputs: d_slot DEVICE [n][L] (atlas slot per level, -1 = no cell at that level, whose features are

@@ -20,7 +20,7 @@ _STATUS = {0: "OO_OK", 1: "OO_ERR_INVALID_ARG", 2: "OO_ERR_NOT_READY", 3: "OO_ER
 EXPORTED_SYMBOLS = ["oo_create", "oo_destroy", "oo_last_error", "oo_upload_tree", "oo_upload_mlp", "oo_reserve", "oo_set_path",
                     "oo_get_info", "oo_sort_queries", "oo_encode", "oo_query", "oo_query_host", "oo_read_padded_map", "oo_set_mode",
                     "oo_encode_full", "oo_upload_scene", "oo_raycast", "oo_upload_disparity", "oo_predict_disparity", "oo_set_presort",
-                    "oo_query_debug", "oo_set_host_chunks", "oo_last_note", "oo_set_host_zero_copy"]
+                    "oo_query_debug", "oo_set_host_chunks", "oo_last_note", "oo_set_host_zero_copy", "oo_sort_queries_static"]
 
 
 class OOError(RuntimeError):
@@ -106,6 +106,7 @@ def load_library():
     L.oo_get_info.argtypes = [vp, C.POINTER(_Info)]
     L.oo_set_presort.argtypes = [vp, C.c_int, u64]
     L.oo_sort_queries.argtypes = [vp, C.POINTER(_Queries), vp, vp]
+    L.oo_sort_queries_static.argtypes = [vp, u64, vp, vp, C.c_char_p, C.c_size_t]
     L.oo_encode.argtypes = [vp, C.POINTER(_Queries), vp, vp, vp, vp]
     L.oo_query.argtypes = [vp, C.POINTER(_Queries), vp, vp]
     L.oo_query_host.argtypes = [vp, C.POINTER(_Queries), vp, vp]
@@ -125,6 +126,32 @@ def load_library():
 
 def _np_ptr(a):
     return a.ctypes.data_as(C.c_void_p)
+
+
+SORT_STATIC_MAX_QUERIES = 1 << 20      # OO_SORT_STATIC_MAX_QUERIES
+
+
+def oo_sort_queries_static(x, perm_out=None):
+    """Morton order of the positions `x` (CUDA fp32 tensor [n][3]) without any device allocation inside the library: the variant
+    of `OctaOctree.oo_sort_queries` for callers that cannot allocate (fixed memory budget after start-up, a host application that
+    owns the device heap, a latency-critical thread).  Needs no context and no oo_reserve; at most SORT_STATIC_MAX_QUERIES
+    positions, more raises OOError(OO_ERR_UNSUPPORTED).  Runs on x's device and on torch's current stream for it.  Pass
+    `perm_out` (int32/uint32 CUDA tensor [n]) to keep this wrapper from allocating the result as well.  Calls share one
+    built-in scratch array per device: do not let two of them overlap on the GPU (see include/oo.h)."""
+    import torch  # device memory and streams only
+    L = load_library()
+    assert x.is_cuda and x.is_contiguous() and x.dtype == torch.float32, "x must be a contiguous fp32 CUDA tensor"
+    n = int(x.shape[0])
+    if perm_out is None:
+        perm_out = torch.empty(n, dtype=torch.int32, device=x.device)
+    assert perm_out.is_cuda and perm_out.is_contiguous() and perm_out.element_size() == 4 and perm_out.numel() >= n
+    err = C.create_string_buffer(256)
+    with torch.cuda.device(x.device):      # the entry point works on the calling thread's current device
+        st = L.oo_sort_queries_static(C.c_void_p(x.data_ptr()), n, C.c_void_p(perm_out.data_ptr()),
+                                      C.c_void_p(torch.cuda.current_stream(x.device).cuda_stream), err, len(err))
+    if st:
+        raise OOError(st, err.value.decode())
+    return perm_out
 
 
 class OctaOctree:

@@ -13,7 +13,7 @@ BUILD = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "liboo.so")
 SOURCES = ["oo_api.cu", "oo_kernels.cu", "oo_fused_tc.cu", "oo_fused_tm.cu", "oo_fused_tm_dbg.cu", "oo_sort.cu",
            "oo_full_encode.cu", "oo_full_fused_w64.cu", "oo_full_fused_w128.cu", "oo_full_fused_w64_dbg.cu",
-           "oo_full_fused_w128_dbg.cu", "oo_raycast.cu", "oo_disparity.cu"]
+           "oo_full_fused_w128_dbg.cu", "oo_raycast.cu", "oo_disparity.cu", "oo_sort_static.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-Xcompiler", "-fPIC",
               "-Xcompiler", "-fvisibility=hidden", "-I", os.path.join(ROOT, "include"), "-I", CSRC] + os.environ.get("OO_NVCC_EXTRA", "").split()
 
