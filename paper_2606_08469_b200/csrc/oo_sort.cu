@@ -426,7 +426,8 @@ __global__ void __launch_bounds__(256) unbin_kernel(const float* __restrict__ bi
 }
 
 // bin_tot: kDigits ints that are ZERO on entry (the caller clears them once when it allocates them; the scatter kernel of every
-// call clears them again after the scan has consumed them, so no call needs a memset of its own)
+// call clears them again after the scan has consumed them, so no call needs a memset of its own; a call whose scan or scatter
+// launch is rejected restores the zeros with a memset before it reports the failure)
 int launch_bin_queries(const QueryParams& Q, uint32_t* keys, uint32_t* hist, uint32_t* bin_tot, float* sx, float* sn, float* sw, float* se,
                        uint32_t* inv, uint32_t* idx, float* sdisp, cudaStream_t stream) {
     if (Q.n == 0) return 0;
@@ -435,9 +436,21 @@ int launch_bin_queries(const QueryParams& Q, uint32_t* keys, uint32_t* hist, uin
     const uint32_t n_tiles = (uint32_t)((Q.n + kTile - 1) / kTile);
     constexpr uint32_t shift = 30 - kBits;
     bin_hist_kernel<<<n_tiles, 1024, 0, stream>>>(Q.x, keys, Q.n, n_tiles, hist, bin_tot, Q.stat, Q.stat_seq);
+    if (cudaPeekAtLastError() != cudaSuccess) return kLaunchCudaError;      // nothing was enqueued: the totals are still zero
     scan_kernel<<<kDigits, kSortThreads, 0, stream>>>(hist, bin_tot, n_tiles);
-    const BinPayload B{Q.x, Q.nrm, Q.wo, Q.extra, Q.extra ? Q.n_extra : 0u, sx, sn, sw, se, idx, sdisp ? Q.disparity : nullptr, sdisp};
-    bin_scatter_kernel<<<n_tiles, kBinThreads, kBinSmemBytes, stream>>>(keys, Q.n, shift, n_tiles, hist, B, inv, bin_tot);
+    bool rejected = cudaPeekAtLastError() != cudaSuccess;
+    if (!rejected) {
+        const BinPayload B{Q.x, Q.nrm, Q.wo, Q.extra, Q.extra ? Q.n_extra : 0u, sx, sn, sw, se, idx, sdisp ? Q.disparity : nullptr, sdisp};
+        bin_scatter_kernel<<<n_tiles, kBinThreads, kBinSmemBytes, stream>>>(keys, Q.n, shift, n_tiles, hist, B, inv, bin_tot);
+        rejected = cudaPeekAtLastError() != cudaSuccess;
+    }
+    if (rejected) {
+        // the counting kernel is enqueued and will add this call's counts to bin_tot, but the kernel that clears them is not:
+        // clear them behind it, or every later binned call on this context would scan stale totals and scatter out of bounds.
+        // (The rejected launch's error stays pending for the caller's report: a call that succeeds does not reset it.)
+        cudaMemsetAsync(bin_tot, 0, sizeof(uint32_t) * kDigits, stream);
+        return kLaunchCudaError;
+    }
     return 3;
 }
 
