@@ -1,5 +1,5 @@
 // oo_full_fused_w128_dbg.cu — the debug (oo_query_debug: index sink compiled in) instances of the fused full-query kernel (oo_full_fused.cuh) for decoders of width 128:
-// four teams of 128 threads (tiles in flight) per SM sharing two accumulator slots; wider first layers: teams of 2 x 128 threads, 2 teams.
+// four teams of 128 threads (tiles in flight) per SM sharing two accumulator slots.  First layers wider than 128 inputs have no instance.
 // A translation unit of its own so that the product instances are neither recompiled nor perturbed.
 #include "oo_full_fused.cuh"
 
@@ -9,12 +9,9 @@ int launch_fused_full_w128_dbg(const TreeParams& T, const MlpParams& M, const Qu
             int n_sms, cudaStream_t stream) {
     if (Q.n == 0) return 0;
     if (M.out_dim > 4 || !M.image_tc || M.k1 > 128 || M.width != 128) return -1;
-    const uint32_t team_cols = 128 + (M.k1 / 2 > 128 / 2 ? M.k1 / 2 : 128 / 2);
-    if (2 * team_cols > 512) return -1;
     // four one-part teams over two accumulator slots (oo_full_fused.cuh, NSLOT): 4 x 64 A columns + 2 x 128 D columns.  Measured on B200 at the
     // paper's shapes against two teams of two parts with a slot each: 0.552 -> 0.456 ms (no shift 0.373 -> 0.283, nearest cell 0.250 -> 0.193).
-    if (M.k1 <= 128) return launch_full_w<128, 1, 4, true, 2>(T, M, Q, mode, rgb, n_sms, 64, stream);
-    return launch_full_w<128, 2, 2, true>(T, M, Q, mode, rgb, n_sms, team_cols, stream);
+    return launch_full_w<128, 1, 4, true, 2>(T, M, Q, mode, rgb, n_sms, 64, stream);
 }
 
 }  // namespace oo
