@@ -556,6 +556,21 @@ def run_ours(args):
         dt, threads = time_oracle(w, sample_q, repeats=3)
         sample_desc += "; best of 3"
         out["cpu_baseline"] = {"value": sample_q.n / dt / 1e6, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample_desc}
+    # `frac` stays what the bench contract defines (algorithmic bytes / measured HBM peak) and can exceed 1 on a coherent frame, where
+    # it is not a bound.  Beside it: the same number under an explicit name, and the tightest bound that does hold for this launch --
+    # the largest of the times the compulsory bytes, the measured DRAM bytes, the issue slots and the MLP FLOPs need -- over the measured time.
+    cand = {"mlp_flops": flop_time * 1e3}
+    if isinstance(roof.get("compulsory"), dict) and "byte_time_ms" in roof["compulsory"]:
+        cand["compulsory_bytes"] = roof["compulsory"]["byte_time_ms"]
+    if "dram" in roof:
+        cand["measured_dram_bytes"] = roof["dram"]["bytes_per_launch"] / (hbm * 1e9) * 1e3
+    if "issue" in roof:
+        cand["issue_slots"] = roof["issue"]["bound_ms"]
+    tight = max(cand, key=cand.get)
+    roof["frac_algorithmic"] = roof["frac"]
+    roof["frac_tightest_bound"] = {"bound": tight, "bound_ms": cand[tight], "frac": cand[tight] / mean_ms, "candidates_ms": cand,
+                                   "note": "a real lower bound on this launch's time over the measured time (<= 1 by construction); read this, "
+                                           "not `frac`, when `frac` is above 1"}
     print(json.dumps(out))
     if world > 1:
         torch.distributed.destroy_process_group()
