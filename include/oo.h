@@ -135,7 +135,10 @@ typedef enum {
  *   event record -- and bins when the mean exceeds 12 (and stops below 6).  The decision therefore lags one call: the first
  *   incoherent batch of a stream runs unsorted.  Without reserved scratch AUTO proceeds unsorted instead of failing.  The
  *   result bytes never depend on the decision.  oo_info.presort_auto_on / coherence_x100 report it.  Sampled by: the fused
- *   tensor-memory kernel, the histogram pass of a binned call, oo_encode's specialised kernel, the full-query kernel. */
+ *   tensor-memory kernel, the histogram pass of a binned call, oo_encode's specialised kernel, the full-query kernel.
+ *   CUDA graphs: a call made while its stream is being captured enqueues its kernels only (no event, no side-stream copy),
+ *   so the capture ends cleanly; the captured graph contains the decision that was current at capture time and replays
+ *   never change it.  Make one ordinary call of the same shape before capturing (first launches configure the kernels). */
 typedef enum { OO_PRESORT_NONE = 0, OO_PRESORT_BIN = 1, OO_PRESORT_AUTO = 2 } oo_presort;
 
 /* The octree and its feature atlases ("every non-empty cell stores a learnable octahedral feature map").

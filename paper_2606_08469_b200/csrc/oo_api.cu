@@ -424,9 +424,13 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
     c->atlas_dev.assign(L, nullptr);
     uint64_t atlas_bytes = 0;
     int launches = 0;
-    unsigned long long* d_changed = nullptr;      // vertex maps: number of boundary vertices the tying rewrote
+    // vertex maps: number of boundary vertices the tying rewrote.  Freed on EVERY way out of this function (the early returns
+    // below included: a failed upload on a usable context must not leave device memory behind).
+    struct FreeAtExit { void* p = nullptr; ~FreeAtExit() { if (p) cudaFree(p); } } changed_owner;
+    unsigned long long* d_changed = nullptr;
     if (vertex) {
-        OO_CUDA(c, cudaMalloc((void**)&d_changed, sizeof(unsigned long long)));
+        OO_CUDA(c, cudaMalloc(&changed_owner.p, sizeof(unsigned long long)));
+        d_changed = (unsigned long long*)changed_owner.p;
         OO_CUDA(c, cudaMemsetAsync(d_changed, 0, sizeof(unsigned long long), stream));
     }
     for (uint32_t l = 0; l < L; ++l) {
@@ -581,7 +585,6 @@ extern "C" OO_API oo_status oo_upload_tree(oo_ctx* c, const oo_tree_desc* t, voi
         unsigned long long h = 0;
         const cudaError_t e = cudaMemcpyAsync(&h, d_changed, sizeof h, cudaMemcpyDeviceToHost, stream);
         const cudaError_t e2 = e == cudaSuccess ? cudaStreamSynchronize(stream) : e;
-        cudaFree(d_changed);
         OO_CUDA(c, e2);
         c->info.tied_vertices = h;
     }
@@ -851,9 +854,16 @@ static void arm_sampling(oo_ctx* c, QueryParams& Q) {
 }
 // After the kernels of a sampling call have been enqueued on the caller's stream: the side stream waits for them and copies the
 // sample array to the host.  Nothing is added to the caller's stream but an event record; failures only lose the sample.
+// While the caller's stream is being CAPTURED into a CUDA graph the copy is left out: waiting on an event recorded in a capturing
+// stream would pull the side stream into the capture, where it never rejoins (cudaStreamEndCapture then fails with
+// cudaErrorStreamCaptureUnjoined).  The kernels still write their samples to the device array, which is harmless; a replayed
+// graph repeats the decision that was current when it was captured.
 static void collect_samples(oo_ctx* c, cudaStream_t stream) {
     if (!c->armed) return;
     c->armed = false;
+    cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(stream, &cap) != cudaSuccess) { (void)cudaGetLastError(); return; }
+    if (cap != cudaStreamCaptureStatusNone) return;
     if (cudaEventRecord(c->ev_stat, stream) != cudaSuccess || cudaStreamWaitEvent(c->s_stat, c->ev_stat, 0) != cudaSuccess ||
         cudaMemcpyAsync(c->h_stat, c->d_stat, kStatSlots * sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->s_stat) != cudaSuccess)
         (void)cudaGetLastError();
@@ -1335,7 +1345,7 @@ extern "C" OO_API oo_status oo_read_padded_map(oo_ctx* c, uint32_t level, uint32
     if (!c) return OO_ERR_INVALID_ARG;
     if (!c->have_tree) return fail(c, OO_ERR_NOT_READY, "no tree uploaded");
     if (level >= c->T.n_levels || slot >= c->level_slots[level] || !h_out) return fail(c, OO_ERR_INVALID_ARG, "bad level/slot/pointer");
-    if (c->T.vertex) return fail(c, OO_ERR_UNSUPPORTED, "vertex maps are stored as given (no padded copy)");
+    if (c->T.vertex) return fail(c, OO_ERR_UNSUPPORTED, "vertex maps have no padded copy (they are stored unpadded, their seam tied at upload)");
     DeviceGuard g(c->device);
     const LevelParams& lv = c->T.lv[level];
     OO_CUDA(c, cudaMemcpy(h_out, (const uint8_t*)c->atlas_dev[level] + (uint64_t)(slot + 1) * lv.map_bytes, lv.map_bytes, cudaMemcpyDeviceToHost));   // + 1: the zero map

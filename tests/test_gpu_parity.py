@@ -627,3 +627,43 @@ def test_presort_auto_follows_the_coherence_of_the_queries(P):
     fi_pipe = ctx.oo_encode(xi, wi, want_debug=True)
     assert ctx.oo_get_info()["encode_pipelined_last"] == 1
     assert all(torch.equal(a, b) for a, b in zip(fi_pipe, fi_fast))  # features, slots and base texels, bit for bit
+
+
+def test_default_presort_policy_is_capturable_into_a_cuda_graph(P):
+    """OO_PRESORT_AUTO is the default, so a caller who captures oo_query / oo_encode into a CUDA graph gets its sampling too.  The
+    side-stream copy of the samples must not be pulled into the capture (it would never rejoin and capture_end would fail with
+    cudaErrorStreamCaptureUnjoined): a captured call enqueues its kernels only.  Replays give the eager bytes, for the unsorted
+    and for the binned decision, and eager calls after the capture still sample."""
+    w = gen.scene_workload(1, width=512, height=512)
+    qc = w.queries
+    qi = gen.incoherent_queries(w.scene, qc.n, 0)
+    ctx = P.OctaOctree(0).upload_workload(w)
+    ctx.oo_reserve(qc.n)
+    xc, nc, wc, _ = _dev(qc)
+    xi, ni, wi, _ = _dev(qi)
+    for (x, n, wo), binned in (((xc, nc, wc), 0), ((xi, ni, wi), 1)):
+        for _ in range(3):                                           # eager calls: configure the kernels, let AUTO settle
+            ref = ctx.oo_query(x, n, wo)
+            torch.cuda.synchronize()
+        assert ctx.oo_get_info()["presorted_last_query"] == binned
+        f_ref = ctx.oo_encode(x, wo)
+        torch.cuda.synchronize()
+        rgb, feat = torch.zeros_like(ref), torch.zeros_like(f_ref)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):                                    # capture_end raises if a stream was left unjoined
+            ctx.oo_query(x, n, wo, rgb=rgb)
+            ctx.oo_encode(x, wo, features=feat)
+        assert ctx.oo_get_info()["presorted_last_query"] == binned
+        for _ in range(2):
+            rgb.zero_()
+            feat.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(rgb, ref) and torch.equal(feat, f_ref)
+        del g
+    # the context is as usable as before: eager calls sample again and the decision follows them back to "coherent"
+    for _ in range(3):
+        ctx.oo_query(xc, nc, wc)
+        torch.cuda.synchronize()
+    info = ctx.oo_get_info()
+    assert info["presorted_last_query"] == 0 and info["presort_auto_on"] == 0, info
