@@ -312,6 +312,7 @@ def run_dry_dist(args):
     (mx,), (tot, chk) = D.reduce_max_sum([1.0 + rank], [mine, checksum if args.scaling == "weak" else 0.0], torch.device("cpu"))
     if rank == 0:
         print(json.dumps({"dry_run": True, "n_gpus": world, "scaling": args.scaling, "queries": int(tot), "frame": n_frame,
+                          "dist_ranks": torch.distributed.get_world_size() if world > 1 else None,
                           "max_ms": mx, "checksum": checksum if args.scaling == "strong" else chk}))
     if world > 1:
         torch.distributed.destroy_process_group()
@@ -413,6 +414,19 @@ def run_ours(args):
                                        "frac": bq * n_mine / (mean_ms * 1e-3) / 1e9 / hbm, "bytes_per_query": bq, "peak_source": which}}))
         return 0
     checksum_dev = float((frame[0] if strong else rgb).double().sum())
+    strong_ok = None
+    if strong:
+        # outside the timed region: every rank evaluates the WHOLE frame alone (the cache is replicated) and compares it with the frame the
+        # all-gather assembled.  RGB per query does not depend on the sharding, so the two are equal bit for bit; a run where they are not
+        # fails on every rank at once (no rank is left waiting in a collective).
+        cuf = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+        alone = ctx.oo_query(cuf(q.x), cuf(q.nrm), cuf(q.wo), cuf(q.extra))
+        torch.cuda.synchronize(dev)
+        strong_ok = bool(torch.equal(alone, frame[0]))
+        if not strong_ok:
+            raise SystemExit("bench.py: rank %d: the all-gathered frame differs from the same frame evaluated on one rank "
+                             "(checksums %r vs %r)" % (rank, checksum_dev, float(alone.double().sum())))
+        del alone
     # e2e: pinned host buffers, H2D + kernels + D2H inside the timed region, through oo_query_host
     pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a[lo:hi])).pin_memory()
     hx, hn, hw, he = pin(q.x), pin(q.nrm), pin(q.wo), pin(q.extra)
@@ -504,7 +518,8 @@ def run_ours(args):
         "data": "synthetic", "config": desc,
         "run": {"l2": "flushed between steps (256 MB memset)", "path": PATH_NAMES[info["path_last_query"]], "ms_per_frame_warm_l2": mx_warm,
                 "presort": args.presort, "presorted": bool(info["presorted_last_query"]), "coherence_distinct_cells_per_32_queries": info["coherence_x100"] / 100.0,
-                "queries_per_rank": n_mine, "checksum_device": checksum_dev,
+                "queries_per_rank": n_mine, "checksum_device": checksum_dev, "strong_checksum_matches_one_rank": strong_ok,
+                "nccl_ranks": torch.distributed.get_world_size() if world > 1 else None,
                 "parallelism": ("one GPU" if world == 1 else
                                 "replicated cache; ONE frame split into contiguous query slices, RGB all-gathered over NCCL inside the timed region" if strong else
                                 "replicated cache; every rank its own frame (camera seed = rank); no data-path collective")},

@@ -1,4 +1,4 @@
-"""Multi-GPU plumbing (DESIGN.md §7): the path shards trivially — queries are independent, the cache is read-only and
+"""Multi-GPU plumbing (DESIGN.md §10): the path shards trivially — queries are independent, the cache is read-only and
 replicated — so there is no data-path collective.  These helpers only split work and reduce timings."""
 from __future__ import annotations
 

@@ -63,12 +63,13 @@ def test_bench_gpus_n_from_a_plain_shell_starts_n_ranks():
     assert one["n_gpus"] == 1 and one["queries"] == one["frame"]
     weak = _bench("--gpus", "2", "--dry-run-dist")
     assert weak["n_gpus"] == 2 and weak["scaling"] == "weak" and weak["queries"] == 2 * one["frame"] and weak["max_ms"] == 2.0
+    assert one["dist_ranks"] is None and weak["dist_ranks"] == 2          # what the process group itself reports, not the flag
     assert weak["checksum"] != 2 * one["checksum"]        # rank 1 rendered its own frame, not a copy of rank 0's
     strong = _bench("--gpus", "2", "--dry-run-dist", "--scaling", "strong")
     assert strong["n_gpus"] == 2 and strong["scaling"] == "strong" and strong["queries"] == one["frame"]
     assert strong["checksum"] == one["checksum"]
     three = _bench("--gpus", "3", "--dry-run-dist", "--scaling", "strong")      # ragged shards
-    assert three["n_gpus"] == 3 and three["checksum"] == one["checksum"]
+    assert three["n_gpus"] == 3 and three["checksum"] == one["checksum"] and three["dist_ranks"] == 3
 
 
 def test_traffic_json_is_refused_when_the_kernel_sources_changed(tmp_path, monkeypatch):
