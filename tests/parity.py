@@ -18,11 +18,24 @@ def check_indices(slot_gpu, tex_gpu, slot_ref, tex_ref):
     assert np.array_equal(np.asarray(tex_gpu, np.int64), np.asarray(tex_ref, np.int64)), "texel indices differ"
 
 
-def check_features(f_gpu, f_ref, storage="f16"):
+def feature_bound(max_abs_texel):
+    """What the GPU's arithmetic can add to a feature of fp16 texels with |texel| <= M, derived:
+      * the four bilinear weights are rounded to fp16 before the FHFMA: they are in [0, 1] and sum to 1, so at most one is >= 1/2
+        (half-ulp 2^-12), at most one more >= 1/4 (2^-13), the rest < 1/4 (<= 2^-14 each): sum of |dw| <= 2^-11, times M;
+      * the fp32 accumulation of four products adds ~4 * 2^-24 * M: nothing at this scale;
+      * oo_encode stores the feature rounded once to fp16: |h| <= M, so <= 2^-11 * M.
+    Total <= 2^-10 * M.  For the BASELINE.json recipe (N(0, 0.1): M ~ 0.57 over 1e8 texels) that is 5.6e-4, inside north_star's
+    1e-3; for texels of O(1) the 1e-3 bar cannot hold for ANY fp16 feature row (the store rounding alone reaches it at |h| >= 2),
+    and this bound takes its place.  The blended full query (Eq. 10: convex combination of such values, fp32 out) obeys it too."""
+    return 2.0 ** -10 * float(max_abs_texel) + 1e-6
+
+
+def check_features(f_gpu, f_ref, storage="f16", atol=None):
     f_gpu = np.asarray(f_gpu, np.float64)
     err = np.abs(f_gpu - f_ref)
     # the stored feature is rounded once to the tree dtype: fp16 spacing is 2^-11 relative, well inside 1e-3 for |h| < 1
-    assert err.max() <= FEATURE_ATOL, "feature max-abs error %.3g > %.3g" % (err.max(), FEATURE_ATOL)
+    atol = FEATURE_ATOL if atol is None else atol
+    assert err.max() <= atol, "feature max-abs error %.3g > %.3g" % (err.max(), atol)
     return float(err.max())
 
 

@@ -1,5 +1,6 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times (config 1: every query against
-the C oracle; config 3: the full 10 M-node / multi-GB atlas, oracle on a sample of queries)."""
+the C oracle; config 3: the full 10 M-node / multi-GB atlas, every one of its 4 M queries against the C oracle; config 4: every query
+at 2^20, every 16th at 2^22 and 2^24; the paper's shapes: 65,536 queries of the frame against the numpy oracle of the full query)."""
 import numpy as np
 import pytest
 
@@ -13,6 +14,29 @@ torch = pytest.importorskip("torch")
 
 def _dev(a):
     return None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+CHUNK = 1 << 19
+
+
+def _oracle_on_every_query(co, q, rgb, slot, texel, feat):
+    """RGB, slots, base texels and feature rows (host arrays, any may be None) of EVERY query of q against the C oracle, a chunk at
+    a time: the oracle's fp64 feature rows of a whole 4 M-query frame would be 2.7 GB.  The RGB bars are applied per chunk (so the
+    mean-abs bar holds on every 2^19 queries, not only on the whole).  Returns the worst max-abs / mean-abs RGB error."""
+    worst = [0.0, 0.0]
+    for lo in range(0, q.n, CHUNK):
+        sl = slice(lo, min(lo + CHUNK, q.n))
+        if rgb is not None:
+            ref = co.query(q.x[sl], q.nrm[sl], q.wo[sl], None if q.extra is None else q.extra[sl])
+            mx, mean = check_rgb(rgb[sl], ref)
+            worst = [max(worst[0], mx), max(worst[1], mean)]
+        if slot is not None or feat is not None:
+            f, s, t = co.encode(q.x[sl], q.wo[sl])
+            if slot is not None:
+                check_indices(slot[sl], texel[sl], s, t)
+            if feat is not None:
+                check_features(feat[sl].astype(np.float32), f)
+    return worst
 
 
 def test_config1_full_frame_all_queries():
@@ -71,46 +95,49 @@ def test_config2_full_frame_all_queries():
     print("cfg2 full: rgb max-abs %.3g mean-abs %.3g" % (mx, mean))
 
 
-def test_config3_full_tree_sampled_queries():
+def test_config3_full_tree_all_queries():
+    """configs[3] at full size ("cfg3: all 4 M queries for parity"): RGB of the timed kernel, the indices out of its debug
+    instance, and oo_encode's feature rows and indices, EVERY one of the 4,194,304 queries against the C oracle."""
     import paper_2606_08469_b200 as P
     w = gen.scene_workload(3, width=2048, height=2048)
     assert w.tree.n_nodes > 5_000_000 and w.atlas.nbytes > 4e9
     q = w.queries
+    assert q.n == 1 << 22
     ctx = P.OctaOctree(0).upload_workload(w)
     x, n, wo = _dev(q.x), _dev(q.nrm), _dev(q.wo)
     got = ctx.oo_query(x, n, wo)
     torch.cuda.synchronize()
-    got = got.cpu().numpy()
-    idx = np.arange(0, q.n, 61)                                  # ~69 k sampled queries across the whole frame
-    qs = q.take(idx)
+    assert ctx.oo_get_info()["path_last_query"] == P.PATH_FUSED_TC_TMEM
     co = OC.from_workload(w)
-    ref = co.query(qs.x, qs.nrm, qs.wo)
-    check_rgb(got[idx], ref)
-    f, s, t = co.encode(qs.x, qs.wo)
-    fe, sl, tx = ctx.oo_encode(_dev(qs.x), _dev(qs.wo), want_debug=True)
-    check_indices(sl.cpu().numpy(), tx.cpu().numpy(), s, t)
-    check_features(fe.float().cpu().numpy(), f)
-    # ALL 4 M queries: the timed kernel's own indices (its debug instance) against oo_encode's kernel bit for bit -- two different
-    # descents (pipelined hop chain vs descend_plan), both checked against the oracle on the sample above -- and its RGB against
-    # a second CUDA path (features through HBM + the mma.sync MLP) within the north-star bars
     ctx.oo_reserve(q.n)
-    rgb_d, s_d, t_d = ctx.oo_query_debug(x, n, wo)
-    assert torch.equal(rgb_d, torch.from_numpy(got).cuda())
-    _, s_e, t_e = ctx.oo_encode(x, wo, want_debug=True)
+    rgb_d, s_d, t_d = ctx.oo_query_debug(x, n, wo)                # the timed kernel's own indices (its debug instance)
+    assert torch.equal(rgb_d, got)
+    fe, s_e, t_e = ctx.oo_encode(x, wo, want_debug=True)          # a different descent (descend_plan), and the feature rows
     assert torch.equal(s_d, s_e) and torch.equal(t_d, t_e)
-    check_indices(s_d[::61].cpu().numpy(), t_d[::61].cpu().numpy(), s, t)
-    del s_e, t_e, s_d, t_d
+    del rgb_d, s_e, t_e
+    got = got.cpu().numpy()
+    mx, mean = _oracle_on_every_query(co, q, got, s_d.cpu().numpy(), t_d.cpu().numpy(), fe.cpu().numpy())
+    print("cfg3 full, all %d queries: rgb max-abs %.3g mean-abs %.3g" % (q.n, mx, mean))
+    del s_d, t_d, fe
+    # and a second CUDA path (features through HBM + the mma.sync MLP) within the north-star bars
     ctx.oo_set_path(P.PATH_UNFUSED)
     second = ctx.oo_query(x, n, wo).cpu().numpy()
     ctx.oo_set_path(P.PATH_AUTO)
     check_rgb(got, second.astype(np.float64))
     del second
-    # incoherent distribution (config 4) on the same tree
-    qi = gen.incoherent_queries(w.scene, 1 << 16, 0)
-    ref = co.query(qi.x, qi.nrm, qi.wo)
-    check_rgb(ctx.oo_query(_dev(qi.x), _dev(qi.nrm), _dev(qi.wo)).cpu().numpy(), ref)
+    # incoherent distribution (config 4) on the same tree: S:539 "all queries for N <= 2^20"
+    qi = gen.incoherent_queries(w.scene, 1 << 20, 0)
+    xi, ni, wi = _dev(qi.x), _dev(qi.nrm), _dev(qi.wo)
+    ctx.oo_set_presort("none")
+    rgb_i, s_i, t_i = ctx.oo_query_debug(xi, ni, wi)
+    f_i = ctx.oo_encode(xi, wi)
+    ctx.oo_set_presort("bin")
+    assert torch.equal(ctx.oo_query(xi, ni, wi), rgb_i) and ctx.oo_get_info()["presorted_last_query"] == 1
+    mx, mean = _oracle_on_every_query(co, qi, rgb_i.cpu().numpy(), s_i.cpu().numpy(), t_i.cpu().numpy(), f_i.cpu().numpy())
+    print("cfg4 2^20 incoherent, all queries: rgb max-abs %.3g mean-abs %.3g" % (mx, mean))
+    del rgb_i, s_i, t_i, f_i
     # config 4 as bench.py --sweep 4 times it: 2^22 incoherent queries, unsorted and with OO_PRESORT_BIN at its default
-    # threshold; the oracle on every 61st query, the two launches against each other on all of them
+    # threshold; the oracle on every 16th query, the two launches against each other on all of them
     qi = gen.incoherent_queries(w.scene, 1 << 22, 0)
     xi, ni, wi = _dev(qi.x), _dev(qi.nrm), _dev(qi.wo)
     ctx.oo_set_presort("none")
@@ -120,14 +147,15 @@ def test_config3_full_tree_sampled_queries():
     binned = ctx.oo_query(xi, ni, wi)
     assert ctx.oo_get_info()["presorted_last_query"] == 1
     assert torch.equal(plain, binned)
-    idx = np.arange(0, qi.n, 61)
+    idx = np.arange(0, qi.n, 16)
     qs = qi.take(idx)
-    check_rgb(binned.cpu().numpy()[idx], co.query(qs.x, qs.nrm, qs.wo))
     fb = ctx.oo_encode(xi, wi)
     assert ctx.oo_get_info()["presorted_last_encode"] == 1
     ctx.oo_set_presort("none")
     assert torch.equal(fb, ctx.oo_encode(xi, wi))
-    check_features(fb[torch.from_numpy(idx).cuda()].float().cpu().numpy(), co.encode(qs.x, qs.wo)[0])
+    _oracle_on_every_query(co, qs, binned.cpu().numpy()[idx], None, None, None)
+    f_ref = np.concatenate([co.encode(qs.x[k:k + CHUNK], qs.wo[k:k + CHUNK])[0] for k in range(0, qs.n, CHUNK)])
+    check_features(fb[torch.from_numpy(idx).cuda()].float().cpu().numpy(), f_ref)
 
 
 def test_paper_shapes_full_frame_sampled_queries():
@@ -148,7 +176,7 @@ def test_paper_shapes_full_frame_sampled_queries():
     feat, slots, _ = ctx.oo_encode_full(x, n, wo, dd, want_debug=True)
     torch.cuda.synchronize()
     assert ctx.oo_get_info()["path_last_query"] == P.PATH_FULL
-    idx = np.arange(0, q.n, 127)                                   # ~8 k queries across the whole frame
+    idx = np.arange(0, q.n, 16)                                    # 65,536 queries across the whole frame
     qs = q.take(idx)
     mode = FO.Mode("trilinear8", "vertex", "shifted", "paper")
     ref_f, ref_s = FO.encode_full(w.tree, w.atlas.levels, qs.x, qs.nrm, qs.wo, mode, d[idx], return_debug=True)
@@ -168,7 +196,7 @@ def test_paper_shapes_full_frame_sampled_queries():
 def test_config4_2pow24_queries(dist):
     """configs[4] at its largest batch, 2^24 queries on the config-3 cache, as bench.py --sweep 4 times it: the coherent
     stream (screen-order hits of a 4096x4096 frame) and the incoherent one (area-weighted surface samples, random order).
-    The oracle on a stride sample; the unsorted and the OO_PRESORT_BIN call against each other on all 16.8 M queries, bit
+    The oracle on every 16th query (1 M of them); the unsorted and the OO_PRESORT_BIN call against each other on all 16.8 M queries, bit
     for bit; the fused kernel's own indices against oo_encode's on all of them."""
     import paper_2606_08469_b200 as P
     w = gen.scene_workload(3, seed=0, width=64, height=64)
@@ -187,16 +215,15 @@ def test_config4_2pow24_queries(dist):
     assert torch.equal(plain, binned)
     del binned
     ctx.oo_set_presort("none")
-    idx = np.arange(0, n, 251)                                   # ~67 k queries across the whole batch
+    idx = np.arange(0, n, 16)                                    # "a stride-16 subsample of the 2^24 batch" = 1,048,576 queries
     qs = q.take(idx)
     co = OC.from_workload(w)
-    mx, mean = check_rgb(plain.cpu().numpy()[idx], co.query(qs.x, qs.nrm, qs.wo))
-    f, s, t = co.encode(qs.x, qs.wo)
     rgb_d, s_d, t_d = ctx.oo_query_debug(x, nr, wo)
     assert torch.equal(rgb_d, plain)
     del rgb_d
-    check_indices(s_d[::251].cpu().numpy(), t_d[::251].cpu().numpy(), s, t)
     fe, s_e, t_e = ctx.oo_encode(x, wo, want_debug=True)
     assert torch.equal(s_d, s_e) and torch.equal(t_d, t_e)
-    check_features(fe[::251].float().cpu().numpy(), f)
+    del s_e, t_e
+    mx, mean = _oracle_on_every_query(co, qs, plain.cpu().numpy()[idx], s_d[::16].cpu().numpy(), t_d[::16].cpu().numpy(),
+                                      fe[::16].cpu().numpy())
     print("cfg4 2^24 %s: rgb max-abs %.3g mean-abs %.3g on %d sampled queries" % (dist, mx, mean, len(idx)))
