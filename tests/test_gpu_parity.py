@@ -151,6 +151,83 @@ def test_direction_magnitudes_and_tiny_components(P):
     ctx.close()
 
 
+def _adversarial_directions(kind, n, rng):
+    """fp32 directions [n][3] aimed at the places where a hand-rolled division could differ from IEEE."""
+    base = rng.standard_normal((n, 3))
+    rows = np.arange(n)
+    if kind == 0:      # anything, anywhere in the range (A22: wo is not normalised)
+        wo = base * np.ldexp(1.0, rng.integers(-70, 71, n))[:, None]
+    elif kind == 1:    # the edges of div2_rn's fast-path window: S around 2^+-60, or one of wx, wy around 2^-60 under a moderate S
+        unit = base / np.abs(base).max(axis=1, keepdims=True)
+        m = rng.choice([1.0, 1.0 + 2.0 ** -23, 2.0 - 2.0 ** -23, 1.5], n)
+        wo = unit * (m * np.ldexp(1.0, rng.choice([-61, -60, -59, 59, 60, 61], n)))[:, None]
+        small = np.ldexp(rng.choice([1.0, 1.0 + 2.0 ** -23, 1.0 - 2.0 ** -24], n), -60) * rng.choice([-1.0, 1.0], n)
+        wo2 = base.copy()
+        wo2[rows, rng.integers(0, 2, n)] = small
+        wo = np.where((rng.random(n) < 0.5)[:, None], wo, wo2)
+    elif kind == 2:    # denormals: every component, or all but one
+        wo = base * np.ldexp(1.0, rng.integers(-149, -120, n))[:, None]
+        keep = rng.random(n) < 0.5
+        big = rng.integers(0, 3, n)
+        wo[rows[keep], big[keep]] = base[rows[keep], big[keep]]
+    elif kind == 3:    # u exactly on a texel boundary of every map resolution up to 64 (u = k/64), both hemispheres, then scaled by
+        kx, ky = rng.integers(-64, 65, n), rng.integers(-64, 65, n)    # factors that are not powers of two and nudged by one ulp
+        out = np.abs(kx) + np.abs(ky) > 64
+        fx = np.where(out, np.sign(kx) * (64 - np.abs(ky)), kx)
+        fy = np.where(out, np.sign(ky) * (64 - np.abs(kx)), ky)
+        ux, uy = fx / 64.0, fy / 64.0
+        z = (1.0 - np.abs(ux) - np.abs(uy)) * rng.choice([-1.0, 1.0], n)
+        scale = np.where(rng.random(n) < 0.3, 1.0, rng.uniform(1.0, 2.0, n)) * np.ldexp(1.0, rng.integers(-40, 41, n))
+        wo = (np.stack([ux, uy, z], 1) * scale[:, None]).astype(np.float32)
+        nudge = rng.random(n) < 0.4
+        c = rng.integers(0, 3, n)
+        wo[rows[nudge], c[nudge]] = np.nextafter(wo[rows[nudge], c[nudge]], np.where(rng.random(nudge.sum()) < 0.5, np.float32(-np.inf), np.float32(np.inf)))
+    else:              # near-ties in S = (|wx| + |wy|) + |wz|: full mantissas, exponents 1..25 apart, exact half-ulp cases among them
+        e = rng.integers(-30, 31, n)
+        mant = 1.0 + rng.integers(0, 1 << 23, (n, 3)) * 2.0 ** -23
+        mant[rng.random((n, 3)) < 0.2] = 1.0
+        gap = np.stack([np.zeros(n, np.int64), rng.integers(1, 26, n), rng.integers(1, 26, n)], 1)
+        wo = mant * np.ldexp(1.0, e[:, None] - gap) * rng.choice([-1.0, 1.0], (n, 3))
+        wo = wo[rows[:, None], np.argsort(rng.random((n, 3)), axis=1)]                  # the large component in any position
+    wo = np.asarray(wo, np.float32)
+    dead = ~np.isfinite(wo).all(axis=1) | (np.abs(wo).max(axis=1) == 0)
+    wo[dead] = (0.0, 0.0, 1.0)
+    return wo
+
+
+def test_division_contract_on_2pow26_directions(P):
+    """The base-texel decision divides by the L1 norm; the kernels share one refined reciprocal between the two divisions (div2_rn,
+    oo_device.cuh) and claim the bits of IEEE division.  In-tree evidence: 2^26 directions -- random over the whole exponent range, at
+    the edges of div2_rn's fast-path window, denormal, exactly on (and one ulp beside) texel boundaries, and with near-tie L1 sums --
+    through oo_encode's specialised and generic kernels, base texels of all four map resolutions against the oracle's fp32 decision
+    (numpy, IEEE division), bit for bit."""
+    w = gen.scene_workload(1, width=64, height=64)
+    ctx = P.OctaOctree(0).upload_workload(w)
+    n = 1 << 22
+    ctx.oo_reserve(n)
+    ctx.oo_set_presort("none")
+    rng = np.random.default_rng(2606)
+    x = torch.from_numpy(gen.u01(7, 1, 3 * n).reshape(-1, 3).astype(np.float32)).cuda()
+    feat = torch.empty((n, 32), dtype=torch.float16, device="cuda")
+    total = 0
+    for chunk in range(16):
+        wo = _adversarial_directions(chunk % 5, n, rng)
+        wo_d = torch.from_numpy(wo).cuda()
+        ref = np.stack([np.stack(O.texel_base_f32(wo, R), -1) for R in w.tree.level_res], 1).astype(np.int16)      # [n][L][2]
+        ref_d = torch.from_numpy(ref).cuda()
+        for path in (P.PATH_UNFUSED, P.PATH_GENERIC) if chunk < 5 else (P.PATH_UNFUSED,):
+            ctx.oo_set_path(path)
+            _, _, t = ctx.oo_encode(x, wo_d, features=feat, want_debug=True)
+            bad = (t != ref_d).any(dim=2).any(dim=1)
+            if bool(bad.any()):
+                i = int(bad.nonzero()[0])
+                raise AssertionError("family %d, path %d: direction %r gives base texels %r, the oracle %r" %
+                                     (chunk % 5, path, wo[i].tolist(), t[i].tolist(), ref[i].tolist()))
+        total += n
+    assert total == 1 << 26
+    ctx.close()
+
+
 def test_non_canonical_levels_fall_back_to_generic(P):
     """Used depths {1, 8}: 8 is more than 3 levels below the top station (depth 4), so there is no hop plan; AUTO must
     run the generic kernels and still match."""
