@@ -33,6 +33,22 @@ def test_binding_mirrors_the_abi():
         assert callable(getattr(P.OctaOctree, n))
 
 
+def test_static_sort_refuses_oversize_batches_before_touching_cuda():
+    """oo_sort_queries_static checks n against its built-in scratch before any CUDA call, so the refusal (status, message that names
+    the limit) can be checked without a GPU; the header's constant, the binding's and the library's agree."""
+    import paper_2606_08469_b200 as P
+    hdr = open(os.path.join(ROOT, "include", "oo.h")).read()
+    limit = int(re.search(r"#define\s+OO_SORT_STATIC_MAX_QUERIES\s+(\d+)u", hdr).group(1))
+    assert limit == P.SORT_STATIC_MAX_QUERIES == 1 << 20
+    L = P.load_library()
+    err = ctypes.create_string_buffer(256)
+    st = L.oo_sort_queries_static(None, limit + 1, None, None, err, len(err))
+    assert st == 3 and b"OO_SORT_STATIC_MAX_QUERIES" in err.value and str(limit).encode() in err.value
+    assert L.oo_sort_queries_static(None, 1 << 40, None, None, None, 0) == 3          # no message buffer: status only
+    short = ctypes.create_string_buffer(8)                                              # a short buffer is filled and terminated, not overrun
+    assert L.oo_sort_queries_static(None, limit + 1, None, None, short, len(short)) == 3 and len(short.value) == 7
+
+
 def test_product_never_imports_the_oracle():
     pkg = os.path.join(ROOT, "paper_2606_08469_b200")
     for dp, _, files in os.walk(pkg):
